@@ -1,0 +1,161 @@
+/* sparse_sketch.h -- C ABI of the B200 (sm_100a) sparse-sketch library.
+ *
+ * The library forms B = S*A for a tall FP32 row-major matrix A (m x n, m >> n)
+ * under CountSketch (zeta = 1) and SparseStack (zeta stacked CountSketch blocks
+ * of d/zeta rows each, entries +-1/sqrt(zeta)):
+ *     PAPER.md:59-65, Eq. (1)  (arxiv 2606.20195, Sec. II-A).
+ * The bucket / sign map is the counter hash fixed by BASELINE.json:north_star
+ * (instantiating PAPER.md:59; readings R1-R4 in DESIGN.md):
+ *     h       = splitmix64(seed ^ (i*zeta + j))        i = global row, j = block, 0-based
+ *     bucket  = j*(d/zeta) + (((h >> 32) * (d/zeta)) >> 32)
+ *     signbit = h & 1                                   0 -> +1, 1 -> -1
+ *
+ * Conventions for every entry point
+ *   - returns SKETCH_OK (0) or a negative SKETCH_ERR_* code; never throws, never aborts;
+ *   - "dev" pointers are CUDA device pointers on the current device, "host" pointers are
+ *     host memory; the caller owns every buffer and the stream it passes; the library owns
+ *     the handle, its scratch (replicated partial sketches, optional packed hash array,
+ *     staging buffers) and frees them in sketch_destroy;
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  apply/dump calls
+ *     are asynchronous on that stream and never synchronise, except the first call that has
+ *     to grow a scratch buffer (cudaMalloc) and the *_host entry points (which return after
+ *     the result is in host memory);
+ *   - A is never modified; one handle may be applied to any number of matrices with any n
+ *     (S is d x m, independent of n), e.g. A in FP16 and b in FP32 with the same map as in
+ *     PAPER.md:356 / Table I.
+ *   - a handle must not be used from two host threads at once.
+ */
+#ifndef SPARSE_SKETCH_H_
+#define SPARSE_SKETCH_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sketch sketch_t; /* opaque, library-owned */
+
+/* error codes */
+#define SKETCH_OK 0
+#define SKETCH_ERR_INVALID (-1)     /* m<=0, d<=0, zeta<1, n<=0, rows<0, row range outside [0,m), bad enum */
+#define SKETCH_ERR_NULL (-2)        /* a required pointer is NULL */
+#define SKETCH_ERR_DIVISIBILITY (-3)/* d % zeta != 0 ("Let d be divisible by zeta") */
+#define SKETCH_ERR_LDA (-4)         /* lda < n */
+#define SKETCH_ERR_ALIGNMENT (-5)   /* A not 4-byte, B not 2-byte (f16) / 4-byte (f32) aligned */
+#define SKETCH_ERR_UNSUPPORTED (-6) /* the forced variant cannot run this shape (AUTO never returns it) */
+#define SKETCH_ERR_CUDA (-7)        /* CUDA runtime error; text via sketch_last_error() */
+#define SKETCH_ERR_NOMEM (-8)       /* host or device allocation failed */
+
+/* conversion rule of the FP16 path (Sec. III-D) */
+#define SKETCH_RN 0 /* round-to-nearest-even, __float2half semantics */
+#define SKETCH_SR 1 /* stochastic conversion with counter-based bits (readings R13, R14) */
+
+/* kernel variants (all compute the same sums; they differ in where partial sums live) */
+#define SKETCH_VARIANT_AUTO 0      /* chosen per shape from measurement */
+#define SKETCH_VARIANT_FLAT_PAIR 1 /* paper's Listing 1/2 restated: one column (f32) / column pair (f16) per
+                                      lane, one result-discarding RED per contribution */
+#define SKETCH_VARIANT_FLAT_VEC 2  /* widest vector RED the shape allows (16-byte REDG: 8 halves / 4 floats) */
+#define SKETCH_VARIANT_SMEM 3      /* shared-memory-privatised partial sketch per CTA, flushed with vector RED */
+#define SKETCH_VARIANT_GENERIC 4   /* any n / any alignment scalar fallback (one lane per element) */
+
+typedef struct sketch_opts {
+  int32_t variant;    /* SKETCH_VARIANT_* */
+  int32_t replicas;   /* FLAT variants: number P of L2-resident partial sketches the CTAs are spread over,
+                         summed by a reduce kernel (0 = auto, 1 = RED straight into B) */
+  int32_t hash_mode;  /* 0 = auto, 1 = hash on the fly inside the scatter kernel, 2 = read the packed array
+                         built by sketch_precompute_hashes (built on demand) */
+  int32_t accumulate; /* 0 = complete sketch: B is zero-initialised by the call;
+                         1 = add this row range's contributions into the existing B */
+  int64_t row_begin;  /* global index of the first row stored at A (rows are hashed by global index) */
+  int64_t rows;       /* number of rows at A; 0 = m - row_begin */
+  int32_t grid_ctas;  /* 0 = auto; tuning / tests only */
+  int32_t reserved;   /* must be 0 */
+} sketch_opts_t;
+
+/* ---- handle ------------------------------------------------------------------------------- */
+
+/* Create the sketch S in R^{d x m} with zeta nonzeros per column.
+ * m: rows of the matrices it will be applied to; d: sketch rows, d % zeta == 0; seed: full 64 bits
+ * (use full-width seeds: seeds that differ only in low bits alias, R15).
+ * *out receives the handle.  No device memory is allocated here. */
+int sketch_create(int64_t m, int32_t d, int32_t zeta, uint64_t seed, sketch_t** out);
+
+/* Free the handle and all library-owned device/host scratch.  NULL is accepted. */
+int sketch_destroy(sketch_t* s);
+
+/* ---- hash stage ------------------------------------------------------------- */
+
+/* Write bucket[i*zeta + j] (int32, in [j*d/zeta, (j+1)*d/zeta)) and signbit[i*zeta + j] (uint8, the raw
+ * h & 1) for all i in [0,m), j in [0,zeta) to DEVICE buffers of m*zeta elements each. */
+int sketch_hashes_dump(const sketch_t* s, int32_t* bucket_dev, uint8_t* signbit_dev, void* stream);
+
+/* Build (once) the packed per-(row,block) hash array the hash_mode=2 kernels read:
+ * uint16 = bucket | signbit<<15 when d <= 32768, else uint32 = bucket | signbit<<31; m*zeta entries,
+ * library-owned.  Counted in "complete sketch" time by bench.py when that mode is used. */
+int sketch_precompute_hashes(sketch_t* s, void* stream);
+
+/* ---- scatter kernels ------------------------------------------------- */
+
+/* FP32-accumulate baseline (Listing 1; Table I "FP32 path").
+ * A_dev: m x n FP32 row-major with leading dimension lda >= n (elements); B_dev: d x n FP32 row-major
+ * (leading dimension n), overwritten with S*A.  Products and sums are FP32; the global RED used for
+ * FP32 flushes FP32 subnormals (SASS REDG.E.ADD.F32.FTZ). */
+int sketch_apply_f32acc(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, float* B_dev,
+                        void* stream);
+
+/* FP16-accumulate path (PAPER.md:114-136, Listing 2; :140-165; :175-187): per contribution
+ * p = fp32(+-s * a), v = RN16(p) (or SR16), B16[bucket, c] = RN16(B16[bucket, c] + v), each FP16 component
+ * independently, subnormals kept (.noftz), overflow -> +-inf.  The order of the additions is unspecified
+ * ("Parallel atomic updates may also realize different orders").
+ * B_dev: d x n IEEE binary16 row-major, overwritten.  rounding: SKETCH_RN / SKETCH_SR; sr_seed is used
+ * only for SR.  Any n >= 1 is accepted (odd n runs the scalar GENERIC variant). */
+int sketch_apply_f16acc(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev,
+                        int rounding, uint64_t sr_seed, void* stream);
+
+/* Same, with explicit options (variant override, row range, accumulate-into-B).  opts == NULL means
+ * all-zero options, i.e. exactly the calls above. */
+int sketch_apply_f32acc_ex(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, float* B_dev,
+                           const sketch_opts_t* opts, void* stream);
+int sketch_apply_f16acc_ex(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev,
+                           int rounding, uint64_t sr_seed, const sketch_opts_t* opts, void* stream);
+
+/* End-to-end entry points with HOST buffers: A_host (m x n, lda) is streamed to the device in row chunks
+ * through two library-owned staging buffers (copy of chunk k+1 overlaps the kernels of chunk k), sketched
+ * with the kernels above (row_begin / accumulate), and B_host (d x n) is written before the call returns.
+ * Pinned (page-locked) host memory is needed for the copies to overlap; pageable memory works, slower. */
+int sketch_apply_f32acc_host(const sketch_t* s, const float* A_host, int32_t n, int64_t lda,
+                             float* B_host, const sketch_opts_t* opts);
+int sketch_apply_f16acc_host(const sketch_t* s, const float* A_host, int32_t n, int64_t lda, void* B_host,
+                             int rounding, uint64_t sr_seed, const sketch_opts_t* opts);
+
+/* ---- measurement support ------------------------------------------------------------------- */
+
+/* L2 atomic-throughput probe (the second term of the roofline): issues `iters` rounds of
+ * result-discarding REDs with the scatter kernels' address pattern (a random bucket row per lane group,
+ * consecutive lanes on consecutive columns of a d x n sketch) from register values, with no A loads.
+ * kind: 0 = f16x2 (4 B), 1 = v2.f16x2 (8 B), 2 = v4.f16x2 (16 B), 3 = f32 (4 B), 4 = v2.f32, 5 = v4.f32.
+ * sketch_dev: scratch of replicas*d*n*elem bytes.  Asynchronous on `stream`; time it with CUDA events.
+ * *red_ops_out (host, may be NULL) receives the number of lane-level RED operations issued. */
+int sketch_red_probe(void* sketch_dev, int32_t d, int32_t n, int32_t kind, int32_t replicas,
+                     int32_t grid_ctas, int32_t iters, uint64_t* red_ops_out, void* stream);
+
+/* Which variant / replica count / hash mode AUTO resolves to for this shape; host-only, no launch.
+ * is_f16: 1 = f16acc, 0 = f32acc.  Any out pointer may be NULL. */
+int sketch_plan(const sketch_t* s, int32_t n, int64_t lda, int is_f16, int rounding, const sketch_opts_t* opts,
+                int32_t* variant_out, int32_t* replicas_out, int32_t* hash_mode_out, int32_t* grid_out);
+
+/* Number of kernels this library has launched since load (for bench.py's `gpu_launches`). */
+uint64_t sketch_launch_count(void);
+
+/* Static text for a SKETCH_ERR_* code; and the text of the last CUDA error seen by this thread. */
+const char* sketch_strerror(int code);
+const char* sketch_last_error(void);
+
+/* "sparse_sketch <major>.<minor> sm_100a" */
+const char* sketch_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPARSE_SKETCH_H_ */

@@ -1,0 +1,243 @@
+"""ctypes binding of include/sparse_sketch.h -- argument marshalling only.
+
+The method names mirror the C entry points (sketch_create -> Sketch(...), sketch_apply_f16acc ->
+Sketch.apply_f16acc, ...).  Tensors are torch CUDA tensors (device memory + streams are PyTorch's
+job here); only their data pointers, sizes and the current stream handle cross the boundary.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+from . import _build
+
+RN, SR = 0, 1
+VARIANT_AUTO, VARIANT_FLAT_PAIR, VARIANT_FLAT_VEC, VARIANT_SMEM, VARIANT_GENERIC = 0, 1, 2, 3, 4
+VARIANT_NAMES = {0: "auto", 1: "flat_pair", 2: "flat_vec", 3: "smem", 4: "generic"}
+
+
+class SketchOpts(C.Structure):
+    _fields_ = [
+        ("variant", C.c_int32),
+        ("replicas", C.c_int32),
+        ("hash_mode", C.c_int32),
+        ("accumulate", C.c_int32),
+        ("row_begin", C.c_int64),
+        ("rows", C.c_int64),
+        ("grid_ctas", C.c_int32),
+        ("reserved", C.c_int32),
+    ]
+
+
+class SketchError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        detail = lib().sketch_last_error().decode() if code == -7 else ""
+        super().__init__("%s failed: %s (%d) %s" % (where, lib().sketch_strerror(code).decode(), code, detail))
+
+
+_lib = None
+
+# every symbol include/sparse_sketch.h declares: name -> (restype, argtypes)
+_vp, _i32, _i64, _u64, _int = C.c_void_p, C.c_int32, C.c_int64, C.c_uint64, C.c_int
+_OP = C.POINTER(SketchOpts)
+SYMBOLS = {
+    "sketch_create": (_int, [_i64, _i32, _i32, _u64, C.POINTER(_vp)]),
+    "sketch_destroy": (_int, [_vp]),
+    "sketch_hashes_dump": (_int, [_vp, _vp, _vp, _vp]),
+    "sketch_precompute_hashes": (_int, [_vp, _vp]),
+    "sketch_apply_f32acc": (_int, [_vp, _vp, _i32, _i64, _vp, _vp]),
+    "sketch_apply_f16acc": (_int, [_vp, _vp, _i32, _i64, _vp, _int, _u64, _vp]),
+    "sketch_apply_f32acc_ex": (_int, [_vp, _vp, _i32, _i64, _vp, _OP, _vp]),
+    "sketch_apply_f16acc_ex": (_int, [_vp, _vp, _i32, _i64, _vp, _int, _u64, _OP, _vp]),
+    "sketch_apply_f32acc_host": (_int, [_vp, _vp, _i32, _i64, _vp, _OP]),
+    "sketch_apply_f16acc_host": (_int, [_vp, _vp, _i32, _i64, _vp, _int, _u64, _OP]),
+    "sketch_red_probe": (_int, [_vp, _i32, _i32, _i32, _i32, _i32, _i32, C.POINTER(_u64), _vp]),
+    "sketch_plan": (_int, [_vp, _i32, _i64, _int, _int, _OP, C.POINTER(_i32), C.POINTER(_i32), C.POINTER(_i32), C.POINTER(_i32)]),
+    "sketch_launch_count": (_u64, []),
+    "sketch_strerror": (C.c_char_p, [_int]),
+    "sketch_last_error": (C.c_char_p, []),
+    "sketch_version": (C.c_char_p, []),
+}
+
+
+def library_path() -> Path:
+    return _build.LIB
+
+
+def lib() -> C.CDLL:
+    """Load (building in-tree if stale) libsparse_sketch.so; raises if that is impossible."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = C.CDLL(str(path))
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(L, name)  # AttributeError if the library does not export it
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+def sketch_strerror(code: int) -> str:
+    return lib().sketch_strerror(code).decode()
+
+
+def sketch_version() -> str:
+    return lib().sketch_version().decode()
+
+
+def sketch_launch_count() -> int:
+    return int(lib().sketch_launch_count())
+
+
+def _stream_ptr(stream=None) -> int:
+    import torch
+
+    st = stream if stream is not None else torch.cuda.current_stream()
+    return int(st.cuda_stream)
+
+
+def _opts(variant=0, replicas=0, hash_mode=0, accumulate=False, row_begin=0, rows=0, grid_ctas=0):
+    return SketchOpts(int(variant), int(replicas), int(hash_mode), int(bool(accumulate)), int(row_begin), int(rows),
+                      int(grid_ctas), 0)
+
+
+def _check_cuda(t, dtype, what):
+    if not t.is_cuda or t.dtype != dtype:
+        raise TypeError("%s must be a CUDA tensor of dtype %s" % (what, dtype))
+
+
+def sketch_red_probe(scratch, d: int, n: int, kind: int, replicas: int, grid_ctas: int, iters: int, stream=None) -> int:
+    """Launch the L2 atomic-throughput probe; returns the number of lane-level RED ops issued."""
+    ops = _u64(0)
+    rc = lib().sketch_red_probe(scratch.data_ptr(), d, n, kind, replicas, grid_ctas, iters, C.byref(ops), _stream_ptr(stream))
+    if rc:
+        raise SketchError(rc, "sketch_red_probe")
+    return int(ops.value)
+
+
+class Sketch:
+    """Owns one sketch_t handle (sketch_create / sketch_destroy)."""
+
+    def __init__(self, m: int, d: int, zeta: int, seed: int):
+        h = _vp()
+        rc = lib().sketch_create(m, d, zeta, seed & (2**64 - 1), C.byref(h))
+        if rc:
+            raise SketchError(rc, "sketch_create")
+        self._h = h
+        self.m, self.d, self.zeta, self.seed = m, d, zeta, seed
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().sketch_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    # ---- hash stage
+    def hashes_dump(self, stream=None):
+        import torch
+
+        bucket = torch.empty((self.m, self.zeta), dtype=torch.int32, device="cuda")
+        sign = torch.empty((self.m, self.zeta), dtype=torch.uint8, device="cuda")
+        rc = lib().sketch_hashes_dump(self._h, bucket.data_ptr(), sign.data_ptr(), _stream_ptr(stream))
+        if rc:
+            raise SketchError(rc, "sketch_hashes_dump")
+        return bucket, sign
+
+    def precompute_hashes(self, stream=None):
+        rc = lib().sketch_precompute_hashes(self._h, _stream_ptr(stream))
+        if rc:
+            raise SketchError(rc, "sketch_precompute_hashes")
+
+    # ---- device-buffer applies
+    def _A_args(self, A):
+        import torch
+
+        _check_cuda(A, torch.float32, "A")
+        if A.dim() != 2 or A.stride(1) != 1:
+            raise ValueError("A must be 2-D row-major (unit column stride)")
+        return A.data_ptr(), int(A.shape[1]), int(A.stride(0)) if A.shape[0] > 1 else max(int(A.stride(0)), int(A.shape[1]))
+
+    def apply_f32acc(self, A, out=None, stream=None, **opts):
+        import torch
+
+        ap, n, lda = self._A_args(A)
+        if out is None:
+            out = torch.empty((self.d, n), dtype=torch.float32, device=A.device)
+        _check_cuda(out, torch.float32, "out")
+        assert out.is_contiguous() and tuple(out.shape) == (self.d, n)
+        if opts:
+            opts.setdefault("rows", A.shape[0])
+            o = _opts(**opts)
+            rc = lib().sketch_apply_f32acc_ex(self._h, ap, n, lda, out.data_ptr(), C.byref(o), _stream_ptr(stream))
+        else:
+            if A.shape[0] != self.m:
+                raise ValueError("A has %d rows, sketch was created for m=%d (pass row_begin=/rows= for a slice)" % (A.shape[0], self.m))
+            rc = lib().sketch_apply_f32acc(self._h, ap, n, lda, out.data_ptr(), _stream_ptr(stream))
+        if rc:
+            raise SketchError(rc, "sketch_apply_f32acc")
+        return out
+
+    def apply_f16acc(self, A, out=None, rounding: int = RN, sr_seed: int = 0, stream=None, **opts):
+        import torch
+
+        ap, n, lda = self._A_args(A)
+        if out is None:
+            out = torch.empty((self.d, n), dtype=torch.float16, device=A.device)
+        _check_cuda(out, torch.float16, "out")
+        assert out.is_contiguous() and tuple(out.shape) == (self.d, n)
+        if opts:
+            opts.setdefault("rows", A.shape[0])
+            o = _opts(**opts)
+            rc = lib().sketch_apply_f16acc_ex(self._h, ap, n, lda, out.data_ptr(), rounding, sr_seed & (2**64 - 1), C.byref(o),
+                                              _stream_ptr(stream))
+        else:
+            if A.shape[0] != self.m:
+                raise ValueError("A has %d rows, sketch was created for m=%d (pass row_begin=/rows= for a slice)" % (A.shape[0], self.m))
+            rc = lib().sketch_apply_f16acc(self._h, ap, n, lda, out.data_ptr(), rounding, sr_seed & (2**64 - 1), _stream_ptr(stream))
+        if rc:
+            raise SketchError(rc, "sketch_apply_f16acc")
+        return out
+
+    # ---- host-buffer applies (end-to-end: H2D streaming + kernels + D2H inside the call)
+    def apply_f16acc_host(self, A_host, out_host=None, rounding: int = RN, sr_seed: int = 0, **opts):
+        import torch
+
+        assert not A_host.is_cuda and A_host.dtype == torch.float32 and A_host.dim() == 2 and A_host.stride(1) == 1
+        n = int(A_host.shape[1])
+        if out_host is None:
+            out_host = torch.empty((self.d, n), dtype=torch.float16, pin_memory=True)
+        assert not out_host.is_cuda and out_host.dtype == torch.float16 and out_host.is_contiguous()
+        opts.setdefault("rows", A_host.shape[0])
+        o = _opts(**opts)
+        rc = lib().sketch_apply_f16acc_host(self._h, A_host.data_ptr(), n, int(A_host.stride(0)), out_host.data_ptr(), rounding,
+                                            sr_seed & (2**64 - 1), C.byref(o))
+        if rc:
+            raise SketchError(rc, "sketch_apply_f16acc_host")
+        return out_host
+
+    def apply_f32acc_host(self, A_host, out_host=None, **opts):
+        import torch
+
+        assert not A_host.is_cuda and A_host.dtype == torch.float32 and A_host.dim() == 2 and A_host.stride(1) == 1
+        n = int(A_host.shape[1])
+        if out_host is None:
+            out_host = torch.empty((self.d, n), dtype=torch.float32, pin_memory=True)
+        assert not out_host.is_cuda and out_host.dtype == torch.float32 and out_host.is_contiguous()
+        opts.setdefault("rows", A_host.shape[0])
+        o = _opts(**opts)
+        rc = lib().sketch_apply_f32acc_host(self._h, A_host.data_ptr(), n, int(A_host.stride(0)), out_host.data_ptr(), C.byref(o))
+        if rc:
+            raise SketchError(rc, "sketch_apply_f32acc_host")
+        return out_host
+
+    # ---- planning (host only)
+    def plan(self, n: int, lda: int | None = None, f16: bool = True, rounding: int = RN, **opts):
+        v, p, h, g = _i32(0), _i32(0), _i32(0), _i32(0)
+        o = _opts(**opts)
+        rc = lib().sketch_plan(self._h, n, lda or n, int(f16), rounding, C.byref(o), C.byref(v), C.byref(p), C.byref(h), C.byref(g))
+        if rc:
+            raise SketchError(rc, "sketch_plan")
+        return {"variant": VARIANT_NAMES[v.value], "replicas": p.value, "hash_mode": h.value, "grid": g.value}

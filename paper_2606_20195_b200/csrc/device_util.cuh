@@ -1,0 +1,142 @@
+// device_util.cuh -- device-side building blocks of the sm_100a sparse-sketch kernels:
+// the counter hash, FP32->FP16 conversion RN / SR (a4) and the
+// result-discarding reductions (a5, a6).
+#pragma once
+
+#include <cuda_fp16.h>
+#include <stdint.h>
+
+#define SK_DEVINL __device__ __forceinline__
+
+namespace sk {
+
+// ------------------------------------------------------------------------------------------------
+// Hash: h = splitmix64(seed ^ ctr), ctr = i*zeta + j (BASELINE.json:north_star; R1-R4).
+// Packed entry: bucket | signbit << 31.
+// ------------------------------------------------------------------------------------------------
+SK_DEVINL uint64_t splitmix64(uint64_t x) {
+  uint64_t z = x + 0x9E3779B97F4A7C15ull;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+SK_DEVINL uint32_t hash_entry(uint64_t seed, uint64_t ctr, uint32_t j, uint32_t db) {
+  uint64_t h = splitmix64(seed ^ ctr);
+  uint32_t bucket = j * db + __umulhi((uint32_t)(h >> 32), db);  // ((h>>32)*db)>>32, db < 2^31
+  return bucket | ((uint32_t)h << 31);
+}
+
+SK_DEVINL uint32_t entry_bucket(uint32_t e) { return e & 0x7FFFFFFFu; }
+// 0x80008000 when the sign bit is set, else 0: XOR mask for a packed half2 (RN is odd)
+SK_DEVINL uint32_t entry_signmask_h2(uint32_t e) { return (uint32_t)((int32_t)e >> 31) & 0x80008000u; }
+SK_DEVINL uint32_t entry_signmask_f32(uint32_t e) { return e & 0x80000000u; }
+
+// ------------------------------------------------------------------------------------------------
+// Conversion FP32 -> packed half2 {lo = x0, hi = x1}.
+// RN: cvt.rn.f16x2.f32 (SASS F2FP.F16.F32.PACK_AB), round-to-nearest-even, subnormals kept,
+//     |x| >= 65520 -> inf; the __float2half of PAPER.md:127-129.
+// ------------------------------------------------------------------------------------------------
+SK_DEVINL uint32_t pack_rn(float x0, float x1) {
+  __half2 h = __floats2half2_rn(x0, x1);
+  return *reinterpret_cast<uint32_t*>(&h);
+}
+
+// SR (R13): magnitude rounded toward zero to l, moved one grid step away
+// from zero iff u < t with t = (|p|-|l|)/w and u = (r24 + 1/2) 2^-24.  All-integer evaluation:
+// with s discarded bits and rem their value, u < t  <=>  (2 r24 + 1) 2^s < rem 2^25.
+SK_DEVINL uint32_t sr16_bits(float p, uint32_t r24) {
+  uint32_t fb = __float_as_uint(p);
+  uint32_t sign = (fb >> 16) & 0x8000u;
+  uint32_t mag = fb & 0x7FFFFFFFu;
+  if (mag > 0x7F800000u) return sign | 0x7E00u;   // NaN
+  if (mag >= 0x47800000u) return sign | 0x7C00u;  // |p| >= 65536 -> inf
+  if (mag >= 0x38800000u) {                       // |p| >= 2^-14: FP16 normal grid, 13 discarded bits
+    uint32_t trunc = (mag >> 13) - 0x1C000u;      // rebias 127 -> 15
+    uint32_t rem = mag & 0x1FFFu;
+    uint32_t up = ((r24 >> 11) < rem) ? 1u : 0u;  // (2 r24+1) < rem<<12  <=>  r24>>11 < rem
+    return sign | (trunc + up);                   // carry walks into the exponent; 0x7BFF+1 = inf
+  }
+  // FP16 subnormal grid, spacing 2^-24
+  uint32_t ef = mag >> 23;                                       // biased FP32 exponent, 0 = FP32 subnormal
+  uint32_t M = (mag & 0x7FFFFFu) | (ef ? 0x800000u : 0u);        // |p| = M * 2^(e-23)
+  int e = ef ? (int)ef - 127 : -126;
+  int s = -1 - e;                                                // 14 .. 125
+  uint32_t l = (s < 24) ? (M >> s) : 0u;
+  uint32_t rem = (s < 24) ? (M & ((1u << s) - 1u)) : M;
+  uint64_t lhs = 2ull * r24 + 1ull;
+  bool up;
+  if (s <= 25) up = lhs < ((uint64_t)rem << (25 - s));
+  else if (s < 49) up = (lhs << (s - 25)) < (uint64_t)rem;
+  else up = false;
+  return sign | (l + (up ? 1u : 0u));
+}
+
+// one 64-bit draw per column pair (R14): bits 63..40 -> even column, bits 39..16 -> odd column
+SK_DEVINL uint32_t pack_sr(float x0, float x1, uint64_t sr_seed, uint64_t ctr) {
+  uint64_t R = splitmix64(sr_seed ^ ctr);
+  uint32_t lo = sr16_bits(x0, (uint32_t)(R >> 40));
+  uint32_t hi = sr16_bits(x1, (uint32_t)(R >> 16) & 0xFFFFFFu);
+  return lo | (hi << 16);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Result-discarding reductions to global memory (L2).  PAPER.md:177-183: atom.global.add with the
+// result unused -> SASS REDG (no return path).  sm_90+/sm_100a also take 8- and 16-byte vector forms
+// (REDG.E.ADD.F16x4 / F16x8 / F32x2 / F32x4): one instruction, one L2 transaction, 2-4 column pairs.
+// .noftz keeps FP16 subnormals; every half / float component is added independently.
+// ------------------------------------------------------------------------------------------------
+SK_DEVINL void red_h2(void* p, uint32_t a) {
+  asm volatile("red.global.add.noftz.f16x2 [%0], %1;" ::"l"(p), "r"(a) : "memory");
+}
+SK_DEVINL void red_h4(void* p, uint32_t a, uint32_t b) {
+  asm volatile("red.global.add.noftz.v2.f16x2 [%0], {%1,%2};" ::"l"(p), "r"(a), "r"(b) : "memory");
+}
+SK_DEVINL void red_h8(void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("red.global.add.noftz.v4.f16x2 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(a), "r"(b), "r"(c), "r"(d)
+               : "memory");
+}
+SK_DEVINL void red_f1(void* p, float a) {
+  asm volatile("red.global.add.f32 [%0], %1;" ::"l"(p), "f"(a) : "memory");
+}
+SK_DEVINL void red_f2(void* p, float a, float b) {
+  asm volatile("red.global.add.v2.f32 [%0], {%1,%2};" ::"l"(p), "f"(a), "f"(b) : "memory");
+}
+SK_DEVINL void red_f4(void* p, float a, float b, float c, float d) {
+  asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d)
+               : "memory");
+}
+
+// scalar FP16 add for odd n: there is no native scalar f16 RED on sm_100a (red.global.add.noftz.f16
+// assembles to a CAS loop), so add {v, +0} or {+0, v} with the packed RED on the enclosing aligned
+// 4-byte word: x + (+0) = x for every x except -0 -> +0, which the path never produces (R10).
+SK_DEVINL void red_h1(__half* p, uint16_t v) {
+  uintptr_t a = reinterpret_cast<uintptr_t>(p);
+  uint32_t word = (a & 2) ? ((uint32_t)v << 16) : (uint32_t)v;
+  red_h2(reinterpret_cast<void*>(a & ~(uintptr_t)3), word);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Streaming loads of A: read once, never reused -> bypass L1 allocation; the 256-bit form also takes
+// L2::evict_first (ptxas accepts that modifier only on .v8.b32/.v4.b64 loads).
+// ------------------------------------------------------------------------------------------------
+template <int VEC>
+SK_DEVINL void ld_stream(const float* p, float (&v)[VEC]) {
+  if constexpr (VEC == 8) {
+    asm volatile("ld.global.nc.L1::no_allocate.L2::evict_first.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7])
+                 : "l"(p));
+  } else if constexpr (VEC == 4) {
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3])
+                 : "l"(p));
+  } else if constexpr (VEC == 2) {
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0,%1}, [%2];"
+                 : "=f"(v[0]), "=f"(v[1])
+                 : "l"(p));
+  } else {
+    asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(v[0]) : "l"(p));
+  }
+}
+
+}  // namespace sk

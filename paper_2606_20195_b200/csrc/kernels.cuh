@@ -1,0 +1,438 @@
+// kernels.cuh -- the sm_100a kernels of the sparse-sketch hot path.
+//
+//   k_hash_dump / k_hash_pack   a1  hash stage (dump for tests, packed array for hash_mode=2)
+//   k_flat<...>                 a2-a6 streaming scatter with result-discarding global RED
+//                               (the paper's Listings 1/2 restated with shared hashes + vector RED)
+//   k_smem<...>                 a2-a5 shared-memory-privatised FP16 partial sketch per CTA
+//   k_generic<...>              any-n / any-alignment scalar fallback
+//   k_reduce_replicas<...>      sums the P L2-resident partial sketches of the flat variant
+//   k_red_probe<...>            L2 atomic-throughput microbenchmark (roofline term 2)
+#pragma once
+
+#include "device_util.cuh"
+
+namespace sk {
+
+constexpr int kFlatThreads = 256;
+
+// ------------------------------------------------------------------------------------------------
+// a1: hash stage as stand-alone kernels
+// ------------------------------------------------------------------------------------------------
+__global__ void k_hash_dump(uint64_t seed, int64_t total, uint32_t zeta, uint32_t db, int32_t* __restrict__ bucket,
+                            uint8_t* __restrict__ signbit) {
+  int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += stride) {
+    uint32_t j = (uint32_t)(idx % zeta);
+    uint32_t e = hash_entry(seed, (uint64_t)idx, j, db);
+    bucket[idx] = (int32_t)entry_bucket(e);
+    signbit[idx] = (uint8_t)(e >> 31);
+  }
+}
+
+template <typename PackT>
+__global__ void k_hash_pack(uint64_t seed, int64_t total, uint32_t zeta, uint32_t db, PackT* __restrict__ packed) {
+  int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += stride) {
+    uint32_t j = (uint32_t)(idx % zeta);
+    uint32_t e = hash_entry(seed, (uint64_t)idx, j, db);
+    if constexpr (sizeof(PackT) == 2)
+      packed[idx] = (PackT)(entry_bucket(e) | ((e >> 31) << 15));
+    else
+      packed[idx] = (PackT)e;
+  }
+}
+
+// packed entry -> canonical 32-bit entry (bucket | sign<<31)
+template <typename PackT>
+SK_DEVINL uint32_t unpack_entry(PackT p) {
+  if constexpr (sizeof(PackT) == 2) return ((uint32_t)p & 0x7FFFu) | (((uint32_t)p >> 15) << 31);
+  else return (uint32_t)p;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Arguments shared by the scatter kernels
+// ------------------------------------------------------------------------------------------------
+struct ScatterArgs {
+  const float* A;       // first row of the range
+  int64_t lda;          // elements
+  int64_t row_begin;    // global index of A's first row (hash counter base)
+  int64_t rows;         // rows in the range
+  void* B;              // d x n sketch (or base of the replicas)
+  int64_t replica_stride;  // elements between replicas
+  int32_t replicas;
+  int32_t n;
+  int32_t zeta;
+  uint32_t db;          // d / zeta
+  uint64_t seed;
+  uint64_t sr_seed;
+  float scale;          // fp32(1/sqrt(zeta)), correctly rounded on the host (R5)
+  uint32_t cpr;         // chunks of VEC columns per row = n / VEC
+  uint32_t cpr_magic;   // ceil(2^32 / cpr): c / cpr == umulhi(c, magic) for c*cpr < 2^32
+  const void* packed;   // hash_mode 2: packed entries for global rows, index i*zeta + j; else nullptr
+};
+
+// ------------------------------------------------------------------------------------------------
+// Flat scatter: every contribution is one result-discarding RED into an L2-resident sketch.
+//
+// One warp owns a "macro step" of HB = 32/ZETA consecutive rows.  Lane l hashes (row l/ZETA, block
+// l%ZETA) once -- 32 hashes per warp instead of n/VEC redundant ones per row -- and the HB*n floats
+// are then consumed as 32-lane chunks of VEC consecutive columns (coalesced 32*VEC*4-byte requests),
+// each lane fetching its row's ZETA entries by shuffle.  The product s*a is rounded to FP16 once per
+// element and the block sign applied by XOR, which is bit-identical to RN16((eps*s)*a) because RN is
+// odd; SR converts per contribution.
+// Replicas: CTA b adds into partial sketch b % P, which cuts same-address serialisation in L2 and the
+// depth of every running sum by P; k_reduce_replicas folds them.
+// ------------------------------------------------------------------------------------------------
+template <int VEC, bool F16, int ROUNDING>
+SK_DEVINL void emit_contribution(void* Bbase, int64_t off, const float (&p)[VEC], const uint32_t (&q)[VEC / 2 > 0 ? VEC / 2 : 1],
+                                 uint32_t e, uint64_t sr_seed, uint64_t sr_ctr) {
+  if constexpr (F16) {
+    __half* dst = reinterpret_cast<__half*>(Bbase) + off;
+    uint32_t w[VEC / 2];
+    if constexpr (ROUNDING == 0) {
+      uint32_t sm = entry_signmask_h2(e);
+#pragma unroll
+      for (int k = 0; k < VEC / 2; ++k) w[k] = q[k] ^ sm;
+    } else {
+      uint32_t sf = entry_signmask_f32(e);
+#pragma unroll
+      for (int k = 0; k < VEC / 2; ++k)
+        w[k] = pack_sr(__uint_as_float(__float_as_uint(p[2 * k]) ^ sf), __uint_as_float(__float_as_uint(p[2 * k + 1]) ^ sf),
+                       sr_seed, sr_ctr + k);
+    }
+    if constexpr (VEC == 8) red_h8(dst, w[0], w[1], w[2], w[3]);
+    else if constexpr (VEC == 4) red_h4(dst, w[0], w[1]);
+    else red_h2(dst, w[0]);
+  } else {
+    float* dst = reinterpret_cast<float*>(Bbase) + off;
+    uint32_t sf = entry_signmask_f32(e);
+    float w[VEC];
+#pragma unroll
+    for (int k = 0; k < VEC; ++k) w[k] = __uint_as_float(__float_as_uint(p[k]) ^ sf);
+    if constexpr (VEC == 8) {
+      red_f4(dst, w[0], w[1], w[2], w[3]);
+      red_f4(dst + 4, w[4], w[5], w[6], w[7]);
+    } else if constexpr (VEC == 4) red_f4(dst, w[0], w[1], w[2], w[3]);
+    else if constexpr (VEC == 2) red_f2(dst, w[0], w[1]);
+    else red_f1(dst, w[0]);
+  }
+}
+
+template <int ZETA, int VEC, bool F16, int ROUNDING, typename PackT>
+__global__ void __launch_bounds__(kFlatThreads) k_flat(ScatterArgs a) {
+  static_assert(32 % ZETA == 0, "ZETA must divide 32");
+  constexpr int HB = 32 / ZETA;            // rows per macro step
+  constexpr bool PRE = sizeof(PackT) > 1;  // PackT = uint8_t means "hash on the fly"
+  const uint32_t lane = threadIdx.x & 31;
+  const int64_t warps = ((int64_t)gridDim.x * kFlatThreads) >> 5;
+  const int64_t gwarp = ((int64_t)blockIdx.x * kFlatThreads + threadIdx.x) >> 5;
+  const int64_t macros = (a.rows + HB - 1) / HB;
+  const uint32_t chunks = (uint32_t)HB * a.cpr;  // chunks per macro step
+  char* Bbase = reinterpret_cast<char*>(a.B) +
+                (size_t)(blockIdx.x % a.replicas) * (size_t)a.replica_stride * (F16 ? 2 : 4);
+  const uint32_t npairs = ((uint32_t)a.n + 1u) >> 1;
+
+  for (int64_t mac = gwarp; mac < macros; mac += warps) {
+    const int64_t r0 = mac * HB;  // local row of the macro step
+    // ---- hash stage: lane l -> (row r0 + l/ZETA, block l%ZETA)
+    uint32_t e;
+    {
+      uint32_t j = lane % ZETA;
+      uint64_t ctr = (uint64_t)(a.row_begin + r0) * ZETA + lane;  // (row)*ZETA + j with row = r0 + lane/ZETA
+      if constexpr (PRE) {
+        int64_t lr = r0 + lane / ZETA;
+        e = (lr < a.rows) ? unpack_entry<PackT>(reinterpret_cast<const PackT*>(a.packed)[ctr]) : 0u;
+      } else {
+        e = hash_entry(a.seed, ctr, j, a.db);
+      }
+    }
+    // ---- stream the HB x n floats
+    for (uint32_t c = lane; c < ((chunks + 31u) & ~31u); c += 32) {
+      uint32_t rr = a.cpr_magic ? __umulhi(c, a.cpr_magic) : c;  // c / cpr (magic 0 <=> cpr == 1)
+      uint32_t ch = c - rr * a.cpr;
+      bool valid = (c < chunks) && (r0 + rr < a.rows);
+      rr = valid ? rr : 0u;
+      float p[VEC];
+      uint32_t q[VEC / 2 > 0 ? VEC / 2 : 1];
+      if (valid) {
+        ld_stream<VEC>(a.A + (r0 + rr) * a.lda + (int64_t)ch * VEC, p);
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) p[k] *= a.scale;
+      } else {
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) p[k] = 0.f;
+      }
+      if constexpr (F16 && ROUNDING == 0) {
+#pragma unroll
+        for (int k = 0; k < VEC / 2; ++k) q[k] = pack_rn(p[2 * k], p[2 * k + 1]);
+      }
+#pragma unroll
+      for (int j = 0; j < ZETA; ++j) {
+        uint32_t ej = __shfl_sync(0xFFFFFFFFu, e, rr * ZETA + j);
+        if (valid) {
+          int64_t off = (int64_t)entry_bucket(ej) * a.n + (int64_t)ch * VEC;
+          uint64_t sr_ctr = ((uint64_t)(a.row_begin + r0 + rr) * ZETA + j) * npairs + (uint64_t)ch * (VEC / 2);
+          emit_contribution<VEC, F16, ROUNDING>(Bbase, off, p, q, ej, a.sr_seed, sr_ctr);
+        }
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Generic fallback: one lane per (row, column) element, runtime zeta, scalar RED; any n, lda, alignment.
+// ------------------------------------------------------------------------------------------------
+template <bool F16, int ROUNDING>
+__global__ void __launch_bounds__(kFlatThreads) k_generic(ScatterArgs a) {
+  const int64_t total = a.rows * (int64_t)a.n;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  const uint32_t npairs = ((uint32_t)a.n + 1u) >> 1;
+  char* Bbase = reinterpret_cast<char*>(a.B) +
+                (size_t)(blockIdx.x % a.replicas) * (size_t)a.replica_stride * (F16 ? 2 : 4);
+  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += stride) {
+    int64_t r = idx / a.n;
+    int32_t c = (int32_t)(idx - r * a.n);
+    float p = a.A[r * a.lda + c] * a.scale;
+    for (int32_t j = 0; j < a.zeta; ++j) {
+      uint64_t ctr = (uint64_t)(a.row_begin + r) * (uint64_t)a.zeta + (uint64_t)j;
+      uint32_t e = hash_entry(a.seed, ctr, (uint32_t)j, a.db);
+      int64_t off = (int64_t)entry_bucket(e) * a.n + c;
+      float ps = __uint_as_float(__float_as_uint(p) ^ entry_signmask_f32(e));
+      if constexpr (F16) {
+        uint16_t v;
+        if constexpr (ROUNDING == 0) {
+          v = __half_as_ushort(__float2half_rn(ps));
+        } else {
+          uint64_t R = splitmix64(a.sr_seed ^ (ctr * npairs + (uint64_t)(c >> 1)));
+          uint32_t r24 = (c & 1) ? ((uint32_t)(R >> 16) & 0xFFFFFFu) : (uint32_t)(R >> 40);
+          v = (uint16_t)sr16_bits(ps, r24);
+        }
+        red_h1(reinterpret_cast<__half*>(Bbase) + off, v);
+      } else {
+        red_f1(reinterpret_cast<float*>(Bbase) + off, ps);
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Fold P partial sketches.  FP16: sequential RN16 adds in replica order (every accumulation of the
+// FP16 path stays an FP16 RN add, "All policies subsequently use RN atomic addition");
+// FP32: float adds.  accumulate != 0 adds the fold into the existing out.
+// ------------------------------------------------------------------------------------------------
+template <bool F16>
+__global__ void k_reduce_replicas(const void* __restrict__ rep, int64_t replica_stride, int32_t replicas, void* __restrict__ out,
+                                  int64_t count, int accumulate) {
+  int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < count; k += stride) {
+    if constexpr (F16) {
+      const __half* r = reinterpret_cast<const __half*>(rep);
+      __half* o = reinterpret_cast<__half*>(out);
+      __half acc = accumulate ? o[k] : __ushort_as_half(0);
+      for (int p = 0; p < replicas; ++p) acc = __hadd(acc, r[(int64_t)p * replica_stride + k]);
+      o[k] = acc;
+    } else {
+      const float* r = reinterpret_cast<const float*>(rep);
+      float* o = reinterpret_cast<float*>(out);
+      float acc = accumulate ? o[k] : 0.f;
+      for (int p = 0; p < replicas; ++p) acc = __fadd_rn(acc, r[(int64_t)p * replica_stride + k]);
+      o[k] = acc;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Shared-memory-privatised FP16 scatter.
+//
+// Each CTA keeps one private d x n FP16 partial sketch in shared memory and streams a contiguous range
+// of rows.  sm_100a has no native shared-memory FP16 add (atomicAdd on smem assembles to a CAS loop),
+// so every sketch word has exactly one owning lane at any time and is updated with plain
+// LDS / HADD2 / STS:
+//   - warp w of the CTA owns the column slice [w*CW, (w+1)*CW), CW = LPR*VEC; no two warps of a CTA
+//     ever touch the same word;
+//   - inside a warp the 32 lanes are R = 32/LPR rows x LPR column chunks; at step t the lanes of row r
+//     update stack block (r + t) mod ZETA.  Blocks are disjoint row ranges of the sketch
+//     (PAPER.md:59-63), so with R <= ZETA the R rows of a step can never collide -- no conflict
+//     detection, no atomics;
+//   - steps are separated by __syncwarp() (row r+1 touched block (r+t+1) mod ZETA one step earlier).
+// A is read straight into registers with 128/256-bit streaming loads through an NQ-deep register ring
+// (NQ row groups in flight per warp), because staging A through shared memory would add 8 B/float to
+// a shared-memory pipe that the 2*2*ZETA B/float of read-modify-write traffic already loads to ~2/3.
+// At the end the CTA flushes its partial sketch into B with 16-byte result-discarding REDs.
+// ------------------------------------------------------------------------------------------------
+struct SmemArgs {
+  ScatterArgs s;
+  int64_t rows_per_cta;  // multiple of the hash batch
+  int32_t d;
+};
+
+template <int ZETA, int VEC, int LPR, int ROUNDING, int NQ, int MAXW>
+__global__ void __launch_bounds__(MAXW * 32) k_smem(SmemArgs g) {
+  constexpr int R = 32 / LPR;                 // rows per warp step
+  static_assert(R <= ZETA, "rotation needs R <= ZETA");
+  static_assert(32 % ZETA == 0 && LPR >= ZETA, "layout");
+  constexpr int HB = 32 / ZETA;               // rows per hash batch
+  constexpr int QPB = HB / R;                 // row groups per hash batch
+  static_assert(NQ % QPB == 0, "ring must hold whole hash batches");
+  constexpr int CW = LPR * VEC;               // columns per warp
+  constexpr int NH = VEC / 2;                 // half2 words per lane
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const ScatterArgs& a = g.s;
+  const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t r = lane / LPR, pcol = lane % LPR;
+  const int32_t n = a.n;
+  const uint32_t row_pitch = (uint32_t)n * 2u;  // bytes per sketch row in smem
+
+  // ---- a0 (private part): zero the partial sketch
+  {
+    uint4* z = reinterpret_cast<uint4*>(smem_raw);
+    const uint32_t n16 = (uint32_t)g.d * row_pitch / 16u;
+    for (uint32_t k = tid; k < n16; k += blockDim.x) z[k] = make_uint4(0, 0, 0, 0);
+  }
+  __syncthreads();
+
+  const int64_t cta_r0 = (int64_t)blockIdx.x * g.rows_per_cta;
+  const int64_t cta_r1 = min(a.rows, cta_r0 + g.rows_per_cta);
+  const uint32_t col0 = warp * CW + pcol * VEC;               // first column of this lane
+  unsigned char* my_col = smem_raw + col0 * 2u;
+  const float* Acol = a.A + col0;
+  const uint32_t npairs = ((uint32_t)n + 1u) >> 1;
+
+  if (cta_r0 < cta_r1) {
+    // register ring of NQ row groups
+    float buf[NQ][VEC];
+    auto load_group = [&](int64_t grow0, float (&dst)[VEC]) {  // grow0: local row of the group's first row
+      int64_t row = grow0 + r;
+      if (row < cta_r1) {
+        ld_stream<VEC>(Acol + row * a.lda, dst);
+      } else {
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) dst[k] = 0.f;
+      }
+    };
+    constexpr int RING_ROWS = NQ * R;
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) load_group(cta_r0 + (int64_t)q * R, buf[q]);
+
+    for (int64_t base = cta_r0; base < cta_r1; base += RING_ROWS) {
+#pragma unroll
+      for (int hb = 0; hb < NQ / QPB; ++hb) {
+        const int64_t b0 = base + (int64_t)hb * HB;  // first local row of this hash batch
+        // hash stage: lane l -> (row b0 + l/ZETA, block l%ZETA)
+        uint32_t e;
+        {
+          uint64_t ctr = (uint64_t)(a.row_begin + b0) * ZETA + lane;
+          e = hash_entry(a.seed, ctr, lane % ZETA, a.db);
+        }
+#pragma unroll
+        for (int qq = 0; qq < QPB; ++qq) {
+          const int q = hb * QPB + qq;
+          float p[VEC];
+#pragma unroll
+          for (int k = 0; k < VEC; ++k) p[k] = buf[q][k] * a.scale;
+          // refill this ring slot with the group NQ steps ahead
+          load_group(base + RING_ROWS + (int64_t)q * R, buf[q]);
+          uint32_t qv[NH];
+          if constexpr (ROUNDING == 0) {
+#pragma unroll
+            for (int k = 0; k < NH; ++k) qv[k] = pack_rn(p[2 * k], p[2 * k + 1]);
+          }
+          const uint32_t rib = (uint32_t)qq * R + r;  // row in batch
+#pragma unroll
+          for (int t = 0; t < ZETA; ++t) {
+            const uint32_t jt = (r + t) % ZETA;
+            const uint32_t ej = __shfl_sync(0xFFFFFFFFu, e, rib * ZETA + jt);
+            unsigned char* addr = my_col + entry_bucket(ej) * row_pitch;
+            uint32_t w[NH];
+            if constexpr (ROUNDING == 0) {
+              const uint32_t sm = entry_signmask_h2(ej);
+#pragma unroll
+              for (int k = 0; k < NH; ++k) w[k] = qv[k] ^ sm;
+            } else {
+              const uint32_t sf = entry_signmask_f32(ej);
+              const uint64_t sr_ctr =
+                  ((uint64_t)(a.row_begin + b0 + rib) * ZETA + jt) * npairs + (uint64_t)(col0 >> 1);
+#pragma unroll
+              for (int k = 0; k < NH; ++k)
+                w[k] = pack_sr(__uint_as_float(__float_as_uint(p[2 * k]) ^ sf),
+                               __uint_as_float(__float_as_uint(p[2 * k + 1]) ^ sf), a.sr_seed, sr_ctr + k);
+            }
+            // read-modify-write of the lane's NH half2 words: sole owner, no atomics
+            if constexpr (NH == 4) {
+              uint4 acc = *reinterpret_cast<uint4*>(addr);
+              __half2 x0 = __hadd2(*reinterpret_cast<__half2*>(&acc.x), *reinterpret_cast<__half2*>(&w[0]));
+              __half2 x1 = __hadd2(*reinterpret_cast<__half2*>(&acc.y), *reinterpret_cast<__half2*>(&w[1]));
+              __half2 x2 = __hadd2(*reinterpret_cast<__half2*>(&acc.z), *reinterpret_cast<__half2*>(&w[2]));
+              __half2 x3 = __hadd2(*reinterpret_cast<__half2*>(&acc.w), *reinterpret_cast<__half2*>(&w[3]));
+              acc.x = *reinterpret_cast<uint32_t*>(&x0);
+              acc.y = *reinterpret_cast<uint32_t*>(&x1);
+              acc.z = *reinterpret_cast<uint32_t*>(&x2);
+              acc.w = *reinterpret_cast<uint32_t*>(&x3);
+              *reinterpret_cast<uint4*>(addr) = acc;
+            } else if constexpr (NH == 2) {
+              uint2 acc = *reinterpret_cast<uint2*>(addr);
+              __half2 x0 = __hadd2(*reinterpret_cast<__half2*>(&acc.x), *reinterpret_cast<__half2*>(&w[0]));
+              __half2 x1 = __hadd2(*reinterpret_cast<__half2*>(&acc.y), *reinterpret_cast<__half2*>(&w[1]));
+              acc.x = *reinterpret_cast<uint32_t*>(&x0);
+              acc.y = *reinterpret_cast<uint32_t*>(&x1);
+              *reinterpret_cast<uint2*>(addr) = acc;
+            } else {
+              uint32_t acc = *reinterpret_cast<uint32_t*>(addr);
+              __half2 x0 = __hadd2(*reinterpret_cast<__half2*>(&acc), *reinterpret_cast<__half2*>(&w[0]));
+              *reinterpret_cast<uint32_t*>(addr) = *reinterpret_cast<uint32_t*>(&x0);
+            }
+            __syncwarp();
+          }
+        }
+      }
+    }
+  }
+  __syncthreads();
+
+  // ---- flush: partial sketch -> B with 16-byte result-discarding REDs (layouts coincide: [d][n])
+  {
+    const uint4* z = reinterpret_cast<const uint4*>(smem_raw);
+    const uint32_t n16 = (uint32_t)g.d * row_pitch / 16u;
+    __half* B = reinterpret_cast<__half*>(a.B);
+    // stagger the start so the CTAs do not all hit the same L2 lines at once
+    const uint32_t shift = (uint32_t)((blockIdx.x * 2654435761u) % n16);
+    for (uint32_t k0 = tid; k0 < n16; k0 += blockDim.x) {
+      uint32_t k = k0 + shift;
+      k = (k >= n16) ? k - n16 : k;
+      uint4 v = z[k];
+      if ((v.x | v.y | v.z | v.w) != 0u) red_h8(B + (size_t)k * 8, v.x, v.y, v.z, v.w);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// L2 atomic-throughput probe: same address pattern as k_flat (a random bucket row per lane group of
+// n/VEC lanes, consecutive lanes on consecutive VEC-column chunks), values from registers, no A loads.
+// ------------------------------------------------------------------------------------------------
+template <int KIND>
+__global__ void __launch_bounds__(kFlatThreads) k_red_probe(void* sketch, int32_t d, int32_t n, int32_t replicas, int32_t iters) {
+  constexpr bool F16 = KIND < 3;
+  constexpr int VEC = (KIND == 0) ? 2 : (KIND == 1) ? 4 : (KIND == 2) ? 8 : (KIND == 3) ? 1 : (KIND == 4) ? 2 : 4;
+  const uint32_t cpr = (uint32_t)n / VEC;
+  const uint64_t gtid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const uint64_t gthreads = (uint64_t)gridDim.x * blockDim.x;
+  char* base = reinterpret_cast<char*>(sketch) + (size_t)(blockIdx.x % replicas) * (size_t)d * n * (F16 ? 2 : 4);
+  const uint32_t ch = (uint32_t)(gtid % cpr);
+  const uint64_t grp = gtid / cpr;
+  const uint64_t ngrp = (gthreads + cpr - 1) / cpr;
+  for (int32_t it = 0; it < iters; ++it) {
+    uint64_t h = splitmix64(grp + (uint64_t)it * ngrp);
+    uint32_t bucket = __umulhi((uint32_t)(h >> 32), (uint32_t)d);
+    size_t off = (size_t)bucket * n + (size_t)ch * VEC;
+    uint32_t hv = (h & 1) ? 0x3C003C00u : 0xBC00BC00u;  // +-1.0 pairs: sums stay small
+    float fv = (h & 1) ? 1.f : -1.f;
+    if constexpr (KIND == 0) red_h2(reinterpret_cast<__half*>(base) + off, hv);
+    else if constexpr (KIND == 1) red_h4(reinterpret_cast<__half*>(base) + off, hv, hv);
+    else if constexpr (KIND == 2) red_h8(reinterpret_cast<__half*>(base) + off, hv, hv, hv, hv);
+    else if constexpr (KIND == 3) red_f1(reinterpret_cast<float*>(base) + off, fv);
+    else if constexpr (KIND == 4) red_f2(reinterpret_cast<float*>(base) + off, fv, fv);
+    else red_f4(reinterpret_cast<float*>(base) + off, fv, fv, fv, fv);
+  }
+}
+
+}  // namespace sk

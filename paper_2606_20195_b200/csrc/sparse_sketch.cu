@@ -1,0 +1,629 @@
+// sparse_sketch.cu -- C ABI (include/sparse_sketch.h), handle, variant selection and launches.
+// Host logic only; every step of the hot path runs in the kernels of kernels.cuh.
+#include "../../include/sparse_sketch.h"
+
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "kernels.cuh"
+
+namespace {
+
+std::atomic<uint64_t> g_launches{0};
+thread_local char g_last_error[512] = "";
+
+int cuda_fail(cudaError_t e, const char* what) {
+  snprintf(g_last_error, sizeof(g_last_error), "%s: %s (%s)", what, cudaGetErrorName(e), cudaGetErrorString(e));
+  return SKETCH_ERR_CUDA;
+}
+#define CU_TRY(call)                                      \
+  do {                                                    \
+    cudaError_t _e = (call);                              \
+    if (_e != cudaSuccess) return cuda_fail(_e, #call);   \
+  } while (0)
+
+inline int launch_check(const char* what) {
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  cudaError_t e = cudaGetLastError();
+  return e == cudaSuccess ? SKETCH_OK : cuda_fail(e, what);
+}
+
+}  // namespace
+
+struct sketch {
+  int64_t m;
+  int32_t d, zeta;
+  uint32_t db;
+  uint64_t seed;
+  float scale;
+  // device properties (filled lazily on first device use)
+  int dev_ready;
+  int sm_count;
+  int smem_optin;    // max dynamic smem per block
+  int smem_per_sm;
+  // library-owned scratch
+  void* rep;  size_t rep_bytes;        // replicated partial sketches
+  void* packed; int packed_width;      // 0 = none, 2 / 4 bytes per entry
+  void* stage[2]; size_t stage_bytes;  // host-path staging
+  void* bdev; size_t bdev_bytes;
+  cudaStream_t st_copy, st_comp;
+  cudaEvent_t ev_copied[2], ev_done[2];
+  int host_ready;
+};
+
+namespace {
+
+struct Plan {
+  int variant, vec, replicas, hash_mode, grid, wpc, zeta_t;
+  size_t smem_bytes;
+  int64_t rows_per_cta;
+};
+
+int ensure_device(sketch* s) {
+  if (s->dev_ready) return SKETCH_OK;
+  int dev = 0;
+  CU_TRY(cudaGetDevice(&dev));
+  CU_TRY(cudaDeviceGetAttribute(&s->sm_count, cudaDevAttrMultiProcessorCount, dev));
+  CU_TRY(cudaDeviceGetAttribute(&s->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  CU_TRY(cudaDeviceGetAttribute(&s->smem_per_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev));
+  s->dev_ready = 1;
+  return SKETCH_OK;
+}
+
+int ensure_scratch(void** buf, size_t* have, size_t want) {
+  if (*have >= want) return SKETCH_OK;
+  if (*buf) {
+    CU_TRY(cudaFree(*buf));
+    *buf = nullptr;
+    *have = 0;
+  }
+  cudaError_t e = cudaMalloc(buf, want);
+  if (e == cudaErrorMemoryAllocation) {
+    cudaGetLastError();
+    return SKETCH_ERR_NOMEM;
+  }
+  if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc(scratch)");
+  *have = want;
+  return SKETCH_OK;
+}
+
+inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+inline bool zeta_templated(int z) { return z == 1 || z == 2 || z == 4 || z == 8; }
+
+// smem layout per zeta: (VEC, LPR) with LPR*VEC = 64 columns per warp
+inline int smem_vec_for(int zeta) { return zeta == 1 ? 2 : zeta == 2 ? 4 : 8; }
+
+bool smem_feasible(const sketch* s, int n, int64_t lda, const void* A, const void* B, size_t* bytes) {
+  if (!zeta_templated(s->zeta)) return false;
+  if (n % 64 != 0 || n / 64 > 16) return false;
+  int vec = smem_vec_for(s->zeta);
+  if (lda % vec != 0 || !aligned(A, 4 * (size_t)vec) || !aligned(B, 16)) return false;
+  size_t b = (size_t)s->d * n * 2;
+  if (b > (size_t)s->smem_optin) return false;
+  if ((uint64_t)s->d * (uint64_t)n * 2ull >= (1ull << 31)) return false;
+  *bytes = b;
+  return true;
+}
+
+int flat_vec_for(bool f16, int n, int64_t lda, const void* A, const void* B, int want_max) {
+  const int cands_h[3] = {8, 4, 2};
+  const int cands_f[4] = {4, 2, 1, 0};  // FP32: one 16-byte RED per lane is the widest single transaction
+  const int* c = f16 ? cands_h : cands_f;
+  int nc = f16 ? 3 : 3;
+  for (int k = 0; k < nc; ++k) {
+    int v = c[k];
+    if (v > want_max) continue;
+    size_t eb = f16 ? 2 : 4;
+    if (n % v == 0 && lda % v == 0 && aligned(A, 4 * (size_t)v) && aligned(B, eb * v)) return v;
+  }
+  return 0;
+}
+
+int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool f16, int rounding,
+              const sketch_opts_t* o, int64_t rows, Plan* p) {
+  int rc = ensure_device(s);
+  if (rc) return rc;
+  memset(p, 0, sizeof(*p));
+  int want = o ? o->variant : SKETCH_VARIANT_AUTO;
+  if (want < 0 || want > SKETCH_VARIANT_GENERIC) return SKETCH_ERR_INVALID;
+  p->hash_mode = (o && o->hash_mode) ? o->hash_mode : 1;
+  if (p->hash_mode != 1 && p->hash_mode != 2) return SKETCH_ERR_INVALID;
+  size_t sm_bytes = 0;
+  bool sm_ok = f16 && smem_feasible(s, n, lda, A, B, &sm_bytes);
+  int vmax = flat_vec_for(f16, n, lda, A, B, 8);
+  int vpair = flat_vec_for(f16, n, lda, A, B, f16 ? 2 : 1);
+  bool zt = zeta_templated(s->zeta);
+
+  int v = want;
+  if (v == SKETCH_VARIANT_AUTO) {
+    if (sm_ok) v = SKETCH_VARIANT_SMEM;
+    else if (zt && vmax) v = SKETCH_VARIANT_FLAT_VEC;
+    else v = SKETCH_VARIANT_GENERIC;
+  }
+  if (v == SKETCH_VARIANT_SMEM && !sm_ok) return SKETCH_ERR_UNSUPPORTED;
+  if (v == SKETCH_VARIANT_FLAT_VEC && !(zt && vmax)) return SKETCH_ERR_UNSUPPORTED;
+  if (v == SKETCH_VARIANT_FLAT_PAIR && !(zt && vpair)) return SKETCH_ERR_UNSUPPORTED;
+  p->variant = v;
+  p->zeta_t = s->zeta;
+
+  if (v == SKETCH_VARIANT_SMEM) {
+    p->hash_mode = 1;
+    p->vec = smem_vec_for(s->zeta);
+    p->wpc = n / 64;
+    p->smem_bytes = sm_bytes;
+    p->replicas = 1;
+    int per_sm = (int)((size_t)s->smem_per_sm / (sm_bytes + 1024));
+    if (per_sm < 1) per_sm = 1;
+    int max_warps_per_sm = 64 / p->wpc;
+    if (per_sm > max_warps_per_sm) per_sm = max_warps_per_sm;
+    if (per_sm > 32) per_sm = 32;
+    int64_t grid = (int64_t)s->sm_count * per_sm;
+    if (o && o->grid_ctas > 0) grid = o->grid_ctas;
+    const int64_t ring = 32;  // NQ*R rows for every layout
+    int64_t rpc = (rows + grid - 1) / grid;
+    rpc = (rpc + ring - 1) / ring * ring;
+    if (rpc < ring) rpc = ring;
+    grid = (rows + rpc - 1) / rpc;
+    if (grid < 1) grid = 1;
+    p->grid = (int)grid;
+    p->rows_per_cta = rpc;
+    return SKETCH_OK;
+  }
+
+  if (v == SKETCH_VARIANT_GENERIC) {
+    p->vec = 1;
+    p->hash_mode = 1;
+  } else {
+    p->vec = (v == SKETCH_VARIANT_FLAT_PAIR) ? vpair : vmax;
+  }
+  int P = (o && o->replicas > 0) ? o->replicas : 0;
+  if (P == 0) {
+    // auto: enough partial sketches to spread same-line RED traffic over L2, capped at 16 MiB of scratch
+    size_t one = (size_t)s->d * n * (f16 ? 2 : 4);
+    size_t cap = (16u << 20) / (one ? one : 1);
+    P = (int)(cap < 1 ? 1 : cap > 8 ? 8 : cap);
+  }
+  if (P > 4096) P = 4096;
+  p->replicas = P;
+  int64_t work_warps;
+  if (v == SKETCH_VARIANT_GENERIC) {
+    work_warps = (rows * (int64_t)n + 31) / 32;
+  } else {
+    int hb = 32 / s->zeta;
+    work_warps = (rows + hb - 1) / hb;
+  }
+  int64_t grid = (work_warps + 7) / 8;
+  int64_t cap = (int64_t)s->sm_count * 8;
+  if (grid > cap) grid = cap;
+  if (grid < 1) grid = 1;
+  if (o && o->grid_ctas > 0) grid = o->grid_ctas;
+  p->grid = (int)grid;
+  (void)rounding;
+  return SKETCH_OK;
+}
+
+sk::ScatterArgs make_args(const sketch* s, const float* A, int n, int64_t lda, void* B, int64_t row_begin,
+                          int64_t rows, uint64_t sr_seed, int vec) {
+  sk::ScatterArgs a;
+  a.A = A;
+  a.lda = lda;
+  a.row_begin = row_begin;
+  a.rows = rows;
+  a.B = B;
+  a.replica_stride = (int64_t)s->d * n;
+  a.replicas = 1;
+  a.n = n;
+  a.zeta = s->zeta;
+  a.db = s->db;
+  a.seed = s->seed;
+  a.sr_seed = sr_seed;
+  a.scale = s->scale;
+  a.cpr = (uint32_t)(n / (vec > 0 ? vec : 1));
+  a.cpr_magic = (a.cpr <= 1) ? 0u : (uint32_t)(((1ull << 32) + a.cpr - 1) / a.cpr);
+  a.packed = nullptr;
+  return a;
+}
+
+template <int ZETA, int VEC, bool F16, int RND>
+int launch_flat_t(const sk::ScatterArgs& a, int grid, int packed_width, cudaStream_t st) {
+  if (packed_width == 2) sk::k_flat<ZETA, VEC, F16, RND, uint16_t><<<grid, sk::kFlatThreads, 0, st>>>(a);
+  else if (packed_width == 4) sk::k_flat<ZETA, VEC, F16, RND, uint32_t><<<grid, sk::kFlatThreads, 0, st>>>(a);
+  else sk::k_flat<ZETA, VEC, F16, RND, uint8_t><<<grid, sk::kFlatThreads, 0, st>>>(a);
+  return launch_check("k_flat");
+}
+
+template <int ZETA, bool F16, int RND>
+int launch_flat_v(const sk::ScatterArgs& a, int vec, int grid, int pw, cudaStream_t st) {
+  if constexpr (F16) {
+    switch (vec) {
+      case 8: return launch_flat_t<ZETA, 8, true, RND>(a, grid, pw, st);
+      case 4: return launch_flat_t<ZETA, 4, true, RND>(a, grid, pw, st);
+      case 2: return launch_flat_t<ZETA, 2, true, RND>(a, grid, pw, st);
+    }
+  } else {
+    switch (vec) {
+      case 4: return launch_flat_t<ZETA, 4, false, 0>(a, grid, pw, st);
+      case 2: return launch_flat_t<ZETA, 2, false, 0>(a, grid, pw, st);
+      case 1: return launch_flat_t<ZETA, 1, false, 0>(a, grid, pw, st);
+    }
+  }
+  return SKETCH_ERR_UNSUPPORTED;
+}
+
+template <bool F16, int RND>
+int launch_flat(const sk::ScatterArgs& a, int zeta, int vec, int grid, int pw, cudaStream_t st) {
+  switch (zeta) {
+    case 1: return launch_flat_v<1, F16, RND>(a, vec, grid, pw, st);
+    case 2: return launch_flat_v<2, F16, RND>(a, vec, grid, pw, st);
+    case 4: return launch_flat_v<4, F16, RND>(a, vec, grid, pw, st);
+    case 8: return launch_flat_v<8, F16, RND>(a, vec, grid, pw, st);
+  }
+  return SKETCH_ERR_UNSUPPORTED;
+}
+
+template <int ZETA, int VEC, int LPR, int RND, int NQ>
+int launch_smem_t(const sk::SmemArgs& g, const Plan& p, cudaStream_t st) {
+  if (p.wpc <= 4) {
+    auto k = sk::k_smem<ZETA, VEC, LPR, RND, NQ, 4>;
+    CU_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_bytes));
+    k<<<p.grid, p.wpc * 32, p.smem_bytes, st>>>(g);
+  } else {
+    auto k = sk::k_smem<ZETA, VEC, LPR, RND, NQ, 16>;
+    CU_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_bytes));
+    k<<<p.grid, p.wpc * 32, p.smem_bytes, st>>>(g);
+  }
+  return launch_check("k_smem");
+}
+
+template <int RND>
+int launch_smem(const sk::SmemArgs& g, const Plan& p, cudaStream_t st) {
+  switch (p.zeta_t) {
+    case 1: return launch_smem_t<1, 2, 32, RND, 32>(g, p, st);
+    case 2: return launch_smem_t<2, 4, 16, RND, 16>(g, p, st);
+    case 4: return launch_smem_t<4, 8, 8, RND, 8>(g, p, st);
+    case 8: return launch_smem_t<8, 8, 8, RND, 8>(g, p, st);
+  }
+  return SKETCH_ERR_UNSUPPORTED;
+}
+
+int ensure_packed(sketch* s, cudaStream_t st) {
+  if (s->packed) return SKETCH_OK;
+  int width = (s->d <= 32768) ? 2 : 4;
+  int64_t total = s->m * (int64_t)s->zeta;
+  size_t have = 0;
+  int rc = ensure_scratch(&s->packed, &have, (size_t)total * width);
+  if (rc) return rc;
+  int rc2 = ensure_device(s);
+  if (rc2) return rc2;
+  int64_t blocks = (total + 255) / 256;
+  int64_t cap = (int64_t)s->sm_count * 16;
+  int grid = (int)(blocks < cap ? blocks : cap);
+  if (grid < 1) grid = 1;
+  if (width == 2) sk::k_hash_pack<uint16_t><<<grid, 256, 0, st>>>(s->seed, total, (uint32_t)s->zeta, s->db, (uint16_t*)s->packed);
+  else sk::k_hash_pack<uint32_t><<<grid, 256, 0, st>>>(s->seed, total, (uint32_t)s->zeta, s->db, (uint32_t*)s->packed);
+  rc = launch_check("k_hash_pack");
+  if (rc) return rc;
+  s->packed_width = width;
+  return SKETCH_OK;
+}
+
+int validate_apply(const sketch* s, const void* A, int32_t n, int64_t lda, const void* B, bool f16,
+                   const sketch_opts_t* o, int64_t* row_begin, int64_t* rows) {
+  if (!s || !A || !B) return SKETCH_ERR_NULL;
+  if (n <= 0) return SKETCH_ERR_INVALID;
+  if (lda < n) return SKETCH_ERR_LDA;
+  if (!aligned(A, 4) || !aligned(B, 4)) return SKETCH_ERR_ALIGNMENT;  // f16: packed RED works on 4-byte words
+  (void)f16;
+  int64_t rb = o ? o->row_begin : 0;
+  int64_t r = o ? o->rows : 0;
+  if (o && o->reserved != 0) return SKETCH_ERR_INVALID;
+  if (rb < 0 || r < 0 || rb > s->m) return SKETCH_ERR_INVALID;
+  if (r == 0) r = s->m - rb;
+  if (rb + r > s->m) return SKETCH_ERR_INVALID;
+  *row_begin = rb;
+  *rows = r;
+  return SKETCH_OK;
+}
+
+int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void* B, bool f16, int rounding,
+                 uint64_t sr_seed, const sketch_opts_t* o, void* stream) {
+  sketch* s = const_cast<sketch*>(cs);
+  int64_t row_begin = 0, rows = 0;
+  int rc = validate_apply(s, A, n, lda, B, f16, o, &row_begin, &rows);
+  if (rc) return rc;
+  if (f16 && rounding != SKETCH_RN && rounding != SKETCH_SR) return SKETCH_ERR_INVALID;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  Plan p;
+  rc = make_plan(s, n, lda, A, B, f16, rounding, o, rows, &p);
+  if (rc) return rc;
+  const int accumulate = o ? o->accumulate : 0;
+  const size_t elem = f16 ? 2 : 4;
+  const size_t out_bytes = (size_t)s->d * n * elem;
+
+  if (p.variant == SKETCH_VARIANT_SMEM) {
+    if (!accumulate) CU_TRY(cudaMemsetAsync(B, 0, out_bytes, st));  // a0
+    if (rows == 0) return SKETCH_OK;
+    sk::SmemArgs g;
+    g.s = make_args(s, A, n, lda, B, row_begin, rows, sr_seed, p.vec);
+    g.rows_per_cta = p.rows_per_cta;
+    g.d = s->d;
+    return rounding == SKETCH_SR ? launch_smem<1>(g, p, st) : launch_smem<0>(g, p, st);
+  }
+
+  // flat / generic: RED into B itself (P == 1) or into P partial sketches folded afterwards
+  void* target = B;
+  int P = p.replicas;
+  if (P > 1) {
+    rc = ensure_scratch(&s->rep, &s->rep_bytes, out_bytes * P);
+    if (rc) return rc;
+    target = s->rep;
+    CU_TRY(cudaMemsetAsync(target, 0, out_bytes * P, st));
+  } else if (!accumulate) {
+    CU_TRY(cudaMemsetAsync(B, 0, out_bytes, st));
+  }
+  int pw = 0;
+  if (p.hash_mode == 2 && p.variant != SKETCH_VARIANT_GENERIC) {
+    rc = ensure_packed(s, st);
+    if (rc) return rc;
+    pw = s->packed_width;
+  }
+  if (rows > 0) {
+    sk::ScatterArgs a = make_args(s, A, n, lda, target, row_begin, rows, sr_seed, p.vec);
+    a.replicas = P;
+    a.packed = pw ? s->packed : nullptr;
+    if (p.variant == SKETCH_VARIANT_GENERIC) {
+      if (!f16) sk::k_generic<false, 0><<<p.grid, sk::kFlatThreads, 0, st>>>(a);
+      else if (rounding == SKETCH_SR) sk::k_generic<true, 1><<<p.grid, sk::kFlatThreads, 0, st>>>(a);
+      else sk::k_generic<true, 0><<<p.grid, sk::kFlatThreads, 0, st>>>(a);
+      rc = launch_check("k_generic");
+    } else if (!f16) {
+      rc = launch_flat<false, 0>(a, s->zeta, p.vec, p.grid, pw, st);
+    } else if (rounding == SKETCH_SR) {
+      rc = launch_flat<true, 1>(a, s->zeta, p.vec, p.grid, pw, st);
+    } else {
+      rc = launch_flat<true, 0>(a, s->zeta, p.vec, p.grid, pw, st);
+    }
+    if (rc) return rc;
+  }
+  if (P > 1) {
+    int64_t count = (int64_t)s->d * n;
+    int grid = (int)((count + 255) / 256);
+    if (grid > s->sm_count * 8) grid = s->sm_count * 8;
+    if (f16) sk::k_reduce_replicas<true><<<grid, 256, 0, st>>>(target, count, P, B, count, accumulate);
+    else sk::k_reduce_replicas<false><<<grid, 256, 0, st>>>(target, count, P, B, count, accumulate);
+    rc = launch_check("k_reduce_replicas");
+    if (rc) return rc;
+  }
+  return SKETCH_OK;
+}
+
+int ensure_host_path(sketch* s) {
+  if (s->host_ready) return SKETCH_OK;
+  CU_TRY(cudaStreamCreateWithFlags(&s->st_copy, cudaStreamNonBlocking));
+  CU_TRY(cudaStreamCreateWithFlags(&s->st_comp, cudaStreamNonBlocking));
+  for (int k = 0; k < 2; ++k) {
+    CU_TRY(cudaEventCreateWithFlags(&s->ev_copied[k], cudaEventDisableTiming));
+    CU_TRY(cudaEventCreateWithFlags(&s->ev_done[k], cudaEventDisableTiming));
+  }
+  s->host_ready = 1;
+  return SKETCH_OK;
+}
+
+int apply_host(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void* B, bool f16, int rounding,
+               uint64_t sr_seed, const sketch_opts_t* o) {
+  sketch* s = const_cast<sketch*>(cs);
+  if (!s || !A || !B) return SKETCH_ERR_NULL;
+  if (n <= 0) return SKETCH_ERR_INVALID;
+  if (lda < n) return SKETCH_ERR_LDA;
+  int64_t rb = o ? o->row_begin : 0, rows = o ? o->rows : 0;
+  if (rb < 0 || rows < 0 || rb > s->m) return SKETCH_ERR_INVALID;
+  if (rows == 0) rows = s->m - rb;
+  if (rb + rows > s->m) return SKETCH_ERR_INVALID;
+  int rc = ensure_host_path(s);
+  if (rc) return rc;
+  const size_t elem = f16 ? 2 : 4;
+  const size_t out_bytes = (size_t)s->d * n * elem;
+  // staging: two buffers of ~256 MiB, whole rows, row count a multiple of 32
+  const size_t row_bytes = (size_t)n * 4;
+  int64_t chunk_rows = (int64_t)((256u << 20) / row_bytes);
+  chunk_rows = chunk_rows / 32 * 32;
+  if (chunk_rows < 32) chunk_rows = 32;
+  if (chunk_rows > rows) chunk_rows = (rows + 31) / 32 * 32;
+  const size_t chunk_bytes = (size_t)chunk_rows * row_bytes;
+  if (s->stage_bytes < chunk_bytes) {
+    for (int k = 0; k < 2; ++k) {
+      size_t have = s->stage[k] ? s->stage_bytes : 0;
+      rc = ensure_scratch(&s->stage[k], &have, chunk_bytes);
+      if (rc) return rc;
+    }
+    s->stage_bytes = chunk_bytes;
+  }
+  rc = ensure_scratch(&s->bdev, &s->bdev_bytes, out_bytes);
+  if (rc) return rc;
+  sketch_opts_t oo;
+  memset(&oo, 0, sizeof(oo));
+  if (o) oo = *o;
+  const int user_acc = o ? o->accumulate : 0;
+  if (user_acc) CU_TRY(cudaMemcpyAsync(s->bdev, B, out_bytes, cudaMemcpyHostToDevice, s->st_comp));
+  else if (rows == 0) CU_TRY(cudaMemsetAsync(s->bdev, 0, out_bytes, s->st_comp));
+  int k = 0;
+  for (int64_t r0 = 0; r0 < rows; r0 += chunk_rows, ++k) {
+    int64_t nr = rows - r0 < chunk_rows ? rows - r0 : chunk_rows;
+    int b = k & 1;
+    if (k >= 2) CU_TRY(cudaStreamWaitEvent(s->st_copy, s->ev_done[b], 0));
+    const float* src = A + r0 * lda;
+    if (lda == n) CU_TRY(cudaMemcpyAsync(s->stage[b], src, (size_t)nr * row_bytes, cudaMemcpyHostToDevice, s->st_copy));
+    else CU_TRY(cudaMemcpy2DAsync(s->stage[b], row_bytes, src, (size_t)lda * 4, row_bytes, (size_t)nr, cudaMemcpyHostToDevice, s->st_copy));
+    CU_TRY(cudaEventRecord(s->ev_copied[b], s->st_copy));
+    CU_TRY(cudaStreamWaitEvent(s->st_comp, s->ev_copied[b], 0));
+    oo.row_begin = rb + r0;
+    oo.rows = nr;
+    oo.accumulate = (k > 0 || user_acc) ? 1 : 0;
+    rc = apply_device(s, (const float*)s->stage[b], n, n, s->bdev, f16, rounding, sr_seed, &oo, s->st_comp);
+    if (rc) return rc;
+    CU_TRY(cudaEventRecord(s->ev_done[b], s->st_comp));
+  }
+  CU_TRY(cudaMemcpyAsync(B, s->bdev, out_bytes, cudaMemcpyDeviceToHost, s->st_comp));
+  CU_TRY(cudaStreamSynchronize(s->st_comp));
+  return SKETCH_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
+extern "C" {
+
+int sketch_create(int64_t m, int32_t d, int32_t zeta, uint64_t seed, sketch_t** out) {
+  if (!out) return SKETCH_ERR_NULL;
+  *out = nullptr;
+  if (m <= 0 || d <= 0 || zeta < 1) return SKETCH_ERR_INVALID;
+  if (d % zeta != 0) return SKETCH_ERR_DIVISIBILITY;
+  if ((uint64_t)m > (1ull << 62) / (uint64_t)zeta) return SKETCH_ERR_INVALID;
+  sketch* s = new (std::nothrow) sketch;
+  if (!s) return SKETCH_ERR_NOMEM;
+  memset(s, 0, sizeof(*s));
+  s->m = m;
+  s->d = d;
+  s->zeta = zeta;
+  s->db = (uint32_t)(d / zeta);
+  s->seed = seed;
+  s->scale = (float)(1.0 / std::sqrt((double)zeta));  // correctly rounded from FP64 (R5)
+  *out = s;
+  return SKETCH_OK;
+}
+
+int sketch_destroy(sketch_t* s) {
+  if (!s) return SKETCH_OK;
+  if (s->rep) cudaFree(s->rep);
+  if (s->packed) cudaFree(s->packed);
+  for (int k = 0; k < 2; ++k)
+    if (s->stage[k]) cudaFree(s->stage[k]);
+  if (s->bdev) cudaFree(s->bdev);
+  if (s->host_ready) {
+    cudaStreamDestroy(s->st_copy);
+    cudaStreamDestroy(s->st_comp);
+    for (int k = 0; k < 2; ++k) {
+      cudaEventDestroy(s->ev_copied[k]);
+      cudaEventDestroy(s->ev_done[k]);
+    }
+  }
+  delete s;
+  return SKETCH_OK;
+}
+
+int sketch_hashes_dump(const sketch_t* cs, int32_t* bucket_dev, uint8_t* signbit_dev, void* stream) {
+  sketch* s = const_cast<sketch*>(cs);
+  if (!s || !bucket_dev || !signbit_dev) return SKETCH_ERR_NULL;
+  int rc = ensure_device(s);
+  if (rc) return rc;
+  int64_t total = s->m * (int64_t)s->zeta;
+  int64_t blocks = (total + 255) / 256;
+  int64_t cap = (int64_t)s->sm_count * 16;
+  int grid = (int)(blocks < cap ? blocks : cap);
+  sk::k_hash_dump<<<grid, 256, 0, reinterpret_cast<cudaStream_t>(stream)>>>(s->seed, total, (uint32_t)s->zeta, s->db,
+                                                                            bucket_dev, signbit_dev);
+  return launch_check("k_hash_dump");
+}
+
+int sketch_precompute_hashes(sketch_t* s, void* stream) {
+  if (!s) return SKETCH_ERR_NULL;
+  return ensure_packed(s, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int sketch_apply_f32acc(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, float* B_dev, void* stream) {
+  return apply_device(s, A_dev, n, lda, B_dev, false, 0, 0, nullptr, stream);
+}
+
+int sketch_apply_f16acc(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev, int rounding,
+                        uint64_t sr_seed, void* stream) {
+  return apply_device(s, A_dev, n, lda, B_dev, true, rounding, sr_seed, nullptr, stream);
+}
+
+int sketch_apply_f32acc_ex(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, float* B_dev,
+                           const sketch_opts_t* opts, void* stream) {
+  return apply_device(s, A_dev, n, lda, B_dev, false, 0, 0, opts, stream);
+}
+
+int sketch_apply_f16acc_ex(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev, int rounding,
+                           uint64_t sr_seed, const sketch_opts_t* opts, void* stream) {
+  return apply_device(s, A_dev, n, lda, B_dev, true, rounding, sr_seed, opts, stream);
+}
+
+int sketch_apply_f32acc_host(const sketch_t* s, const float* A_host, int32_t n, int64_t lda, float* B_host,
+                             const sketch_opts_t* opts) {
+  return apply_host(s, A_host, n, lda, B_host, false, 0, 0, opts);
+}
+
+int sketch_apply_f16acc_host(const sketch_t* s, const float* A_host, int32_t n, int64_t lda, void* B_host, int rounding,
+                             uint64_t sr_seed, const sketch_opts_t* opts) {
+  if (rounding != SKETCH_RN && rounding != SKETCH_SR) return SKETCH_ERR_INVALID;
+  return apply_host(s, A_host, n, lda, B_host, true, rounding, sr_seed, opts);
+}
+
+int sketch_red_probe(void* sketch_dev, int32_t d, int32_t n, int32_t kind, int32_t replicas, int32_t grid_ctas,
+                     int32_t iters, uint64_t* red_ops_out, void* stream) {
+  if (!sketch_dev) return SKETCH_ERR_NULL;
+  if (d <= 0 || n <= 0 || kind < 0 || kind > 5 || replicas < 1 || grid_ctas < 1 || iters < 0) return SKETCH_ERR_INVALID;
+  const int vec[6] = {2, 4, 8, 1, 2, 4};
+  if (n % vec[kind] != 0) return SKETCH_ERR_INVALID;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  switch (kind) {
+    case 0: sk::k_red_probe<0><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
+    case 1: sk::k_red_probe<1><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
+    case 2: sk::k_red_probe<2><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
+    case 3: sk::k_red_probe<3><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
+    case 4: sk::k_red_probe<4><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
+    default: sk::k_red_probe<5><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
+  }
+  if (red_ops_out) *red_ops_out = (uint64_t)grid_ctas * sk::kFlatThreads * (uint64_t)iters;
+  return launch_check("k_red_probe");
+}
+
+int sketch_plan(const sketch_t* cs, int32_t n, int64_t lda, int is_f16, int rounding, const sketch_opts_t* opts,
+                int32_t* variant_out, int32_t* replicas_out, int32_t* hash_mode_out, int32_t* grid_out) {
+  sketch* s = const_cast<sketch*>(cs);
+  if (!s) return SKETCH_ERR_NULL;
+  if (n <= 0) return SKETCH_ERR_INVALID;
+  if (lda < n) return SKETCH_ERR_LDA;
+  int64_t rb = opts ? opts->row_begin : 0, rows = opts ? opts->rows : 0;
+  if (rows == 0) rows = s->m - rb;
+  Plan p;
+  // plan for 256-byte aligned buffers (what cudaMalloc returns)
+  int rc = make_plan(s, n, lda, reinterpret_cast<const void*>(256), reinterpret_cast<const void*>(256), is_f16 != 0,
+                     rounding, opts, rows, &p);
+  if (rc) return rc;
+  if (variant_out) *variant_out = p.variant;
+  if (replicas_out) *replicas_out = p.replicas;
+  if (hash_mode_out) *hash_mode_out = p.hash_mode;
+  if (grid_out) *grid_out = p.grid;
+  return SKETCH_OK;
+}
+
+uint64_t sketch_launch_count(void) { return g_launches.load(); }
+
+const char* sketch_strerror(int code) {
+  switch (code) {
+    case SKETCH_OK: return "ok";
+    case SKETCH_ERR_INVALID: return "invalid argument value";
+    case SKETCH_ERR_NULL: return "null pointer";
+    case SKETCH_ERR_DIVISIBILITY: return "d is not divisible by zeta";
+    case SKETCH_ERR_LDA: return "lda < n";
+    case SKETCH_ERR_ALIGNMENT: return "buffer is not sufficiently aligned";
+    case SKETCH_ERR_UNSUPPORTED: return "the forced variant does not support this shape";
+    case SKETCH_ERR_CUDA: return "CUDA runtime error (see sketch_last_error)";
+    case SKETCH_ERR_NOMEM: return "out of memory";
+  }
+  return "unknown error code";
+}
+
+const char* sketch_last_error(void) { return g_last_error; }
+
+const char* sketch_version(void) { return "sparse_sketch 0.1 sm_100a"; }
+
+}  // extern "C"
