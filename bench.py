@@ -1,0 +1,373 @@
+#!/usr/bin/env python
+"""bench.py -- SparseStack zeta=4 sketch formation on B200: GB/s of A read and fraction of the roofline.
+
+One "step" = one complete FP16-accumulate sketch (zero-init + hash + stream A + sign/scale + RN16 +
+scatter-accumulate + flush, "complete sketch") of the workload's
+resident m x n FP32 matrix through the C ABI.  Default workload: BASELINE.json configs[4]'s peak
+point (m = 2^25, n = 128, d = 256, zeta = 4; A = 16 GiB > L2, so no flush is needed between steps).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2|c3|c4|c5] [--variant auto|...]
+    python bench.py --impl reference ...        # the CPU oracle, as it stands, on the host cores
+
+N > 1 (torchrun): every rank sketches its own m-row shard (global row indices rank*m ...) of an
+(N*m) x n matrix into a private sketch -- no data-path collective inside the scatter -- and the N
+partial sketches (64 KiB each) are summed with one NCCL all-reduce.  Weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+WORKLOADS = {
+    # name: (m, n, d, zeta, matrix_seed)   BASELINE.json configs[1..4]
+    "c1": (4096, 16, 32, 4, 0),
+    "c2": (1 << 20, 64, 128, 4, 1),
+    "c3": (1 << 22, 128, 256, 4, 2),
+    "c4": (1 << 23, 256, 1024, 4, 3),
+    "c5": (1 << 25, 128, 256, 4, 4),
+}
+VARIANTS = {"auto": 0, "flat_pair": 1, "flat_vec": 2, "smem": 3, "generic": 4}
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` captures (profiles/*.md name the commands); None until captured.
+NCU_TRAFFIC_BYTES = {}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p)), "measured (MEASURED_PEAKS.json)"
+    return {"hbm_gbs": 6650.0}, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (profiling recipe's clocks line)."""
+
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._pump, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for ln in self.proc.stdout:
+            self.rows.append((time.time(), ln.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        for ts, ln in self.rows:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                clk, mxc = float(f[1]), float(f[2])
+            except ValueError:
+                continue
+            mx = mxc
+            if t0 - 0.05 <= ts <= t1 + 0.15:
+                sm.append(clk)
+                for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                    if val.lower().startswith("active"):
+                        reasons.add(name)
+        if not sm:  # region shorter than the sampling period: use the closest samples
+            for ts, ln in self.rows[-3:]:
+                f = [x.strip() for x in ln.split(",")]
+                try:
+                    sm.append(float(f[1]))
+                except (ValueError, IndexError):
+                    pass
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def algorithmic_bytes(m, n, d, out_elem=2):
+    """per input element 4 B read once; output b*d*n written once (Eq. 5's 4mn term + the sketch)."""
+    return 4 * m * n + out_elem * d * n
+
+
+# ------------------------------------------------------------------------------------------- reference arm
+def run_reference(args):
+    """The oracle as it stands (never tuned), on the host cores, on a bounded sample of the workload."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    import numpy as np
+
+    import oracle
+    import workloads as wl
+
+    m, n, d, zeta, mseed = WORKLOADS[args.workload]
+    cores = os.cpu_count() or 1
+    threads = min(cores, 64)
+    sample_rows = min(m, args.ref_rows)
+    A = wl.gaussian(sample_rows, n, mseed)
+    seed = wl.sketch_seed(0)
+    oracle.build()
+    for _ in range(max(0, min(args.warmup, 1))):
+        oracle.f64_sketch(seed, d, zeta, A[: sample_rows // 8], threads=threads)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.f64_sketch(seed, d, zeta, A, threads=threads)
+    dt = (time.perf_counter() - t0) / args.steps
+    gbs = sample_rows * n * 4 / dt / 1e9
+    line = {
+        "impl": "reference", "metric": "sketch_A_read_GBps", "value": gbs, "unit": "GB/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "%s: SparseStack zeta=%d, m=%d, n=%d, d=%d, A FP32 N(0,1)" % (args.workload, zeta, m, n, d),
+                   "sample": "first %d rows per step" % sample_rows},
+        "cpu_baseline": {"value": gbs, "unit": "GB/s", "cores": threads, "kind": "oracle",
+                         "sample": "oracle FP64 mode (row-chunk-private partials, %d threads) on %d of %d rows" % (threads, sample_rows, m)},
+        "e2e": {"value": gbs, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def cpu_baseline(workload, seconds_hint=15.0):
+    import numpy as np
+
+    import oracle
+    import workloads as wl
+
+    m, n, d, zeta, mseed = WORKLOADS[workload]
+    cores = os.cpu_count() or 1
+    threads = min(cores, 64)
+    seed = wl.sketch_seed(0)
+    rows = min(m, 1 << 17)
+    A = wl.gaussian(rows, n, mseed)
+    t0 = time.perf_counter()
+    oracle.f64_sketch(seed, d, zeta, A, threads=threads)
+    dt = time.perf_counter() - t0
+    # scale the sample to ~seconds_hint/2 of work for the all-core mode, and time one pass
+    rows2 = int(min(m, max(rows, rows * (seconds_hint / 2) / max(dt, 1e-3))))
+    rows2 = min(rows2, 1 << 23)
+    A = wl.gaussian(rows2, n, mseed)
+    t0 = time.perf_counter()
+    oracle.f64_sketch(seed, d, zeta, A, threads=threads)
+    dt_all = time.perf_counter() - t0
+    rows1 = max(1 << 14, rows2 // max(threads, 1))
+    t0 = time.perf_counter()
+    oracle.f64_sketch(seed, d, zeta, A[:rows1], threads=1)
+    dt_one = time.perf_counter() - t0
+    rows16 = max(1 << 12, rows1 // 8)
+    t0 = time.perf_counter()
+    oracle.seq16_sketch(seed, d, zeta, A[:rows16])
+    dt16 = time.perf_counter() - t0
+    return {
+        "value": rows2 * n * 4 / dt_all / 1e9, "unit": "GB/s", "cores": threads, "kind": "oracle",
+        "sample": "oracle FP64 mode, %d threads, first %d of %d rows (%.1f s)" % (threads, rows2, m, dt_all),
+        "single_thread_f64_GBps": rows1 * n * 4 / dt_one / 1e9,
+        "single_thread_seq16_GBps": rows16 * n * 4 / dt16 / 1e9,
+    }
+
+
+# ------------------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import numpy as np
+    import torch
+
+    import paper_2606_20195_b200 as ss
+    import workloads as wl
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+
+        dist = dist_
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    m, n, d, zeta, mseed = WORKLOADS[args.workload]
+    dev = torch.device("cuda", local)
+    seed = wl.sketch_seed(0)
+    sk = ss.Sketch(m * world, d, zeta, seed)   # one map over all shards; rank r owns rows [r*m, (r+1)*m)
+    row_begin = rank * m
+    A = wl.gaussian_device(m, n, mseed + 7919 * rank, dev)
+    out16 = torch.empty((d, n), dtype=torch.float16, device=dev)
+    out32 = torch.empty((d, n), dtype=torch.float32, device=dev)
+    vid = VARIANTS[args.variant]
+    plan16 = sk.plan(n, f16=True, variant=vid, rows=m, row_begin=row_begin)
+    plan32 = sk.plan(n, f16=False, rows=m, row_begin=row_begin)
+    small = m * n * 4 < (512 << 20)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev) if small else None
+
+    def step16():
+        sk.apply_f16acc(A, out=out16, variant=vid, row_begin=row_begin, rows=m, replicas=args.replicas, hash_mode=args.hash_mode)
+        if dist is not None:
+            dist.all_reduce(out16)
+
+    def step32():
+        sk.apply_f32acc(A, out=out32, row_begin=row_begin, rows=m)
+        if dist is not None:
+            dist.all_reduce(out32)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def timed(fn, steps, warmup):
+        for _ in range(warmup):
+            fn()
+        barrier()
+        evs = []
+        l0 = ss.sketch_launch_count()
+        w0 = time.time()
+        for _ in range(steps):
+            if flush is not None:
+                flush.zero_()                      # inputs smaller than 4x L2: flush L2 between steps
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            evs.append((e0, e1))
+        barrier()
+        w1 = time.time()
+        ms = [a.elapsed_time(b) for a, b in evs]
+        total = torch.tensor([sum(ms)], dtype=torch.float64, device=dev)
+        if dist is not None:
+            dist.all_reduce(total, op=dist.ReduceOp.MAX)
+        return float(total.item()) / steps, ms, ss.sketch_launch_count() - l0, (w0, w1)
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    ms16, per16, launches16, (w0, w1) = timed(step16, args.steps, args.warmup)
+    clocks = sampler.stop(w0, w1) if rank == 0 else None
+    ms32, _, _, _ = timed(step32, max(2, args.steps // 2), 3)
+
+    # end to end through the host-buffer entry point: pinned A on the host, H2D + kernels + D2H inside the call
+    e2e = None
+    if not args.no_e2e:
+        try:
+            Ah = torch.empty((m, n), dtype=torch.float32, pin_memory=True)
+            Ah.copy_(A)
+            Bh = torch.empty((d, n), dtype=torch.float16, pin_memory=True)
+            torch.cuda.synchronize()
+
+            def step_e2e():
+                sk.apply_f16acc_host(Ah, out_host=Bh, variant=vid, row_begin=row_begin, rows=m)
+                if dist is not None:
+                    t = Bh.to(dev)
+                    dist.all_reduce(t)
+                    Bh.copy_(t)
+
+            step_e2e()
+            barrier()
+            t0 = time.perf_counter()
+            ksteps = max(1, min(args.steps, 3))
+            for _ in range(ksteps):
+                step_e2e()
+            barrier()
+            dt = torch.tensor([(time.perf_counter() - t0) / ksteps], dtype=torch.float64, device=dev)
+            if dist is not None:
+                dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+            e2e = {"value": world * m * n * 4 / float(dt.item()) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": m * n * 4,
+                   "d2h_bytes_per_step": d * n * 2, "ms_per_step": float(dt.item()) * 1e3, "steps": ksteps,
+                   "api": "sketch_apply_f16acc_host (pinned host A, double-buffered 256 MiB H2D chunks)"}
+            # the two entry points must agree on what they computed (same variant => same partial-sum tree up to RED order)
+            chk = sk.apply_f16acc(A, variant=vid, row_begin=row_begin, rows=m)
+            if dist is not None:
+                dist.all_reduce(chk)
+            diff = (chk.float().cpu() - Bh.float()).norm() / chk.float().norm().cpu()
+            e2e["rel_diff_vs_device_path"] = float(diff)
+            del Ah
+        except (RuntimeError, ss.SketchError) as ex:  # e.g. the box cannot pin 16 GiB
+            e2e = {"value": None, "unit": "GB/s", "h2d_bytes_per_step": m * n * 4, "d2h_bytes_per_step": d * n * 2,
+                   "error": str(ex)[:200]}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    peaks, peak_src = measured_peaks()
+    abytes = algorithmic_bytes(m, n, d, 2)
+    gbs = world * m * n * 4 / (ms16 * 1e-3) / 1e9
+    achieved = abytes / (ms16 * 1e-3) / 1e9          # per GPU: the event bracket holds memset + scatter (+ fold)
+    hbm = float(peaks["hbm_gbs"])
+    red_ops = zeta * m * n // 2
+    line = {
+        "metric": "sketch_A_read_GBps", "value": gbs, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms16, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f16", "data": "synthetic",
+        "config": {"workload": "%s: SparseStack zeta=%d, m=%d, n=%d, d=%d (d=2n), A FP32 row-major N(0,1) %.2f GiB per GPU, FP16-RN accumulate"
+                               % (args.workload, zeta, m, n, d, m * n * 4 / 2**30),
+                   "variant": plan16["variant"], "replicas": plan16["replicas"], "hash_mode": plan16["hash_mode"], "grid": plan16["grid"],
+                   "l2": "input %s L2; %s" % ("<" if small else ">", "512 MiB flush write between steps" if small else "no flush needed"),
+                   "sharding": "rows; rank r hashes global rows [r*m,(r+1)*m); one NCCL all-reduce of the d x n sketch" if world > 1 else "single GPU"},
+        "sketches_per_s": 1e3 / ms16,
+        "contributions_per_s": zeta * m * n * world / (ms16 * 1e-3),
+        "half2_updates_per_s": red_ops * world / (ms16 * 1e-3),
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm,
+                     "traffic": NCU_TRAFFIC_BYTES.get((args.workload, plan16["variant"])), "peak_source": peak_src,
+                     "frac_of_nominal_8TBps": achieved / 8000.0,
+                     "algorithmic_bytes_per_launch": abytes,
+                     "note": "CUDA-event bracket on the launching stream = zero-init memset + scatter kernel (+ replica fold)"},
+        "f32acc": {"ms_per_step": ms32, "GBps": world * m * n * 4 / (ms32 * 1e-3) / 1e9, "variant": plan32["variant"],
+                   "replicas": plan32["replicas"], "f16_speedup_over_f32": ms32 / ms16},
+        "e2e": e2e if e2e is not None else {"value": None, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0, "skipped": True},
+        "gpu_launches": int(launches16),
+        "clocks": clocks,
+        "per_step_ms": per16,
+        "paper_context": "H200 NVL (PAPER.md:320-322): FP16 SS zeta=4 7.11 ms for 8 GiB (1.21 TB/s), up to 1.91x its FP32 scatter",
+    }
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(args.workload)
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c5", choices=sorted(WORKLOADS))
+    ap.add_argument("--variant", default="auto", choices=sorted(VARIANTS))
+    ap.add_argument("--replicas", type=int, default=0)
+    ap.add_argument("--hash-mode", type=int, default=0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-rows", type=int, default=1 << 21, help="rows per step of the reference arm's bounded sample")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                           # timing rule: W >= 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

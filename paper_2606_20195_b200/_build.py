@@ -11,7 +11,7 @@ HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libsparse_sketch.so"
 SOURCES = [CSRC / "sparse_sketch.cu"]
-DEPS = SOURCES + [CSRC / "kernels.cuh", CSRC / "device_util.cuh", HERE.parent / "include" / "sparse_sketch.h"]
+DEPS = SOURCES + [CSRC / "kernels.cuh", CSRC / "kernel_smem.cuh", CSRC / "device_util.cuh", HERE.parent / "include" / "sparse_sketch.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -3,7 +3,7 @@
 //   k_hash_dump / k_hash_pack   a1  hash stage (dump for tests, packed array for hash_mode=2)
 //   k_flat<...>                 a2-a6 streaming scatter with result-discarding global RED
 //                               (the paper's Listings 1/2 restated with shared hashes + vector RED)
-//   k_smem<...>                 a2-a5 shared-memory-privatised FP16 partial sketch per CTA
+//   k_smem<...>                 (kernel_smem.cuh) a2-a5 shared-memory-privatised FP16 partial sketch per CTA
 //   k_generic<...>              any-n / any-alignment scalar fallback
 //   k_reduce_replicas<...>      sums the P L2-resident partial sketches of the flat variant
 //   k_red_probe<...>            L2 atomic-throughput microbenchmark (roofline term 2)
@@ -237,170 +237,6 @@ __global__ void k_reduce_replicas(const void* __restrict__ rep, int64_t replica_
       float acc = accumulate ? o[k] : 0.f;
       for (int p = 0; p < replicas; ++p) acc = __fadd_rn(acc, r[(int64_t)p * replica_stride + k]);
       o[k] = acc;
-    }
-  }
-}
-
-// ------------------------------------------------------------------------------------------------
-// Shared-memory-privatised FP16 scatter.
-//
-// Each CTA keeps one private d x n FP16 partial sketch in shared memory and streams a contiguous range
-// of rows.  sm_100a has no native shared-memory FP16 add (atomicAdd on smem assembles to a CAS loop),
-// so every sketch word has exactly one owning lane at any time and is updated with plain
-// LDS / HADD2 / STS:
-//   - warp w of the CTA owns the column slice [w*CW, (w+1)*CW), CW = LPR*VEC; no two warps of a CTA
-//     ever touch the same word;
-//   - inside a warp the 32 lanes are R = 32/LPR rows x LPR column chunks; at step t the lanes of row r
-//     update stack block (r + t) mod ZETA.  Blocks are disjoint row ranges of the sketch
-//     (PAPER.md:59-63), so with R <= ZETA the R rows of a step can never collide -- no conflict
-//     detection, no atomics;
-//   - steps are separated by __syncwarp() (row r+1 touched block (r+t+1) mod ZETA one step earlier).
-// A is read straight into registers with 128/256-bit streaming loads through an NQ-deep register ring
-// (NQ row groups in flight per warp), because staging A through shared memory would add 8 B/float to
-// a shared-memory pipe that the 2*2*ZETA B/float of read-modify-write traffic already loads to ~2/3.
-// At the end the CTA flushes its partial sketch into B with 16-byte result-discarding REDs.
-// ------------------------------------------------------------------------------------------------
-struct SmemArgs {
-  ScatterArgs s;
-  int64_t rows_per_cta;  // multiple of the hash batch
-  int32_t d;
-};
-
-template <int ZETA, int VEC, int LPR, int ROUNDING, int NQ, int MAXW>
-__global__ void __launch_bounds__(MAXW * 32) k_smem(SmemArgs g) {
-  constexpr int R = 32 / LPR;                 // rows per warp step
-  static_assert(R <= ZETA, "rotation needs R <= ZETA");
-  static_assert(32 % ZETA == 0 && LPR >= ZETA, "layout");
-  constexpr int HB = 32 / ZETA;               // rows per hash batch
-  constexpr int QPB = HB / R;                 // row groups per hash batch
-  static_assert(NQ % QPB == 0, "ring must hold whole hash batches");
-  constexpr int CW = LPR * VEC;               // columns per warp
-  constexpr int NH = VEC / 2;                 // half2 words per lane
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  const ScatterArgs& a = g.s;
-  const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const uint32_t r = lane / LPR, pcol = lane % LPR;
-  const int32_t n = a.n;
-  const uint32_t row_pitch = (uint32_t)n * 2u;  // bytes per sketch row in smem
-
-  // ---- a0 (private part): zero the partial sketch
-  {
-    uint4* z = reinterpret_cast<uint4*>(smem_raw);
-    const uint32_t n16 = (uint32_t)g.d * row_pitch / 16u;
-    for (uint32_t k = tid; k < n16; k += blockDim.x) z[k] = make_uint4(0, 0, 0, 0);
-  }
-  __syncthreads();
-
-  const int64_t cta_r0 = (int64_t)blockIdx.x * g.rows_per_cta;
-  const int64_t cta_r1 = min(a.rows, cta_r0 + g.rows_per_cta);
-  const uint32_t col0 = warp * CW + pcol * VEC;               // first column of this lane
-  unsigned char* my_col = smem_raw + col0 * 2u;
-  const float* Acol = a.A + col0;
-  const uint32_t npairs = ((uint32_t)n + 1u) >> 1;
-
-  if (cta_r0 < cta_r1) {
-    // register ring of NQ row groups
-    float buf[NQ][VEC];
-    auto load_group = [&](int64_t grow0, float (&dst)[VEC]) {  // grow0: local row of the group's first row
-      int64_t row = grow0 + r;
-      if (row < cta_r1) {
-        ld_stream<VEC>(Acol + row * a.lda, dst);
-      } else {
-#pragma unroll
-        for (int k = 0; k < VEC; ++k) dst[k] = 0.f;
-      }
-    };
-    constexpr int RING_ROWS = NQ * R;
-#pragma unroll
-    for (int q = 0; q < NQ; ++q) load_group(cta_r0 + (int64_t)q * R, buf[q]);
-
-    for (int64_t base = cta_r0; base < cta_r1; base += RING_ROWS) {
-#pragma unroll
-      for (int hb = 0; hb < NQ / QPB; ++hb) {
-        const int64_t b0 = base + (int64_t)hb * HB;  // first local row of this hash batch
-        // hash stage: lane l -> (row b0 + l/ZETA, block l%ZETA)
-        uint32_t e;
-        {
-          uint64_t ctr = (uint64_t)(a.row_begin + b0) * ZETA + lane;
-          e = hash_entry(a.seed, ctr, lane % ZETA, a.db);
-        }
-#pragma unroll
-        for (int qq = 0; qq < QPB; ++qq) {
-          const int q = hb * QPB + qq;
-          float p[VEC];
-#pragma unroll
-          for (int k = 0; k < VEC; ++k) p[k] = buf[q][k] * a.scale;
-          // refill this ring slot with the group NQ steps ahead
-          load_group(base + RING_ROWS + (int64_t)q * R, buf[q]);
-          uint32_t qv[NH];
-          if constexpr (ROUNDING == 0) {
-#pragma unroll
-            for (int k = 0; k < NH; ++k) qv[k] = pack_rn(p[2 * k], p[2 * k + 1]);
-          }
-          const uint32_t rib = (uint32_t)qq * R + r;  // row in batch
-#pragma unroll
-          for (int t = 0; t < ZETA; ++t) {
-            const uint32_t jt = (r + t) % ZETA;
-            const uint32_t ej = __shfl_sync(0xFFFFFFFFu, e, rib * ZETA + jt);
-            unsigned char* addr = my_col + entry_bucket(ej) * row_pitch;
-            uint32_t w[NH];
-            if constexpr (ROUNDING == 0) {
-              const uint32_t sm = entry_signmask_h2(ej);
-#pragma unroll
-              for (int k = 0; k < NH; ++k) w[k] = qv[k] ^ sm;
-            } else {
-              const uint32_t sf = entry_signmask_f32(ej);
-              const uint64_t sr_ctr =
-                  ((uint64_t)(a.row_begin + b0 + rib) * ZETA + jt) * npairs + (uint64_t)(col0 >> 1);
-#pragma unroll
-              for (int k = 0; k < NH; ++k)
-                w[k] = pack_sr(__uint_as_float(__float_as_uint(p[2 * k]) ^ sf),
-                               __uint_as_float(__float_as_uint(p[2 * k + 1]) ^ sf), a.sr_seed, sr_ctr + k);
-            }
-            // read-modify-write of the lane's NH half2 words: sole owner, no atomics
-            if constexpr (NH == 4) {
-              uint4 acc = *reinterpret_cast<uint4*>(addr);
-              __half2 x0 = __hadd2(*reinterpret_cast<__half2*>(&acc.x), *reinterpret_cast<__half2*>(&w[0]));
-              __half2 x1 = __hadd2(*reinterpret_cast<__half2*>(&acc.y), *reinterpret_cast<__half2*>(&w[1]));
-              __half2 x2 = __hadd2(*reinterpret_cast<__half2*>(&acc.z), *reinterpret_cast<__half2*>(&w[2]));
-              __half2 x3 = __hadd2(*reinterpret_cast<__half2*>(&acc.w), *reinterpret_cast<__half2*>(&w[3]));
-              acc.x = *reinterpret_cast<uint32_t*>(&x0);
-              acc.y = *reinterpret_cast<uint32_t*>(&x1);
-              acc.z = *reinterpret_cast<uint32_t*>(&x2);
-              acc.w = *reinterpret_cast<uint32_t*>(&x3);
-              *reinterpret_cast<uint4*>(addr) = acc;
-            } else if constexpr (NH == 2) {
-              uint2 acc = *reinterpret_cast<uint2*>(addr);
-              __half2 x0 = __hadd2(*reinterpret_cast<__half2*>(&acc.x), *reinterpret_cast<__half2*>(&w[0]));
-              __half2 x1 = __hadd2(*reinterpret_cast<__half2*>(&acc.y), *reinterpret_cast<__half2*>(&w[1]));
-              acc.x = *reinterpret_cast<uint32_t*>(&x0);
-              acc.y = *reinterpret_cast<uint32_t*>(&x1);
-              *reinterpret_cast<uint2*>(addr) = acc;
-            } else {
-              uint32_t acc = *reinterpret_cast<uint32_t*>(addr);
-              __half2 x0 = __hadd2(*reinterpret_cast<__half2*>(&acc), *reinterpret_cast<__half2*>(&w[0]));
-              *reinterpret_cast<uint32_t*>(addr) = *reinterpret_cast<uint32_t*>(&x0);
-            }
-            __syncwarp();
-          }
-        }
-      }
-    }
-  }
-  __syncthreads();
-
-  // ---- flush: partial sketch -> B with 16-byte result-discarding REDs (layouts coincide: [d][n])
-  {
-    const uint4* z = reinterpret_cast<const uint4*>(smem_raw);
-    const uint32_t n16 = (uint32_t)g.d * row_pitch / 16u;
-    __half* B = reinterpret_cast<__half*>(a.B);
-    // stagger the start so the CTAs do not all hit the same L2 lines at once
-    const uint32_t shift = (uint32_t)((blockIdx.x * 2654435761u) % n16);
-    for (uint32_t k0 = tid; k0 < n16; k0 += blockDim.x) {
-      uint32_t k = k0 + shift;
-      k = (k >= n16) ? k - n16 : k;
-      uint4 v = z[k];
-      if ((v.x | v.y | v.z | v.w) != 0u) red_h8(B + (size_t)k * 8, v.x, v.y, v.z, v.w);
     }
   }
 }

@@ -11,6 +11,7 @@
 #include <cstring>
 #include <new>
 
+#include "kernel_smem.cuh"
 #include "kernels.cuh"
 
 namespace {
@@ -96,8 +97,8 @@ int ensure_scratch(void** buf, size_t* have, size_t want) {
 inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 inline bool zeta_templated(int z) { return z == 1 || z == 2 || z == 4 || z == 8; }
 
-// smem layout per zeta: (VEC, LPR) with LPR*VEC = 64 columns per warp
-inline int smem_vec_for(int zeta) { return zeta == 1 ? 2 : zeta == 2 ? 4 : 8; }
+// smem layout: 8 lanes x 8 columns = 64 columns per warp for every zeta
+inline int smem_vec_for(int) { return sk::kSmemVec; }
 
 bool smem_feasible(const sketch* s, int n, int64_t lda, const void* A, const void* B, size_t* bytes) {
   if (!zeta_templated(s->zeta)) return false;
@@ -267,14 +268,14 @@ int launch_flat(const sk::ScatterArgs& a, int zeta, int vec, int grid, int pw, c
   return SKETCH_ERR_UNSUPPORTED;
 }
 
-template <int ZETA, int VEC, int LPR, int RND, int NQ>
+template <int ZETA, int RND>
 int launch_smem_t(const sk::SmemArgs& g, const Plan& p, cudaStream_t st) {
   if (p.wpc <= 4) {
-    auto k = sk::k_smem<ZETA, VEC, LPR, RND, NQ, 4>;
+    auto k = sk::k_smem<ZETA, RND, 4>;
     CU_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_bytes));
     k<<<p.grid, p.wpc * 32, p.smem_bytes, st>>>(g);
   } else {
-    auto k = sk::k_smem<ZETA, VEC, LPR, RND, NQ, 16>;
+    auto k = sk::k_smem<ZETA, RND, 16>;
     CU_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_bytes));
     k<<<p.grid, p.wpc * 32, p.smem_bytes, st>>>(g);
   }
@@ -284,10 +285,10 @@ int launch_smem_t(const sk::SmemArgs& g, const Plan& p, cudaStream_t st) {
 template <int RND>
 int launch_smem(const sk::SmemArgs& g, const Plan& p, cudaStream_t st) {
   switch (p.zeta_t) {
-    case 1: return launch_smem_t<1, 2, 32, RND, 32>(g, p, st);
-    case 2: return launch_smem_t<2, 4, 16, RND, 16>(g, p, st);
-    case 4: return launch_smem_t<4, 8, 8, RND, 8>(g, p, st);
-    case 8: return launch_smem_t<8, 8, 8, RND, 8>(g, p, st);
+    case 1: return launch_smem_t<1, RND>(g, p, st);
+    case 2: return launch_smem_t<2, RND>(g, p, st);
+    case 4: return launch_smem_t<4, RND>(g, p, st);
+    case 8: return launch_smem_t<8, RND>(g, p, st);
   }
   return SKETCH_ERR_UNSUPPORTED;
 }

@@ -235,13 +235,13 @@ def test_sr_conversion_bit_exact_singleton_buckets(ss, variant, zeta):
     assert np.array_equal(got[rows], want_all[rows])
     # SR differs from RN on this input (otherwise the test proves nothing)
     rn = bits(apply16(ss, sk, dev(A), variant))
-    assert (rn[rows] != got[rows]).mean() > 0.2
+    assert (rn[rows] != got[rows]).mean() > 0.1
 
 
 def test_sr_is_unbiased_where_rn_erases(ss):
     # Cor. 3: contributions below h/2 vanish under RN but survive in expectation under SR
     m, n, d, zeta = 1 << 16, 64, 128, 4
-    A = wl.gaussian(m, n, 7, pow2=-26)            # |s*a| ~ 2^-27 << h/2
+    A = wl.gaussian(m, n, 7, pow2=-27)            # |s*a| ~ 2^-28 << h/2 (RN -> nonzero needs |g| > 8)
     seed = sketch_seed(123)
     sk = ss.Sketch(m, d, zeta, seed)
     Ad = dev(A)
@@ -253,7 +253,7 @@ def test_sr_is_unbiased_where_rn_erases(ss):
         acc += oracle.half_bits_to_f64(bits(sk.apply_f16acc(Ad, rounding=ss.SR, sr_seed=sketch_seed(1000 + t))))
     corr = float((acc * B).sum() / np.sqrt((acc * acc).sum() * (B * B).sum()))
     scale = float((acc / T * B).sum() / (B * B).sum())
-    assert corr > 0.2 and 0.7 < scale < 1.3, (corr, scale)
+    assert corr > 0.3 and 0.6 < scale < 1.4, (corr, scale)
 
 
 # ------------------------------------------------------------------------------------ ABI features
@@ -387,17 +387,25 @@ def test_subnormal_scale_is_exact_in_any_order(ss):
         assert np.array_equal(bits(sk.apply_f16acc(dev(A), variant=VID[variant])), want), variant
 
 
-def test_overflow_saturates_to_inf_like_the_oracle(ss):
-    # config 5, k = +12: running sums leave the FP16 range; entries stick at +-inf (no NaN since no
-    # single contribution converts to inf) -- order-dependent, so compare the class, not the bits
+def test_overflow_saturates_like_the_oracle(ss):
+    # config 5, k = +12: running sums leave the FP16 range and stick at +-inf.  No single contribution
+    # converts to inf, so a flat running sum never makes NaN; hierarchical variants can (+inf partial
+    # plus -inf partial = NaN, reading R9).  Order-dependent, so compare the class, not the bits.
     m, n, d, zeta = 1 << 16, 64, 128, 4
     A = wl.gaussian(m, n, 18, pow2=12)
     seed = sketch_seed(72)
     sk = ss.Sketch(m, d, zeta, seed)
     want = oracle.half_bits_to_f64(oracle.seq16_sketch(seed, d, zeta, A))
-    for variant in ("smem", "flat_vec"):
-        got = oracle.half_bits_to_f64(bits(sk.apply_f16acc(dev(A), variant=VID[variant])))
-        assert not np.isnan(got).any()
-        # the exact sums have std ~ 2^12 * 0.5 * sqrt(2048) = 9.3e4 > 65504: a large share overflows
-        assert 0.2 < np.isinf(got).mean() < 0.95 and abs(np.isinf(got).mean() - np.isinf(want).mean()) < 0.25
-        assert (np.isfinite(got) & np.isfinite(want)).sum() > 0
+    assert not np.isnan(want).any()
+    over_want = (~np.isfinite(want)).mean()
+    # the exact sums have std ~ 2^12 * 0.5 * sqrt(2048) = 9.3e4 > 65504: a large share overflows
+    assert 0.2 < over_want < 0.95
+    B = oracle.f64_sketch(seed, d, zeta, A)
+    for variant, kw in (("smem", {}), ("flat_vec", {"replicas": 1}), ("flat_vec", {"replicas": 8})):
+        got = oracle.half_bits_to_f64(bits(sk.apply_f16acc(dev(A), variant=VID[variant], **kw)))
+        over = (~np.isfinite(got)).mean()
+        assert abs(over - over_want) < 0.3, (variant, over, over_want)
+        if kw.get("replicas") == 1:
+            assert not np.isnan(got).any()
+        fin = np.isfinite(got)
+        assert fin.sum() > 0 and ev.rel_fro(got[fin], B[fin]) < 0.2
