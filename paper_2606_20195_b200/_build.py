@@ -1,47 +1,67 @@
 """In-tree build of the CUDA library (nvcc, sm_100a only).  No JIT cache: the .so sits next to the
-sources so it travels to the GPU box with the repository snapshot."""
+sources so it travels to the GPU box with the repository snapshot.  One translation unit per kernel
+family, compiled concurrently, then linked into libsparse_sketch.so."""
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 from pathlib import Path
 
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
+OBJ = HERE / "_obj"
 LIB = HERE / "libsparse_sketch.so"
-SOURCES = [CSRC / "sparse_sketch.cu"]
-DEPS = SOURCES + [CSRC / "kernels.cuh", CSRC / "kernel_smem.cuh", CSRC / "device_util.cuh", HERE.parent / "include" / "sparse_sketch.h"]
+SOURCES = [CSRC / n for n in ("sparse_sketch.cu", "launch_flat_f16.cu", "launch_flat_f32.cu", "launch_smem.cu")]
+HEADERS = [CSRC / n for n in ("args.h", "launch.h", "device_util.cuh", "kernel_flat.cuh", "kernel_misc.cuh", "kernel_smem.cuh")]
+HEADERS.append(HERE.parent / "include" / "sparse_sketch.h")
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",
-    "-shared", "-Xcompiler", "-fPIC",
+    "-Xcompiler", "-fPIC",
     "-Xptxas", "-v",
 ]
 
 
-def is_stale() -> bool:
-    if not LIB.exists():
+def _nvcc() -> str:
+    return os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+
+
+def _stale(target: Path, deps) -> bool:
+    if not target.exists():
         return True
-    t = LIB.stat().st_mtime
-    return any(p.stat().st_mtime > t for p in DEPS)
+    t = target.stat().st_mtime
+    return any(p.stat().st_mtime > t for p in deps)
+
+
+def _compile(src: Path, force: bool) -> Path:
+    obj = OBJ / (src.stem + ".o")
+    if force or _stale(obj, [src] + HEADERS):
+        res = subprocess.run([_nvcc()] + NVCC_FLAGS + ["-c", str(src), "-o", str(obj)], capture_output=True, text=True)
+        (OBJ / (src.stem + ".ptxas.log")).write_text(res.stderr)
+        if res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+            raise RuntimeError("nvcc failed on %s" % src.name)
+    return obj
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:
-    if not force and not is_stale():
+    OBJ.mkdir(exist_ok=True)
+    if not force and not _stale(LIB, SOURCES + HEADERS):
         return LIB
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+        objs = list(ex.map(lambda s: _compile(s, force), SOURCES))
     tmp = LIB.with_suffix(".so.tmp%d" % os.getpid())
-    cmd = [nvcc] + NVCC_FLAGS + ["-o", str(tmp)] + [str(s) for s in SOURCES]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    (HERE / "build_ptxas.log").write_text(res.stderr)
+    res = subprocess.run([_nvcc(), "-shared", "-o", str(tmp)] + [str(o) for o in objs], capture_output=True, text=True)
     if res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)
-        raise RuntimeError("nvcc failed building libsparse_sketch.so")
-    if verbose:
-        sys.stderr.write(res.stderr)
+        raise RuntimeError("link of libsparse_sketch.so failed")
     os.replace(tmp, LIB)
+    if verbose:
+        for s in SOURCES:
+            sys.stderr.write((OBJ / (s.stem + ".ptxas.log")).read_text())
     return LIB
 
 

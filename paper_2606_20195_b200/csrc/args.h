@@ -1,0 +1,35 @@
+// args.h -- plain argument structs passed by value to the scatter kernels (host + device).
+#pragma once
+#include <stdint.h>
+
+namespace sk {
+
+struct ScatterArgs {
+  const float* A;       // first row of the range
+  int64_t lda;          // elements
+  int64_t row_begin;    // global index of A's first row (hash counter base)
+  int64_t rows;         // rows in the range
+  void* B;              // d x n sketch (or base of the replicas)
+  int64_t replica_stride;  // elements between replicas
+  int32_t replicas;
+  int32_t n;
+  int32_t zeta;
+  uint32_t db;          // d / zeta
+  uint64_t seed;
+  uint64_t sr_seed;
+  float scale;          // fp32(1/sqrt(zeta)), correctly rounded on the host (R5)
+  uint32_t cpr;         // chunks of VEC columns per row = n / VEC
+  uint32_t cpr_magic;   // ceil(2^32 / cpr): c / cpr == umulhi(c, magic) for c*cpr < 2^32
+  const void* packed;   // hash_mode 2: packed entries for global rows, index i*zeta + j (ranked u16 or u32); else nullptr
+};
+
+
+struct SmemArgs {
+  ScatterArgs s;
+  int64_t rows_per_cta;  // multiple of 4 (row groups stay aligned in the global row index)
+  int32_t d;
+};
+
+constexpr int kFlatThreads = 256;
+
+}  // namespace sk

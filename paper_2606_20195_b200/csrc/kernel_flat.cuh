@@ -1,75 +1,20 @@
-// kernels.cuh -- the sm_100a kernels of the sparse-sketch hot path.
-//
-//   k_hash_dump / k_hash_pack   a1  hash stage (dump for tests, packed array for hash_mode=2)
-//   k_flat<...>                 a2-a6 streaming scatter with result-discarding global RED
-//                               (the paper's Listings 1/2 restated with shared hashes + vector RED)
-//   k_smem<...>                 (kernel_smem.cuh) a2-a5 shared-memory-privatised FP16 partial sketch per CTA
-//   k_generic<...>              any-n / any-alignment scalar fallback
-//   k_reduce_replicas<...>      sums the P L2-resident partial sketches of the flat variant
-//   k_red_probe<...>            L2 atomic-throughput microbenchmark (roofline term 2)
+// kernel_flat.cuh -- streaming scatter kernels with result-discarding global RED:
+//   k_flat<...>     the paper's Listings 1/2 restated for sm_100a: shared hashes + 8/16-byte vector RED
+//   k_generic<...>  any-n / any-alignment scalar fallback
 #pragma once
 
+#include "args.h"
 #include "device_util.cuh"
 
 namespace sk {
 
-constexpr int kFlatThreads = 256;
-
-// ------------------------------------------------------------------------------------------------
-// a1: hash stage as stand-alone kernels
-// ------------------------------------------------------------------------------------------------
-__global__ void k_hash_dump(uint64_t seed, int64_t total, uint32_t zeta, uint32_t db, int32_t* __restrict__ bucket,
-                            uint8_t* __restrict__ signbit) {
-  int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += stride) {
-    uint32_t j = (uint32_t)(idx % zeta);
-    uint32_t e = hash_entry(seed, (uint64_t)idx, j, db);
-    bucket[idx] = (int32_t)entry_bucket(e);
-    signbit[idx] = (uint8_t)(e >> 31);
-  }
-}
-
-template <typename PackT>
-__global__ void k_hash_pack(uint64_t seed, int64_t total, uint32_t zeta, uint32_t db, PackT* __restrict__ packed) {
-  int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += stride) {
-    uint32_t j = (uint32_t)(idx % zeta);
-    uint32_t e = hash_entry(seed, (uint64_t)idx, j, db);
-    if constexpr (sizeof(PackT) == 2)
-      packed[idx] = (PackT)(entry_bucket(e) | ((e >> 31) << 15));
-    else
-      packed[idx] = (PackT)e;
-  }
-}
-
-// packed entry -> canonical 32-bit entry (bucket | sign<<31)
+// packed entry -> canonical 32-bit entry (bucket | sign<<31).  16-bit entries are the ranked form written by
+// k_hash_pack_ranked (kernel_smem.cuh): bucket in bits 0..10, sign in bit 15 (rank bits ignored here).
 template <typename PackT>
 SK_DEVINL uint32_t unpack_entry(PackT p) {
-  if constexpr (sizeof(PackT) == 2) return ((uint32_t)p & 0x7FFFu) | (((uint32_t)p >> 15) << 31);
+  if constexpr (sizeof(PackT) == 2) return ((uint32_t)p & 0x07FFu) | (((uint32_t)p >> 15) << 31);
   else return (uint32_t)p;
 }
-
-// ------------------------------------------------------------------------------------------------
-// Arguments shared by the scatter kernels
-// ------------------------------------------------------------------------------------------------
-struct ScatterArgs {
-  const float* A;       // first row of the range
-  int64_t lda;          // elements
-  int64_t row_begin;    // global index of A's first row (hash counter base)
-  int64_t rows;         // rows in the range
-  void* B;              // d x n sketch (or base of the replicas)
-  int64_t replica_stride;  // elements between replicas
-  int32_t replicas;
-  int32_t n;
-  int32_t zeta;
-  uint32_t db;          // d / zeta
-  uint64_t seed;
-  uint64_t sr_seed;
-  float scale;          // fp32(1/sqrt(zeta)), correctly rounded on the host (R5)
-  uint32_t cpr;         // chunks of VEC columns per row = n / VEC
-  uint32_t cpr_magic;   // ceil(2^32 / cpr): c / cpr == umulhi(c, magic) for c*cpr < 2^32
-  const void* packed;   // hash_mode 2: packed entries for global rows, index i*zeta + j; else nullptr
-};
 
 // ------------------------------------------------------------------------------------------------
 // Flat scatter: every contribution is one result-discarding RED into an L2-resident sketch.
@@ -212,62 +157,6 @@ __global__ void __launch_bounds__(kFlatThreads) k_generic(ScatterArgs a) {
         red_f1(reinterpret_cast<float*>(Bbase) + off, ps);
       }
     }
-  }
-}
-
-// ------------------------------------------------------------------------------------------------
-// Fold P partial sketches.  FP16: sequential RN16 adds in replica order (every accumulation of the
-// FP16 path stays an FP16 RN add, "All policies subsequently use RN atomic addition");
-// FP32: float adds.  accumulate != 0 adds the fold into the existing out.
-// ------------------------------------------------------------------------------------------------
-template <bool F16>
-__global__ void k_reduce_replicas(const void* __restrict__ rep, int64_t replica_stride, int32_t replicas, void* __restrict__ out,
-                                  int64_t count, int accumulate) {
-  int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < count; k += stride) {
-    if constexpr (F16) {
-      const __half* r = reinterpret_cast<const __half*>(rep);
-      __half* o = reinterpret_cast<__half*>(out);
-      __half acc = accumulate ? o[k] : __ushort_as_half(0);
-      for (int p = 0; p < replicas; ++p) acc = __hadd(acc, r[(int64_t)p * replica_stride + k]);
-      o[k] = acc;
-    } else {
-      const float* r = reinterpret_cast<const float*>(rep);
-      float* o = reinterpret_cast<float*>(out);
-      float acc = accumulate ? o[k] : 0.f;
-      for (int p = 0; p < replicas; ++p) acc = __fadd_rn(acc, r[(int64_t)p * replica_stride + k]);
-      o[k] = acc;
-    }
-  }
-}
-
-// ------------------------------------------------------------------------------------------------
-// L2 atomic-throughput probe: same address pattern as k_flat (a random bucket row per lane group of
-// n/VEC lanes, consecutive lanes on consecutive VEC-column chunks), values from registers, no A loads.
-// ------------------------------------------------------------------------------------------------
-template <int KIND>
-__global__ void __launch_bounds__(kFlatThreads) k_red_probe(void* sketch, int32_t d, int32_t n, int32_t replicas, int32_t iters) {
-  constexpr bool F16 = KIND < 3;
-  constexpr int VEC = (KIND == 0) ? 2 : (KIND == 1) ? 4 : (KIND == 2) ? 8 : (KIND == 3) ? 1 : (KIND == 4) ? 2 : 4;
-  const uint32_t cpr = (uint32_t)n / VEC;
-  const uint64_t gtid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const uint64_t gthreads = (uint64_t)gridDim.x * blockDim.x;
-  char* base = reinterpret_cast<char*>(sketch) + (size_t)(blockIdx.x % replicas) * (size_t)d * n * (F16 ? 2 : 4);
-  const uint32_t ch = (uint32_t)(gtid % cpr);
-  const uint64_t grp = gtid / cpr;
-  const uint64_t ngrp = (gthreads + cpr - 1) / cpr;
-  for (int32_t it = 0; it < iters; ++it) {
-    uint64_t h = splitmix64(grp + (uint64_t)it * ngrp);
-    uint32_t bucket = __umulhi((uint32_t)(h >> 32), (uint32_t)d);
-    size_t off = (size_t)bucket * n + (size_t)ch * VEC;
-    uint32_t hv = (h & 1) ? 0x3C003C00u : 0xBC00BC00u;  // +-1.0 pairs: sums stay small
-    float fv = (h & 1) ? 1.f : -1.f;
-    if constexpr (KIND == 0) red_h2(reinterpret_cast<__half*>(base) + off, hv);
-    else if constexpr (KIND == 1) red_h4(reinterpret_cast<__half*>(base) + off, hv, hv);
-    else if constexpr (KIND == 2) red_h8(reinterpret_cast<__half*>(base) + off, hv, hv, hv, hv);
-    else if constexpr (KIND == 3) red_f1(reinterpret_cast<float*>(base) + off, fv);
-    else if constexpr (KIND == 4) red_f2(reinterpret_cast<float*>(base) + off, fv, fv);
-    else red_f4(reinterpret_cast<float*>(base) + off, fv, fv, fv, fv);
   }
 }
 

@@ -1,45 +1,98 @@
-// kernel_smem.cuh -- shared-memory-privatised FP16 scatter for sm_100a.
+// kernel_smem.cuh -- shared-memory-privatised FP16-RN scatter for sm_100a.
 //
 // Each CTA keeps one private d x n FP16 partial sketch in shared memory and streams a contiguous range
 // of rows; at the end it flushes the partial sketch into B with 16-byte result-discarding REDs.
 // sm_100a has no native shared-memory FP16 add (atomicAdd on shared assembles to a CAS loop), so every
 // sketch word has exactly one owner at any time and is updated with plain LDS.128 / HFMA2 / STS.128:
 //   - warp w of the CTA owns the 64-column slice [64w, 64w+64): no two warps touch the same word;
-//   - inside a warp the lanes are R = 4 rows x 8 column chunks of 8 columns.  One "row group" (4 rows)
-//     is scattered per step: for every stack block j the 4 rows read-modify-write their 4 buckets of
-//     block j at once.  Two rows of a group collide in block j with probability ~6/(d/zeta); the hash
-//     stage ranks such rows (rank = number of earlier rows of the group with the same bucket in that
-//     block), and a group with any non-zero rank takes a slow path that applies the ranks one after
-//     the other.  In the common path the ZETA read-modify-writes of a group are independent, so the
-//     ZETA LDS.128 are in flight together (blocks are disjoint row ranges of the sketch).
+//   - inside a warp the lanes are R = 4 rows x 8 column chunks of 8 columns.  One "row group" (4
+//     consecutive rows, aligned to 4 in the global row index) is scattered per step: for every stack
+//     block j the 4 rows read-modify-write their 4 buckets of block j at once.  Two rows of a group
+//     collide in block j with probability ~6/(d/zeta); the hash stage ranks such rows (rank = number
+//     of earlier rows of the group with the same bucket in that block) and a group with a non-zero
+//     rank takes a slow path that applies rank 0, then rank 1, ...  In the common path the ZETA
+//     read-modify-writes of a group are independent (blocks are disjoint row ranges of the sketch,
+//     PAPER.md:59-63), so the ZETA LDS.128 are in flight together.
 // The product s*a is rounded to FP16 once per element; the block sign enters as the +-1 multiplier of
 // HFMA2 (q * (+-1) + acc: the product is exact, one rounding = RN16(acc +- q)).
-// A goes straight from HBM into registers with 256-bit streaming loads through an 8-deep register
-// ring (8 row groups = 8 KiB in flight per warp): staging A through shared memory would add 8 B/float
-// to a shared-memory pipe that the 2*2*ZETA B/float of read-modify-write traffic already loads.
+// A goes straight from HBM into registers with 256-bit streaming loads through an NQ-deep register
+// ring (NQ row groups = NQ KiB in flight per warp): staging A through shared memory would add
+// 8 B/float to a shared-memory pipe that the 2*2*ZETA B/float of read-modify-write traffic already
+// loads, and the register file is otherwise idle (2-6 warps per SM).
+// Hash stage (a1) in its precomputed form: k_hash_pack_ranked writes one 16-bit entry per (row, block)
+//   bucket | rank<<11 | group_max_rank<<13 | sign<<15
+// and every lane loads its row's ZETA entries (2*ZETA bytes, +ZETA/(2n) of A's traffic) through the
+// same register ring.  (The on-the-fly form of this kernel cost ~25 of 135 instructions per row group,
+// profiles/r01_smem_hash_on_the_fly.md; the flat kernels keep both forms.)
 #pragma once
 
-#include "kernels.cuh"
+#include <type_traits>
+
+#include "args.h"
+#include "device_util.cuh"
 
 namespace sk {
 
-struct SmemArgs {
-  ScatterArgs s;
-  int64_t rows_per_cta;  // multiple of kSmemRingRows
-  int32_t d;
-};
-
-constexpr int kSmemVec = 8;                 // columns per lane
-constexpr int kSmemLpr = 8;                 // lanes per row
-constexpr int kSmemR = 4;                   // rows per group
-constexpr int kSmemNq = 8;                  // ring depth in row groups
-constexpr int kSmemRingRows = kSmemNq * kSmemR;  // 32
+constexpr int kSmemVec = 8;                            // columns per lane
+constexpr int kSmemLpr = 8;                            // lanes per row
+constexpr int kSmemR = 4;                              // rows per group
 constexpr int kSmemColsPerWarp = kSmemVec * kSmemLpr;  // 64
-constexpr uint32_t kRankShift = 28;         // entry bits 28..30: rank inside the row group
-constexpr uint32_t kRankMask = 7u << kRankShift;
-constexpr uint32_t kBucketMask = (1u << kRankShift) - 1u;
+constexpr int kSmemMaxBucket = 2048;                   // 11-bit bucket field of the ranked 16-bit entry
+constexpr int kSmemPadRows = 128;                      // rows the packed array extends beyond m (ring look-ahead)
 
-// acc (4 half2 words) += sign * q
+// ranked 16-bit entry
+constexpr uint32_t kE16Bucket = 0x07FFu;
+constexpr uint32_t kE16RankShift = 11;  // 2 bits
+constexpr uint32_t kE16GmaxShift = 13;  // 2 bits: largest rank in the row group (same in all its entries)
+
+// ring depth (row groups in flight per warp) per instantiation; the host sizes rows_per_cta from it
+constexpr int smem_ring_depth(int zeta, bool small_cta) { return small_cta ? (zeta == 8 ? 8 : 12) : 4; }
+
+// ------------------------------------------------------------------------------------------------
+// a1 (precomputed form): ranked entries for every (row, block), rows padded beyond m.
+// One warp hashes 32/ZETA rows; ranks come from shuffles inside the aligned 4-row group.
+// ------------------------------------------------------------------------------------------------
+template <int ZETA>
+__global__ void k_hash_pack_ranked(uint64_t seed, int64_t rows_padded, uint32_t db, uint16_t* __restrict__ packed) {
+  constexpr int HB = 32 / ZETA;
+  constexpr int GL = kSmemR * ZETA;  // lanes per row group
+  static_assert(GL <= 32, "ZETA <= 8");
+  const uint32_t lane = threadIdx.x & 31;
+  const int64_t warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  const int64_t batches = rows_padded / HB;
+  for (int64_t b = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; b < batches; b += warps) {
+    const uint64_t ctr = (uint64_t)b * 32 + lane;  // (row)*ZETA + j with row = b*HB + lane/ZETA
+    const uint32_t e = hash_entry(seed, ctr, lane % ZETA, db);
+    const uint32_t bucket = entry_bucket(e);
+    const uint32_t row_in_group = (lane / ZETA) % kSmemR;
+    uint32_t rank = 0;
+#pragma unroll
+    for (int k = 1; k < kSmemR; ++k) {
+      const uint32_t other = __shfl_up_sync(0xFFFFFFFFu, bucket, k * ZETA);
+      rank += (row_in_group >= (uint32_t)k && other == bucket) ? 1u : 0u;
+    }
+    uint32_t gmax = rank;
+#pragma unroll
+    for (int off = 1; off < GL; off <<= 1) gmax = max(gmax, __shfl_xor_sync(0xFFFFFFFFu, gmax, off));
+    packed[ctr] = (uint16_t)(bucket | (rank << kE16RankShift) | (gmax << kE16GmaxShift) | ((e >> 31) << 15));
+  }
+}
+
+template <int ZETA> struct EntRow;  // a row's ZETA 16-bit entries as one load
+template <> struct EntRow<1> { using type = uint16_t; };
+template <> struct EntRow<2> { using type = uint32_t; };
+template <> struct EntRow<4> { using type = uint2; };
+template <> struct EntRow<8> { using type = uint4; };
+
+template <int ZETA>
+SK_DEVINL uint32_t entrow_word(const typename EntRow<ZETA>::type& e, int w) {
+  if constexpr (ZETA == 1) return (uint32_t)e;
+  else if constexpr (ZETA == 2) return e;
+  else if constexpr (ZETA == 4) return w == 0 ? e.x : e.y;
+  else return w == 0 ? e.x : w == 1 ? e.y : w == 2 ? e.z : e.w;
+}
+
+// acc (4 half2 words) += mult * q  (mult = +-1 in both halves)
 SK_DEVINL void rmw_add(uint4& acc, const uint32_t (&q)[4], uint32_t mult) {
   const __half2 m = *reinterpret_cast<const __half2*>(&mult);
   __half2 x0 = __hfma2(*reinterpret_cast<const __half2*>(&q[0]), m, *reinterpret_cast<__half2*>(&acc.x));
@@ -52,15 +105,14 @@ SK_DEVINL void rmw_add(uint4& acc, const uint32_t (&q)[4], uint32_t mult) {
   acc.w = *reinterpret_cast<uint32_t*>(&x3);
 }
 
-template <int ZETA, int ROUNDING, int MAXW>
+template <int ZETA, int NQ, int MAXW>
 __global__ void __launch_bounds__(MAXW * 32) k_smem(SmemArgs g) {
-  constexpr int VEC = kSmemVec, LPR = kSmemLpr, R = kSmemR, NQ = kSmemNq;
-  static_assert(32 % ZETA == 0, "ZETA must divide 32");
-  constexpr int HB = 32 / ZETA;                 // rows per hash batch (lane l -> row l/ZETA, block l%ZETA)
-  constexpr int GPB = (HB >= R) ? HB / R : 1;   // row groups per hash batch
-  constexpr int BPG = (HB >= R) ? 1 : R / HB;   // hash batches per row group (ZETA = 16, 32)
-  static_assert(BPG == 1, "ZETA <= 8 supported");
-  constexpr int JC = ZETA < 4 ? ZETA : 4;       // blocks handled together (bounds the accumulator registers)
+  constexpr int VEC = kSmemVec, LPR = kSmemLpr, R = kSmemR;
+  static_assert(ZETA == 1 || ZETA == 2 || ZETA == 4 || ZETA == 8, "ZETA in {1,2,4,8}");
+  static_assert(2 * NQ * R <= kSmemPadRows, "packed-array padding covers the look-ahead");
+  constexpr int RING_ROWS = NQ * R;
+  constexpr int JC = ZETA < 4 ? ZETA : 4;  // blocks handled together (bounds the accumulator registers)
+  using ent_t = typename EntRow<ZETA>::type;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const ScatterArgs& a = g.s;
   const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -79,18 +131,20 @@ __global__ void __launch_bounds__(MAXW * 32) k_smem(SmemArgs g) {
   const int64_t cta_r1 = min(a.rows, cta_r0 + g.rows_per_cta);
   const uint32_t col0 = warp * kSmemColsPerWarp + pcol * VEC;  // first column of this lane
   unsigned char* const my_col = smem_raw + col0 * 2u;
-  const uint32_t npairs = ((uint32_t)a.n + 1u) >> 1;
 
   if (cta_r0 < cta_r1) {
     const int64_t nrows = cta_r1 - cta_r0;
-    const int64_t iters = (nrows + kSmemRingRows - 1) / kSmemRingRows;
-    const int64_t full_iters = nrows / kSmemRingRows;  // iterations whose 32 rows all exist
-    // lane's load pointer for (iteration 0, group 0); a group is R rows further, an iteration 32 rows
+    const int64_t iters = (nrows + RING_ROWS - 1) / RING_ROWS;
+    const int64_t full_iters = nrows / RING_ROWS;  // iterations whose RING_ROWS rows all exist
+    // this lane's pointers for the current iteration's group 0; group q is q groups further
     const float* ld_ptr = a.A + (cta_r0 + r) * a.lda + col0;
     const int64_t group_stride = (int64_t)R * a.lda;
+    const int64_t iter_stride = (int64_t)NQ * group_stride;
+    const ent_t* ent_ptr = reinterpret_cast<const ent_t*>(a.packed) + (a.row_begin + cta_r0 + r);
 
     float buf[NQ][VEC];
-    // prologue: iteration 0's groups
+    ent_t ent[NQ];
+    // prologue: iteration 0's groups (row-checked; the packed array is padded, its loads need no check)
 #pragma unroll
     for (int q = 0; q < NQ; ++q) {
       if ((int64_t)q * R + r < nrows) ld_stream<VEC>(ld_ptr + q * group_stride, buf[q]);
@@ -98,118 +152,84 @@ __global__ void __launch_bounds__(MAXW * 32) k_smem(SmemArgs g) {
 #pragma unroll
         for (int k = 0; k < VEC; ++k) buf[q][k] = 0.f;
       }
+      ent[q] = __ldg(ent_ptr + q * R);
     }
 
-    for (int64_t it = 0; it < iters; ++it) {
-      const int64_t it_row0 = cta_r0 + it * kSmemRingRows;  // local row of this iteration's first row
-      // how the next iteration's loads must be issued: 0 = none, 1 = unchecked, 2 = row-checked
-      const int next_mode = (it + 1 < full_iters) ? 1 : (it + 1 < iters) ? 2 : 0;
-      const float* next_ptr = ld_ptr + (it + 1) * (int64_t)NQ * group_stride;
-      const int64_t next_rows_left = nrows - (it + 1) * kSmemRingRows;  // rows that exist in the next iteration
-
+    // one ring iteration; NEXT: 0 = no further loads, 1 = next iteration is complete (unchecked loads),
+    // 2 = next iteration is the ragged tail (row-checked loads; rows past the range read as zeros, which
+    // add +-0 to valid buckets)
+    auto ring_iteration = [&](int64_t it, auto next_tag) {
+      constexpr int NEXT = decltype(next_tag)::value;
+      const float* next_ptr = ld_ptr + iter_stride;
+      const int64_t next_rows_left = nrows - (it + 1) * RING_ROWS;
 #pragma unroll
-      for (int hb = 0; hb < NQ / GPB; ++hb) {
-        // ---- hash stage for HB rows: lane l -> (row l/ZETA, block l%ZETA), plus the rank inside its group
-        uint32_t e;
-        {
-          const int64_t b0 = it_row0 + (int64_t)hb * HB;
-          const uint64_t ctr = (uint64_t)(a.row_begin + b0) * ZETA + lane;
-          e = hash_entry(a.seed, ctr, lane % ZETA, a.db);
-          const uint32_t bucket = entry_bucket(e);
-          const uint32_t row_in_group = (lane / ZETA) % R;
-          uint32_t rank = 0;
+      for (int q = 0; q < NQ; ++q) {
+        float p[VEC];
 #pragma unroll
-          for (int k = 1; k < R; ++k) {
-            const uint32_t other = __shfl_up_sync(0xFFFFFFFFu, bucket, k * ZETA);
-            rank += (row_in_group >= (uint32_t)k && other == bucket) ? 1u : 0u;
+        for (int k = 0; k < VEC; ++k) p[k] = buf[q][k] * a.scale;
+        const ent_t my_ent = ent[q];
+        // refill this ring slot with the same group of the next iteration
+        if constexpr (NEXT == 1) {
+          ld_stream<VEC>(next_ptr + q * group_stride, buf[q]);
+        } else if constexpr (NEXT == 2) {
+          if ((int64_t)q * R + r < next_rows_left) ld_stream<VEC>(next_ptr + q * group_stride, buf[q]);
+          else {
+#pragma unroll
+            for (int k = 0; k < VEC; ++k) buf[q][k] = 0.f;
           }
-          e |= rank << kRankShift;
         }
+        if constexpr (NEXT != 0) ent[q] = __ldg(ent_ptr + RING_ROWS + q * R);
+
+        uint32_t qv[VEC / 2];
 #pragma unroll
-        for (int gq = 0; gq < GPB; ++gq) {
-          const int q = hb * GPB + gq;
-          float p[VEC];
+        for (int k = 0; k < VEC / 2; ++k) qv[k] = pack_rn(p[2 * k], p[2 * k + 1]);
 #pragma unroll
-          for (int k = 0; k < VEC; ++k) p[k] = buf[q][k] * a.scale;
-          // refill this ring slot with the same group of the next iteration
-          if (next_mode == 1) {
-            ld_stream<VEC>(next_ptr + q * group_stride, buf[q]);
-          } else if (next_mode == 2) {
-            if ((int64_t)q * R + r < next_rows_left) ld_stream<VEC>(next_ptr + q * group_stride, buf[q]);
-            else {
+        for (int jc = 0; jc < ZETA; jc += JC) {
+          unsigned char* addr[JC];
+          uint32_t mult[JC], e16[JC];
 #pragma unroll
-              for (int k = 0; k < VEC; ++k) buf[q][k] = 0.f;
-            }
+          for (int j = 0; j < JC; ++j) {
+            const uint32_t w = entrow_word<ZETA>(my_ent, (jc + j) >> 1);
+            e16[j] = ((jc + j) & 1) ? (w >> 16) : (w & 0xFFFFu);
+            addr[j] = my_col + (e16[j] & kE16Bucket) * row_pitch;
+            // sign bit of the entry replicated into both halves, XOR +1.0: +-1.0 in both halves
+            mult[j] = (__byte_perm(w, 0, ((jc + j) & 1) ? 0x3232 : 0x1010) & 0x80008000u) ^ 0x3C003C00u;
           }
-          uint32_t qv[VEC / 2];
-          if constexpr (ROUNDING == 0) {
+          const uint32_t gmax = (e16[0] >> kE16GmaxShift) & 3u;  // warp-uniform: the warp is one row group
+          if (gmax == 0u) {
+            // common path: the JC read-modify-writes are independent -> all loads first
+            uint4 acc[JC];
 #pragma unroll
-            for (int k = 0; k < VEC / 2; ++k) qv[k] = pack_rn(p[2 * k], p[2 * k + 1]);
-          }
-          const uint32_t rib = (uint32_t)gq * R + r;  // row in hash batch
+            for (int j = 0; j < JC; ++j) acc[j] = *reinterpret_cast<uint4*>(addr[j]);
 #pragma unroll
-          for (int jc = 0; jc < ZETA; jc += JC) {
-            uint32_t ej[JC];
-            unsigned char* addr[JC];
-            uint32_t mult[JC];
-            uint32_t anyrank = 0;
+            for (int j = 0; j < JC; ++j) rmw_add(acc[j], qv, mult[j]);
 #pragma unroll
-            for (int j = 0; j < JC; ++j) {
-              ej[j] = __shfl_sync(0xFFFFFFFFu, e, rib * ZETA + jc + j);
-              addr[j] = my_col + (ej[j] & kBucketMask) * row_pitch;
-              mult[j] = (entry_signmask_h2(ej[j])) ^ 0x3C003C00u;  // +-1.0 in both halves
-              anyrank |= ej[j];
-            }
-            uint32_t w[JC][VEC / 2];
+            for (int j = 0; j < JC; ++j) *reinterpret_cast<uint4*>(addr[j]) = acc[j];
+          } else {
+            // some rows of the group share a bucket: apply rank 0, then rank 1, ...
+            for (uint32_t k = 0; k <= gmax; ++k) {
 #pragma unroll
-            for (int j = 0; j < JC; ++j) {
-              if constexpr (ROUNDING == 0) {
-#pragma unroll
-                for (int k = 0; k < VEC / 2; ++k) w[j][k] = qv[k];
-              } else {
-                // SR converts every contribution separately (the draw depends on (row, block, pair))
-                const uint32_t sf = entry_signmask_f32(ej[j]);
-                const int64_t grow = a.row_begin + it_row0 + (int64_t)hb * HB + rib;
-                const uint64_t sr_ctr = ((uint64_t)grow * ZETA + (jc + j)) * npairs + (uint64_t)(col0 >> 1);
-#pragma unroll
-                for (int k = 0; k < VEC / 2; ++k)
-                  w[j][k] = pack_sr(__uint_as_float(__float_as_uint(p[2 * k]) ^ sf),
-                                    __uint_as_float(__float_as_uint(p[2 * k + 1]) ^ sf), a.sr_seed, sr_ctr + k);
-                mult[j] = 0x3C003C00u;  // sign already applied before the conversion
-              }
-            }
-            if (!__any_sync(0xFFFFFFFFu, (anyrank & kRankMask) != 0u)) {
-              // common path: the JC read-modify-writes are independent -> all loads first
-              uint4 acc[JC];
-#pragma unroll
-              for (int j = 0; j < JC; ++j) acc[j] = *reinterpret_cast<uint4*>(addr[j]);
-#pragma unroll
-              for (int j = 0; j < JC; ++j) rmw_add(acc[j], w[j], mult[j]);
-#pragma unroll
-              for (int j = 0; j < JC; ++j) *reinterpret_cast<uint4*>(addr[j]) = acc[j];
-            } else {
-              // some rows of the group share a bucket: apply rank 0, then rank 1, ...
-              for (uint32_t k = 0; k < (uint32_t)R; ++k) {
-                bool more = false;
-#pragma unroll
-                for (int j = 0; j < JC; ++j) {
-                  const uint32_t rk = (ej[j] & kRankMask) >> kRankShift;
-                  if (rk == k) {
-                    uint4 acc = *reinterpret_cast<uint4*>(addr[j]);
-                    rmw_add(acc, w[j], mult[j]);
-                    *reinterpret_cast<uint4*>(addr[j]) = acc;
-                  }
-                  more |= rk > k;
+              for (int j = 0; j < JC; ++j) {
+                if (((e16[j] >> kE16RankShift) & 3u) == k) {
+                  uint4 acc = *reinterpret_cast<uint4*>(addr[j]);
+                  rmw_add(acc, qv, mult[j]);
+                  *reinterpret_cast<uint4*>(addr[j]) = acc;
                 }
-                __syncwarp();
-                if (!__any_sync(0xFFFFFFFFu, more)) break;
               }
+              __syncwarp();
             }
-            __syncwarp();
           }
+          __syncwarp();
         }
       }
-    }
+      ld_ptr += iter_stride;
+      ent_ptr += RING_ROWS;
+    };
+
+    int64_t it = 0;
+    for (; it + 1 < full_iters; ++it) ring_iteration(it, std::integral_constant<int, 1>{});
+    for (; it + 1 < iters; ++it) ring_iteration(it, std::integral_constant<int, 2>{});
+    ring_iteration(it, std::integral_constant<int, 0>{});
   }
   __syncthreads();
 

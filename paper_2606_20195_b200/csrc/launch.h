@@ -1,0 +1,24 @@
+// launch.h -- host-side launchers, one translation unit per kernel family so nvcc compiles them in parallel.
+// Each returns the launch status (cudaGetLastError) or cudaErrorInvalidValue for an unsupported combination.
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include "args.h"
+
+namespace sk {
+
+cudaError_t launch_flat_f16(const ScatterArgs& a, int zeta, int vec, int rounding, int packed_width, int grid,
+                            cudaStream_t st);
+cudaError_t launch_flat_f32(const ScatterArgs& a, int zeta, int vec, int packed_width, int grid, cudaStream_t st);
+cudaError_t launch_generic(const ScatterArgs& a, bool f16, int rounding, int grid, cudaStream_t st);
+
+// shared-memory-privatised FP16-RN scatter; wpc = warps per CTA = n / 64
+cudaError_t launch_smem_f16(const SmemArgs& g, int zeta, int wpc, int grid, size_t smem_bytes, cudaStream_t st);
+int smem_ring_rows(int zeta, int wpc);  // rows one ring iteration of that instantiation covers
+cudaError_t launch_hash_pack_ranked(uint64_t seed, int zeta, int64_t rows_padded, uint32_t db, uint16_t* out, int grid,
+                                    cudaStream_t st);
+int smem_pad_rows();
+int smem_max_bucket();
+
+}  // namespace sk

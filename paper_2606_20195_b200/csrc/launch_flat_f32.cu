@@ -1,0 +1,45 @@
+// launch_flat_f32.cu -- instantiations of the flat FP32 scatter (the in-library baseline) and the generic fallback.
+#include "kernel_flat.cuh"
+#include "launch.h"
+
+namespace sk {
+namespace {
+
+template <int ZETA, int VEC>
+cudaError_t go(const ScatterArgs& a, int pw, int grid, cudaStream_t st) {
+  if (pw == 2) k_flat<ZETA, VEC, false, 0, uint16_t><<<grid, kFlatThreads, 0, st>>>(a);
+  else if (pw == 4) k_flat<ZETA, VEC, false, 0, uint32_t><<<grid, kFlatThreads, 0, st>>>(a);
+  else k_flat<ZETA, VEC, false, 0, uint8_t><<<grid, kFlatThreads, 0, st>>>(a);
+  return cudaGetLastError();
+}
+
+template <int ZETA>
+cudaError_t by_vec(const ScatterArgs& a, int vec, int pw, int grid, cudaStream_t st) {
+  switch (vec) {
+    case 4: return go<ZETA, 4>(a, pw, grid, st);
+    case 2: return go<ZETA, 2>(a, pw, grid, st);
+    case 1: return go<ZETA, 1>(a, pw, grid, st);
+  }
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace
+
+cudaError_t launch_flat_f32(const ScatterArgs& a, int zeta, int vec, int packed_width, int grid, cudaStream_t st) {
+  switch (zeta) {
+    case 1: return by_vec<1>(a, vec, packed_width, grid, st);
+    case 2: return by_vec<2>(a, vec, packed_width, grid, st);
+    case 4: return by_vec<4>(a, vec, packed_width, grid, st);
+    case 8: return by_vec<8>(a, vec, packed_width, grid, st);
+  }
+  return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_generic(const ScatterArgs& a, bool f16, int rounding, int grid, cudaStream_t st) {
+  if (!f16) k_generic<false, 0><<<grid, kFlatThreads, 0, st>>>(a);
+  else if (rounding) k_generic<true, 1><<<grid, kFlatThreads, 0, st>>>(a);
+  else k_generic<true, 0><<<grid, kFlatThreads, 0, st>>>(a);
+  return cudaGetLastError();
+}
+
+}  // namespace sk

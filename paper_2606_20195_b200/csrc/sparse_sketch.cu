@@ -1,5 +1,5 @@
 // sparse_sketch.cu -- C ABI (include/sparse_sketch.h), handle, variant selection and launches.
-// Host logic only; every step of the hot path runs in the kernels of kernels.cuh.
+// Host logic only; every step of the hot path runs in the kernels of kernel_*.cuh (launched via launch.h).
 #include "../../include/sparse_sketch.h"
 
 #include <cuda_runtime.h>
@@ -11,8 +11,8 @@
 #include <cstring>
 #include <new>
 
-#include "kernel_smem.cuh"
-#include "kernels.cuh"
+#include "kernel_misc.cuh"
+#include "launch.h"
 
 namespace {
 
@@ -50,7 +50,7 @@ struct sketch {
   int smem_per_sm;
   // library-owned scratch
   void* rep;  size_t rep_bytes;        // replicated partial sketches
-  void* packed; int packed_width;      // 0 = none, 2 / 4 bytes per entry
+  void* packed; size_t packed_bytes; int packed_width;  // 0 = none, 2 = ranked 16-bit entries, 4 = plain 32-bit
   void* stage[2]; size_t stage_bytes;  // host-path staging
   void* bdev; size_t bdev_bytes;
   cudaStream_t st_copy, st_comp;
@@ -96,9 +96,10 @@ int ensure_scratch(void** buf, size_t* have, size_t want) {
 
 inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 inline bool zeta_templated(int z) { return z == 1 || z == 2 || z == 4 || z == 8; }
+inline bool ranked_ok(const sketch* s) { return zeta_templated(s->zeta) && s->d <= sk::smem_max_bucket(); }
 
 // smem layout: 8 lanes x 8 columns = 64 columns per warp for every zeta
-inline int smem_vec_for(int) { return sk::kSmemVec; }
+inline int smem_vec_for(int) { return 8; }
 
 bool smem_feasible(const sketch* s, int n, int64_t lda, const void* A, const void* B, size_t* bytes) {
   if (!zeta_templated(s->zeta)) return false;
@@ -136,7 +137,10 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
   p->hash_mode = (o && o->hash_mode) ? o->hash_mode : 1;
   if (p->hash_mode != 1 && p->hash_mode != 2) return SKETCH_ERR_INVALID;
   size_t sm_bytes = 0;
-  bool sm_ok = f16 && smem_feasible(s, n, lda, A, B, &sm_bytes);
+  // the privatised kernel is FP16-RN with precomputed ranked hashes; its 4-row groups must be aligned in the
+  // global row index.  Everything else (FP32, SR, odd shapes) runs the flat / generic kernels.
+  const int64_t rb0 = o ? o->row_begin : 0;
+  bool sm_ok = f16 && rounding == SKETCH_RN && ranked_ok(s) && (rb0 % 4 == 0) && smem_feasible(s, n, lda, A, B, &sm_bytes);
   int vmax = flat_vec_for(f16, n, lda, A, B, 8);
   int vpair = flat_vec_for(f16, n, lda, A, B, f16 ? 2 : 1);
   bool zt = zeta_templated(s->zeta);
@@ -154,7 +158,7 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
   p->zeta_t = s->zeta;
 
   if (v == SKETCH_VARIANT_SMEM) {
-    p->hash_mode = 1;
+    p->hash_mode = 2;  // always the precomputed ranked entries
     p->vec = smem_vec_for(s->zeta);
     p->wpc = n / 64;
     p->smem_bytes = sm_bytes;
@@ -166,7 +170,7 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
     if (per_sm > 32) per_sm = 32;
     int64_t grid = (int64_t)s->sm_count * per_sm;
     if (o && o->grid_ctas > 0) grid = o->grid_ctas;
-    const int64_t ring = 32;  // NQ*R rows for every layout
+    const int64_t ring = sk::smem_ring_rows(s->zeta, p->wpc);  // rows per ring iteration of that instantiation
     int64_t rpc = (rows + grid - 1) / grid;
     rpc = (rpc + ring - 1) / ring * ring;
     if (rpc < ring) rpc = ring;
@@ -231,86 +235,39 @@ sk::ScatterArgs make_args(const sketch* s, const float* A, int n, int64_t lda, v
   return a;
 }
 
-template <int ZETA, int VEC, bool F16, int RND>
-int launch_flat_t(const sk::ScatterArgs& a, int grid, int packed_width, cudaStream_t st) {
-  if (packed_width == 2) sk::k_flat<ZETA, VEC, F16, RND, uint16_t><<<grid, sk::kFlatThreads, 0, st>>>(a);
-  else if (packed_width == 4) sk::k_flat<ZETA, VEC, F16, RND, uint32_t><<<grid, sk::kFlatThreads, 0, st>>>(a);
-  else sk::k_flat<ZETA, VEC, F16, RND, uint8_t><<<grid, sk::kFlatThreads, 0, st>>>(a);
-  return launch_check("k_flat");
+int launched(cudaError_t e, const char* what) {
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  if (e == cudaErrorInvalidValue) return SKETCH_ERR_UNSUPPORTED;
+  return e == cudaSuccess ? SKETCH_OK : cuda_fail(e, what);
 }
 
-template <int ZETA, bool F16, int RND>
-int launch_flat_v(const sk::ScatterArgs& a, int vec, int grid, int pw, cudaStream_t st) {
-  if constexpr (F16) {
-    switch (vec) {
-      case 8: return launch_flat_t<ZETA, 8, true, RND>(a, grid, pw, st);
-      case 4: return launch_flat_t<ZETA, 4, true, RND>(a, grid, pw, st);
-      case 2: return launch_flat_t<ZETA, 2, true, RND>(a, grid, pw, st);
-    }
-  } else {
-    switch (vec) {
-      case 4: return launch_flat_t<ZETA, 4, false, 0>(a, grid, pw, st);
-      case 2: return launch_flat_t<ZETA, 2, false, 0>(a, grid, pw, st);
-      case 1: return launch_flat_t<ZETA, 1, false, 0>(a, grid, pw, st);
-    }
-  }
-  return SKETCH_ERR_UNSUPPORTED;
-}
+// a1 in its precomputed form.  Ranked 16-bit entries (bucket | rank<<11 | group_max_rank<<13 | sign<<15, rows
+// padded to 64 beyond m) when the sketch fits them, else plain 32-bit entries.  force: re-run the pack kernel.
 
-template <bool F16, int RND>
-int launch_flat(const sk::ScatterArgs& a, int zeta, int vec, int grid, int pw, cudaStream_t st) {
-  switch (zeta) {
-    case 1: return launch_flat_v<1, F16, RND>(a, vec, grid, pw, st);
-    case 2: return launch_flat_v<2, F16, RND>(a, vec, grid, pw, st);
-    case 4: return launch_flat_v<4, F16, RND>(a, vec, grid, pw, st);
-    case 8: return launch_flat_v<8, F16, RND>(a, vec, grid, pw, st);
-  }
-  return SKETCH_ERR_UNSUPPORTED;
-}
-
-template <int ZETA, int RND>
-int launch_smem_t(const sk::SmemArgs& g, const Plan& p, cudaStream_t st) {
-  if (p.wpc <= 4) {
-    auto k = sk::k_smem<ZETA, RND, 4>;
-    CU_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_bytes));
-    k<<<p.grid, p.wpc * 32, p.smem_bytes, st>>>(g);
-  } else {
-    auto k = sk::k_smem<ZETA, RND, 16>;
-    CU_TRY(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_bytes));
-    k<<<p.grid, p.wpc * 32, p.smem_bytes, st>>>(g);
-  }
-  return launch_check("k_smem");
-}
-
-template <int RND>
-int launch_smem(const sk::SmemArgs& g, const Plan& p, cudaStream_t st) {
-  switch (p.zeta_t) {
-    case 1: return launch_smem_t<1, RND>(g, p, st);
-    case 2: return launch_smem_t<2, RND>(g, p, st);
-    case 4: return launch_smem_t<4, RND>(g, p, st);
-    case 8: return launch_smem_t<8, RND>(g, p, st);
-  }
-  return SKETCH_ERR_UNSUPPORTED;
-}
-
-int ensure_packed(sketch* s, cudaStream_t st) {
-  if (s->packed) return SKETCH_OK;
-  int width = (s->d <= 32768) ? 2 : 4;
-  int64_t total = s->m * (int64_t)s->zeta;
-  size_t have = 0;
-  int rc = ensure_scratch(&s->packed, &have, (size_t)total * width);
+int ensure_packed(sketch* s, cudaStream_t st, bool force) {
+  if (s->packed_width && !force) return SKETCH_OK;
+  int rc = ensure_device(s);
   if (rc) return rc;
-  int rc2 = ensure_device(s);
-  if (rc2) return rc2;
+  const bool ranked = ranked_ok(s);
+  const int64_t pad = sk::smem_pad_rows();
+  const int64_t rows_padded = ((s->m + 31) / 32) * 32 + pad;
+  const int64_t total = (ranked ? rows_padded : s->m) * (int64_t)s->zeta;
+  rc = ensure_scratch(&s->packed, &s->packed_bytes, (size_t)total * (ranked ? 2 : 4));
+  if (rc) return rc;
   int64_t blocks = (total + 255) / 256;
   int64_t cap = (int64_t)s->sm_count * 16;
   int grid = (int)(blocks < cap ? blocks : cap);
   if (grid < 1) grid = 1;
-  if (width == 2) sk::k_hash_pack<uint16_t><<<grid, 256, 0, st>>>(s->seed, total, (uint32_t)s->zeta, s->db, (uint16_t*)s->packed);
-  else sk::k_hash_pack<uint32_t><<<grid, 256, 0, st>>>(s->seed, total, (uint32_t)s->zeta, s->db, (uint32_t*)s->packed);
-  rc = launch_check("k_hash_pack");
+  if (ranked) {
+    rc = launched(sk::launch_hash_pack_ranked(s->seed, s->zeta, rows_padded, s->db, (uint16_t*)s->packed, grid, st),
+                  "k_hash_pack_ranked");
+  } else {
+    sk::k_hash_pack32<<<grid, 256, 0, st>>>(s->seed, total, (uint32_t)s->zeta, s->db, (uint32_t*)s->packed);
+    rc = launch_check("k_hash_pack32");
+  }
+
   if (rc) return rc;
-  s->packed_width = width;
+  s->packed_width = ranked ? 2 : 4;
   return SKETCH_OK;
 }
 
@@ -354,7 +311,10 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
     g.s = make_args(s, A, n, lda, B, row_begin, rows, sr_seed, p.vec);
     g.rows_per_cta = p.rows_per_cta;
     g.d = s->d;
-    return rounding == SKETCH_SR ? launch_smem<1>(g, p, st) : launch_smem<0>(g, p, st);
+    rc = ensure_packed(s, st, false);
+    if (rc) return rc;
+    g.s.packed = s->packed;
+    return launched(sk::launch_smem_f16(g, s->zeta, p.wpc, p.grid, p.smem_bytes, st), "k_smem");
   }
 
   // flat / generic: RED into B itself (P == 1) or into P partial sketches folded afterwards
@@ -370,7 +330,7 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
   }
   int pw = 0;
   if (p.hash_mode == 2 && p.variant != SKETCH_VARIANT_GENERIC) {
-    rc = ensure_packed(s, st);
+    rc = ensure_packed(s, st, false);
     if (rc) return rc;
     pw = s->packed_width;
   }
@@ -379,16 +339,11 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
     a.replicas = P;
     a.packed = pw ? s->packed : nullptr;
     if (p.variant == SKETCH_VARIANT_GENERIC) {
-      if (!f16) sk::k_generic<false, 0><<<p.grid, sk::kFlatThreads, 0, st>>>(a);
-      else if (rounding == SKETCH_SR) sk::k_generic<true, 1><<<p.grid, sk::kFlatThreads, 0, st>>>(a);
-      else sk::k_generic<true, 0><<<p.grid, sk::kFlatThreads, 0, st>>>(a);
-      rc = launch_check("k_generic");
+      rc = launched(sk::launch_generic(a, f16, rounding == SKETCH_SR, p.grid, st), "k_generic");
     } else if (!f16) {
-      rc = launch_flat<false, 0>(a, s->zeta, p.vec, p.grid, pw, st);
-    } else if (rounding == SKETCH_SR) {
-      rc = launch_flat<true, 1>(a, s->zeta, p.vec, p.grid, pw, st);
+      rc = launched(sk::launch_flat_f32(a, s->zeta, p.vec, pw, p.grid, st), "k_flat<f32>");
     } else {
-      rc = launch_flat<true, 0>(a, s->zeta, p.vec, p.grid, pw, st);
+      rc = launched(sk::launch_flat_f16(a, s->zeta, p.vec, rounding == SKETCH_SR, pw, p.grid, st), "k_flat<f16>");
     }
     if (rc) return rc;
   }
@@ -534,7 +489,7 @@ int sketch_hashes_dump(const sketch_t* cs, int32_t* bucket_dev, uint8_t* signbit
 
 int sketch_precompute_hashes(sketch_t* s, void* stream) {
   if (!s) return SKETCH_ERR_NULL;
-  return ensure_packed(s, reinterpret_cast<cudaStream_t>(stream));
+  return ensure_packed(s, reinterpret_cast<cudaStream_t>(stream), true);
 }
 
 int sketch_apply_f32acc(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, float* B_dev, void* stream) {
