@@ -26,7 +26,7 @@ struct ScatterArgs {
 
 struct SmemArgs {
   ScatterArgs s;
-  int64_t rows_per_cta;  // multiple of 4 (row groups stay aligned in the global row index)
+  int64_t rows_per_cta;  // multiple of the kernel's ring rows (NQ*4); so is ScatterArgs::rows for this kernel
   int32_t d;
 };
 

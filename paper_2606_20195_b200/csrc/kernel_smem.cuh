@@ -26,8 +26,6 @@
 // profiles/r01_smem_hash_on_the_fly.md; the flat kernels keep both forms.)
 #pragma once
 
-#include <type_traits>
-
 #include "args.h"
 #include "device_util.cuh"
 
@@ -128,40 +126,36 @@ __global__ void __launch_bounds__(MAXW * 32) k_smem(SmemArgs g) {
   __syncthreads();
 
   const int64_t cta_r0 = (int64_t)blockIdx.x * g.rows_per_cta;
-  const int64_t cta_r1 = min(a.rows, cta_r0 + g.rows_per_cta);
+  const int64_t cta_r1 = min(a.rows, cta_r0 + g.rows_per_cta);  // a.rows is a multiple of RING_ROWS here
   const uint32_t col0 = warp * kSmemColsPerWarp + pcol * VEC;  // first column of this lane
   unsigned char* const my_col = smem_raw + col0 * 2u;
+  unsigned char* const my_dummy = smem_raw + (uint32_t)g.d * row_pitch + tid * 16u;  // 16 private bytes behind the sketch
 
+  // The host gives every CTA a whole number of ring iterations (rows_per_cta and the range handed to this
+  // kernel are multiples of NQ*R rows; the ragged remainder of a range goes to the flat kernel), so the
+  // loop below needs no row checks and exists in a single copy.
   if (cta_r0 < cta_r1) {
-    const int64_t nrows = cta_r1 - cta_r0;
-    const int64_t iters = (nrows + RING_ROWS - 1) / RING_ROWS;
-    const int64_t full_iters = nrows / RING_ROWS;  // iterations whose RING_ROWS rows all exist
-    // this lane's pointers for the current iteration's group 0; group q is q groups further
-    const float* ld_ptr = a.A + (cta_r0 + r) * a.lda + col0;
+    const int64_t iters = (cta_r1 - cta_r0) / RING_ROWS;
     const int64_t group_stride = (int64_t)R * a.lda;
-    const int64_t iter_stride = (int64_t)NQ * group_stride;
+    const float* const first_ptr = a.A + (cta_r0 + r) * a.lda + col0;        // this lane's (iteration 0, group 0)
     const ent_t* ent_ptr = reinterpret_cast<const ent_t*>(a.packed) + (a.row_begin + cta_r0 + r);
 
     float buf[NQ][VEC];
     ent_t ent[NQ];
-    // prologue: iteration 0's groups (row-checked; the packed array is padded, its loads need no check)
+    const float* ld_ptr = first_ptr;  // walks one group per load
 #pragma unroll
     for (int q = 0; q < NQ; ++q) {
-      if ((int64_t)q * R + r < nrows) ld_stream<VEC>(ld_ptr + q * group_stride, buf[q]);
-      else {
-#pragma unroll
-        for (int k = 0; k < VEC; ++k) buf[q][k] = 0.f;
-      }
+      ld_stream<VEC>(ld_ptr, buf[q]);
+      ld_ptr += group_stride;
       ent[q] = __ldg(ent_ptr + q * R);
     }
 
-    // one ring iteration; NEXT: 0 = no further loads, 1 = next iteration is complete (unchecked loads),
-    // 2 = next iteration is the ragged tail (row-checked loads; rows past the range read as zeros, which
-    // add +-0 to valid buckets)
-    auto ring_iteration = [&](int64_t it, auto next_tag) {
-      constexpr int NEXT = decltype(next_tag)::value;
-      const float* next_ptr = ld_ptr + iter_stride;
-      const int64_t next_rows_left = nrows - (it + 1) * RING_ROWS;
+    for (int64_t it = 0; it < iters; ++it) {
+      // the last iteration has nothing left to prefetch: it re-reads iteration 0 (valid addresses, data unused)
+      if (it + 1 == iters) {
+        ld_ptr = first_ptr;
+        ent_ptr -= it * RING_ROWS + RING_ROWS;
+      }
 #pragma unroll
       for (int q = 0; q < NQ; ++q) {
         float p[VEC];
@@ -169,16 +163,9 @@ __global__ void __launch_bounds__(MAXW * 32) k_smem(SmemArgs g) {
         for (int k = 0; k < VEC; ++k) p[k] = buf[q][k] * a.scale;
         const ent_t my_ent = ent[q];
         // refill this ring slot with the same group of the next iteration
-        if constexpr (NEXT == 1) {
-          ld_stream<VEC>(next_ptr + q * group_stride, buf[q]);
-        } else if constexpr (NEXT == 2) {
-          if ((int64_t)q * R + r < next_rows_left) ld_stream<VEC>(next_ptr + q * group_stride, buf[q]);
-          else {
-#pragma unroll
-            for (int k = 0; k < VEC; ++k) buf[q][k] = 0.f;
-          }
-        }
-        if constexpr (NEXT != 0) ent[q] = __ldg(ent_ptr + RING_ROWS + q * R);
+        ld_stream<VEC>(ld_ptr, buf[q]);
+        ld_ptr += group_stride;
+        ent[q] = __ldg(ent_ptr + RING_ROWS + q * R);
 
         uint32_t qv[VEC / 2];
 #pragma unroll
@@ -195,41 +182,43 @@ __global__ void __launch_bounds__(MAXW * 32) k_smem(SmemArgs g) {
             // sign bit of the entry replicated into both halves, XOR +1.0: +-1.0 in both halves
             mult[j] = (__byte_perm(w, 0, ((jc + j) & 1) ? 0x3232 : 0x1010) & 0x80008000u) ^ 0x3C003C00u;
           }
-          const uint32_t gmax = (e16[0] >> kE16GmaxShift) & 3u;  // warp-uniform: the warp is one row group
-          if (gmax == 0u) {
-            // common path: the JC read-modify-writes are independent -> all loads first
+          // pass 0: every (row, block) of rank 0.  No two of them share a word, so the JC read-modify-writes
+          // are independent: all loads first.  Ranked-later rows aim at the lane's private dummy word instead
+          // (no branch, no predicate on the memory operations).
+          {
             uint4 acc[JC];
 #pragma unroll
-            for (int j = 0; j < JC; ++j) acc[j] = *reinterpret_cast<uint4*>(addr[j]);
+            for (int j = 0; j < JC; ++j) {
+              unsigned char* const a0 = (e16[j] & (3u << kE16RankShift)) ? my_dummy : addr[j];
+              acc[j] = *reinterpret_cast<uint4*>(a0);
+            }
 #pragma unroll
             for (int j = 0; j < JC; ++j) rmw_add(acc[j], qv, mult[j]);
 #pragma unroll
-            for (int j = 0; j < JC; ++j) *reinterpret_cast<uint4*>(addr[j]) = acc[j];
-          } else {
-            // some rows of the group share a bucket: apply rank 0, then rank 1, ...
-            for (uint32_t k = 0; k <= gmax; ++k) {
-#pragma unroll
-              for (int j = 0; j < JC; ++j) {
-                if (((e16[j] >> kE16RankShift) & 3u) == k) {
-                  uint4 acc = *reinterpret_cast<uint4*>(addr[j]);
-                  rmw_add(acc, qv, mult[j]);
-                  *reinterpret_cast<uint4*>(addr[j]) = acc;
-                }
-              }
-              __syncwarp();
+            for (int j = 0; j < JC; ++j) {
+              unsigned char* const a0 = (e16[j] & (3u << kE16RankShift)) ? my_dummy : addr[j];
+              *reinterpret_cast<uint4*>(a0) = acc[j];
             }
           }
           __syncwarp();
+          // rows that share a bucket with an earlier row of the group (~6/(d/zeta) of the groups per block):
+          // one more pass per rank; gmax is the same in every lane (the warp is one row group)
+          const uint32_t gmax = (e16[0] >> kE16GmaxShift) & 3u;
+          for (uint32_t k = 1; k <= gmax; ++k) {
+#pragma unroll
+            for (int j = 0; j < JC; ++j) {
+              if (((e16[j] >> kE16RankShift) & 3u) == k) {
+                uint4 acc = *reinterpret_cast<uint4*>(addr[j]);
+                rmw_add(acc, qv, mult[j]);
+                *reinterpret_cast<uint4*>(addr[j]) = acc;
+              }
+            }
+            __syncwarp();
+          }
         }
       }
-      ld_ptr += iter_stride;
       ent_ptr += RING_ROWS;
-    };
-
-    int64_t it = 0;
-    for (; it + 1 < full_iters; ++it) ring_iteration(it, std::integral_constant<int, 1>{});
-    for (; it + 1 < iters; ++it) ring_iteration(it, std::integral_constant<int, 2>{});
-    ring_iteration(it, std::integral_constant<int, 0>{});
+    }
   }
   __syncthreads();
 

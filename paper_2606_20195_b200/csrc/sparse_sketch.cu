@@ -64,6 +64,7 @@ struct Plan {
   int variant, vec, replicas, hash_mode, grid, wpc, zeta_t;
   size_t smem_bytes;
   int64_t rows_per_cta;
+  int64_t rows_main;  // smem variant: rows handled by k_smem (multiple of its ring rows); the rest go to k_flat
 };
 
 int ensure_device(sketch* s) {
@@ -106,7 +107,7 @@ bool smem_feasible(const sketch* s, int n, int64_t lda, const void* A, const voi
   if (n % 64 != 0 || n / 64 > 16) return false;
   int vec = smem_vec_for(s->zeta);
   if (lda % vec != 0 || !aligned(A, 4 * (size_t)vec) || !aligned(B, 16)) return false;
-  size_t b = (size_t)s->d * n * 2;
+  size_t b = (size_t)s->d * n * 2 + (size_t)(n / 64) * 32 * 16;  // partial sketch + one dummy 16-byte word per thread
   if (b > (size_t)s->smem_optin) return false;
   if ((uint64_t)s->d * (uint64_t)n * 2ull >= (1ull << 31)) return false;
   *bytes = b;
@@ -170,11 +171,15 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
     if (per_sm > 32) per_sm = 32;
     int64_t grid = (int64_t)s->sm_count * per_sm;
     if (o && o->grid_ctas > 0) grid = o->grid_ctas;
-    const int64_t ring = sk::smem_ring_rows(s->zeta, p->wpc);  // rows per ring iteration of that instantiation
-    int64_t rpc = (rows + grid - 1) / grid;
+    // every CTA gets a whole number of ring iterations; the < ring ragged rows at the end of the range are
+    // scattered by the flat kernel straight into B (apply_device)
+    const int64_t ring = sk::smem_ring_rows(s->zeta, p->wpc);
+    const int64_t rows_main = rows / ring * ring;
+    p->rows_main = rows_main;
+    int64_t rpc = (rows_main + grid - 1) / grid;
     rpc = (rpc + ring - 1) / ring * ring;
     if (rpc < ring) rpc = ring;
-    grid = (rows + rpc - 1) / rpc;
+    grid = (rows_main + rpc - 1) / rpc;
     if (grid < 1) grid = 1;
     p->grid = (int)grid;
     p->rows_per_cta = rpc;
@@ -306,15 +311,26 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
 
   if (p.variant == SKETCH_VARIANT_SMEM) {
     if (!accumulate) CU_TRY(cudaMemsetAsync(B, 0, out_bytes, st));  // a0
-    if (rows == 0) return SKETCH_OK;
-    sk::SmemArgs g;
-    g.s = make_args(s, A, n, lda, B, row_begin, rows, sr_seed, p.vec);
-    g.rows_per_cta = p.rows_per_cta;
-    g.d = s->d;
-    rc = ensure_packed(s, st, false);
-    if (rc) return rc;
-    g.s.packed = s->packed;
-    return launched(sk::launch_smem_f16(g, s->zeta, p.wpc, p.grid, p.smem_bytes, st), "k_smem");
+    if (p.rows_main > 0) {
+      sk::SmemArgs g;
+      g.s = make_args(s, A, n, lda, B, row_begin, p.rows_main, sr_seed, p.vec);
+      g.rows_per_cta = p.rows_per_cta;
+      g.d = s->d;
+      rc = ensure_packed(s, st, false);
+      if (rc) return rc;
+      g.s.packed = s->packed;
+      rc = launched(sk::launch_smem_f16(g, s->zeta, p.wpc, p.grid, p.smem_bytes, st), "k_smem");
+      if (rc) return rc;
+    }
+    if (p.rows_main < rows) {  // ragged tail (< one ring iteration): flat 16-byte REDs straight into B
+      const int64_t tail = rows - p.rows_main;
+      sk::ScatterArgs a = make_args(s, A + p.rows_main * lda, n, lda, B, row_begin + p.rows_main, tail, sr_seed, 8);
+      const int hb = 32 / s->zeta;
+      const int grid = (int)((((tail + hb - 1) / hb) + 7) / 8);
+      rc = launched(sk::launch_flat_f16(a, s->zeta, 8, 0, 0, grid < 1 ? 1 : grid, st), "k_flat<f16> (tail)");
+      if (rc) return rc;
+    }
+    return SKETCH_OK;
   }
 
   // flat / generic: RED into B itself (P == 1) or into P partial sketches folded afterwards
