@@ -28,6 +28,7 @@ struct SmemArgs {
   ScatterArgs s;
   int64_t rows_per_cta;  // multiple of the kernel's ring rows (NQ*4); so is ScatterArgs::rows for this kernel
   int32_t d;
+  uint32_t zero;  // always 0; the kernel uses it to build a scheduling dependency ptxas cannot fold away
 };
 
 constexpr int kFlatThreads = 256;

@@ -8,11 +8,11 @@
 
 namespace sk {
 
-// packed entry -> canonical 32-bit entry (bucket | sign<<31).  16-bit entries are the ranked form written by
-// k_hash_pack_ranked (kernel_smem.cuh): bucket in bits 0..10, sign in bit 15 (rank bits ignored here).
+// packed entry -> canonical 32-bit entry (bucket | sign<<31).  16-bit entries are the form written by
+// k_hash_pack_rot (kernel_smem.cuh): bucket in bits 0..14, sign in bit 15, stored in sub-step order.
 template <typename PackT>
 SK_DEVINL uint32_t unpack_entry(PackT p) {
-  if constexpr (sizeof(PackT) == 2) return ((uint32_t)p & 0x07FFu) | (((uint32_t)p >> 15) << 31);
+  if constexpr (sizeof(PackT) == 2) return ((uint32_t)p & 0x7FFFu) | (((uint32_t)p >> 15) << 31);
   else return (uint32_t)p;
 }
 
@@ -86,7 +86,13 @@ __global__ void __launch_bounds__(kFlatThreads) k_flat(ScatterArgs a) {
       uint64_t ctr = (uint64_t)(a.row_begin + r0) * ZETA + lane;  // (row)*ZETA + j with row = r0 + lane/ZETA
       if constexpr (PRE) {
         int64_t lr = r0 + lane / ZETA;
-        e = (lr < a.rows) ? unpack_entry<PackT>(reinterpret_cast<const PackT*>(a.packed)[ctr]) : 0u;
+        uint64_t idx = ctr;
+        if constexpr (sizeof(PackT) == 2) {  // entry of block j sits at sub-step t = (j - row mod R) mod ZETA
+          constexpr uint32_t R = ZETA >= 4 ? 4 : ZETA;
+          const uint32_t rr = (uint32_t)((uint64_t)(a.row_begin + lr) % R);
+          idx = ctr - j + ((j + ZETA - rr) % ZETA);
+        }
+        e = (lr < a.rows) ? unpack_entry<PackT>(reinterpret_cast<const PackT*>(a.packed)[idx]) : 0u;
       } else {
         e = hash_entry(a.seed, ctr, j, a.db);
       }

@@ -3,27 +3,29 @@
 // Each CTA keeps one private d x n FP16 partial sketch in shared memory and streams a contiguous range
 // of rows; at the end it flushes the partial sketch into B with 16-byte result-discarding REDs.
 // sm_100a has no native shared-memory FP16 add (atomicAdd on shared assembles to a CAS loop), so every
-// sketch word has exactly one owner at any time and is updated with plain LDS.128 / HFMA2 / STS.128:
-//   - warp w of the CTA owns the 64-column slice [64w, 64w+64): no two warps touch the same word;
-//   - inside a warp the lanes are R = 4 rows x 8 column chunks of 8 columns.  One "row group" (4
-//     consecutive rows, aligned to 4 in the global row index) is scattered per step: for every stack
-//     block j the 4 rows read-modify-write their 4 buckets of block j at once.  Two rows of a group
-//     collide in block j with probability ~6/(d/zeta); the hash stage ranks such rows (rank = number
-//     of earlier rows of the group with the same bucket in that block) and a group with a non-zero
-//     rank takes a slow path that applies rank 0, then rank 1, ...  In the common path the ZETA
-//     read-modify-writes of a group are independent (blocks are disjoint row ranges of the sketch,
-//     PAPER.md:59-63), so the ZETA LDS.128 are in flight together.
+// sketch word is updated with plain LDS / HFMA2 / STS and the schedule guarantees that no two lanes
+// touch one word in the same instruction:
+//   - warp w of the CTA owns the 64-column slice [64w, 64w+64): no two warps ever touch the same word;
+//   - inside a warp the lanes are R rows x LPR column chunks of VEC columns (R = min(zeta, 4); zeta >= 4:
+//     4 rows x 8 lanes x 8 columns).  One "step" scatters R consecutive rows (aligned to R in the global
+//     row index) in zeta "sub-steps": in sub-step t the lanes of row r update stack block (r + t) mod zeta.
+//     The R rows of a step therefore hit R DIFFERENT blocks in every instruction, and blocks are disjoint
+//     row ranges of the sketch: a Latin-square schedule with no same-instruction
+//     conflicts, whatever the hash says.  Two rows that share a bucket meet in different sub-steps; the
+//     sub-steps of a warp are ordered (LDS/STS issue in order, __syncwarp between them), so the second
+//     one reads what the first one wrote.  No ranks, no slow path, no divergence.
 // The product s*a is rounded to FP16 once per element; the block sign enters as the +-1 multiplier of
 // HFMA2 (q * (+-1) + acc: the product is exact, one rounding = RN16(acc +- q)).
-// A goes straight from HBM into registers with 256-bit streaming loads through an NQ-deep register
-// ring (NQ row groups = NQ KiB in flight per warp): staging A through shared memory would add
-// 8 B/float to a shared-memory pipe that the 2*2*ZETA B/float of read-modify-write traffic already
-// loads, and the register file is otherwise idle (2-6 warps per SM).
-// Hash stage (a1) in its precomputed form: k_hash_pack_ranked writes one 16-bit entry per (row, block)
-//   bucket | rank<<11 | group_max_rank<<13 | sign<<15
-// and every lane loads its row's ZETA entries (2*ZETA bytes, +ZETA/(2n) of A's traffic) through the
-// same register ring.  (The on-the-fly form of this kernel cost ~25 of 135 instructions per row group,
-// profiles/r01_smem_hash_on_the_fly.md; the flat kernels keep both forms.)
+// A goes straight from HBM into registers with 256-bit streaming loads (staging A through shared memory
+// would add 8 B/float to the L1/shared data pipe that the 4*zeta B/float of read-modify-write traffic
+// already loads to ~3/4 of its 128 B/clk).  ptxas tracks all of a warp's global loads with ONE scoreboard,
+// so a wait for any load waits for every load in flight: loads are therefore issued in batches of K
+// steps.  A batch is converted (a3, a4) into a work set as soon as it has arrived, the next batch is issued
+// into the freed registers and is in flight for the whole time the work set is being scattered
+// (profiles/r01_smem_v4_scoreboard.md shows what a rolling ring does instead).
+// Hash stage (a1) in its precomputed form: k_hash_pack_rot writes one 16-bit entry per (row, sub-step)
+//   bucket | sign<<15      for block (row mod R + t) mod zeta
+// and every lane loads its row's zeta entries (2*zeta bytes per row, +zeta/(2n) of A's traffic).
 #pragma once
 
 #include "args.h"
@@ -31,193 +33,182 @@
 
 namespace sk {
 
-constexpr int kSmemVec = 8;                            // columns per lane
-constexpr int kSmemLpr = 8;                            // lanes per row
-constexpr int kSmemR = 4;                              // rows per group
-constexpr int kSmemColsPerWarp = kSmemVec * kSmemLpr;  // 64
-constexpr int kSmemMaxBucket = 2048;                   // 11-bit bucket field of the ranked 16-bit entry
-constexpr int kSmemPadRows = 128;                      // rows the packed array extends beyond m (ring look-ahead)
+constexpr int kSmemColsPerWarp = 64;
+constexpr int kSmemMaxBucket = 32767;  // 15-bit bucket field; index d is the CTA's dummy row
 
-// ranked 16-bit entry
-constexpr uint32_t kE16Bucket = 0x07FFu;
-constexpr uint32_t kE16RankShift = 11;  // 2 bits
-constexpr uint32_t kE16GmaxShift = 13;  // 2 bits: largest rank in the row group (same in all its entries)
+template <int ZETA>
+struct SmemGeom {
+  static constexpr int R = ZETA >= 4 ? 4 : ZETA;  // rows per step
+  static constexpr int LPR = 32 / R;              // lanes per row
+  static constexpr int VEC = kSmemColsPerWarp / LPR;  // columns per lane: 8 / 4 / 2
+  static constexpr int H2 = VEC / 2;              // half2 words per lane
+};
 
-// ring depth (row groups in flight per warp) per instantiation; the host sizes rows_per_cta from it
-constexpr int smem_ring_depth(int zeta, bool small_cta) { return small_cta ? (zeta == 8 ? 8 : 12) : 4; }
+constexpr int smem_rows_per_step(int zeta) { return zeta >= 4 ? 4 : zeta; }
+// K: steps per load batch; the host sizes rows_per_cta from it
+constexpr int smem_batch_steps(int zeta, bool small_cta) { return small_cta ? 8 : 2; }
 
 // ------------------------------------------------------------------------------------------------
-// a1 (precomputed form): ranked entries for every (row, block), rows padded beyond m.
-// One warp hashes 32/ZETA rows; ranks come from shuffles inside the aligned 4-row group.
+// a1 (precomputed form): entry (row, t) = hash of block (row mod R + t) mod ZETA.  One thread per entry.
 // ------------------------------------------------------------------------------------------------
 template <int ZETA>
-__global__ void k_hash_pack_ranked(uint64_t seed, int64_t rows_padded, uint32_t db, uint16_t* __restrict__ packed) {
-  constexpr int HB = 32 / ZETA;
-  constexpr int GL = kSmemR * ZETA;  // lanes per row group
-  static_assert(GL <= 32, "ZETA <= 8");
-  const uint32_t lane = threadIdx.x & 31;
-  const int64_t warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
-  const int64_t batches = rows_padded / HB;
-  for (int64_t b = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; b < batches; b += warps) {
-    const uint64_t ctr = (uint64_t)b * 32 + lane;  // (row)*ZETA + j with row = b*HB + lane/ZETA
-    const uint32_t e = hash_entry(seed, ctr, lane % ZETA, db);
-    const uint32_t bucket = entry_bucket(e);
-    const uint32_t row_in_group = (lane / ZETA) % kSmemR;
-    uint32_t rank = 0;
-#pragma unroll
-    for (int k = 1; k < kSmemR; ++k) {
-      const uint32_t other = __shfl_up_sync(0xFFFFFFFFu, bucket, k * ZETA);
-      rank += (row_in_group >= (uint32_t)k && other == bucket) ? 1u : 0u;
-    }
-    uint32_t gmax = rank;
-#pragma unroll
-    for (int off = 1; off < GL; off <<= 1) gmax = max(gmax, __shfl_xor_sync(0xFFFFFFFFu, gmax, off));
-    packed[ctr] = (uint16_t)(bucket | (rank << kE16RankShift) | (gmax << kE16GmaxShift) | ((e >> 31) << 15));
+__global__ void k_hash_pack_rot(uint64_t seed, int64_t rows, uint32_t db, uint16_t* __restrict__ packed) {
+  constexpr int R = SmemGeom<ZETA>::R;
+  const int64_t total = rows * ZETA;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += stride) {
+    const uint64_t row = (uint64_t)idx / ZETA;
+    const uint32_t t = (uint32_t)((uint64_t)idx % ZETA);
+    const uint32_t j = ((uint32_t)(row % R) + t) % ZETA;
+    const uint32_t e = hash_entry(seed, row * ZETA + j, j, db);
+    packed[idx] = (uint16_t)(entry_bucket(e) | ((e >> 31) << 15));
   }
 }
 
 template <int ZETA> struct EntRow;  // a row's ZETA 16-bit entries as one load
-template <> struct EntRow<1> { using type = uint16_t; };
-template <> struct EntRow<2> { using type = uint32_t; };
-template <> struct EntRow<4> { using type = uint2; };
-template <> struct EntRow<8> { using type = uint4; };
+template <> struct EntRow<1> { using type = uint16_t; static constexpr int W = 1; };
+template <> struct EntRow<2> { using type = uint32_t; static constexpr int W = 1; };
+template <> struct EntRow<4> { using type = uint2; static constexpr int W = 2; };
+template <> struct EntRow<8> { using type = uint4; static constexpr int W = 4; };
 
 template <int ZETA>
-SK_DEVINL uint32_t entrow_word(const typename EntRow<ZETA>::type& e, int w) {
-  if constexpr (ZETA == 1) return (uint32_t)e;
-  else if constexpr (ZETA == 2) return e;
-  else if constexpr (ZETA == 4) return w == 0 ? e.x : e.y;
-  else return w == 0 ? e.x : w == 1 ? e.y : w == 2 ? e.z : e.w;
+SK_DEVINL void entrow_load(const void* p, uint32_t (&w)[EntRow<ZETA>::W]) {
+  if constexpr (ZETA == 1) w[0] = __ldg(reinterpret_cast<const uint16_t*>(p));
+  else if constexpr (ZETA == 2) w[0] = __ldg(reinterpret_cast<const uint32_t*>(p));
+  else if constexpr (ZETA == 4) {
+    const uint2 v = __ldg(reinterpret_cast<const uint2*>(p));
+    w[0] = v.x; w[1] = v.y;
+  } else {
+    const uint4 v = __ldg(reinterpret_cast<const uint4*>(p));
+    w[0] = v.x; w[1] = v.y; w[2] = v.z; w[3] = v.w;
+  }
 }
 
-// acc (4 half2 words) += mult * q  (mult = +-1 in both halves)
-SK_DEVINL void rmw_add(uint4& acc, const uint32_t (&q)[4], uint32_t mult) {
-  const __half2 m = *reinterpret_cast<const __half2*>(&mult);
-  __half2 x0 = __hfma2(*reinterpret_cast<const __half2*>(&q[0]), m, *reinterpret_cast<__half2*>(&acc.x));
-  __half2 x1 = __hfma2(*reinterpret_cast<const __half2*>(&q[1]), m, *reinterpret_cast<__half2*>(&acc.y));
-  __half2 x2 = __hfma2(*reinterpret_cast<const __half2*>(&q[2]), m, *reinterpret_cast<__half2*>(&acc.z));
-  __half2 x3 = __hfma2(*reinterpret_cast<const __half2*>(&q[3]), m, *reinterpret_cast<__half2*>(&acc.w));
-  acc.x = *reinterpret_cast<uint32_t*>(&x0);
-  acc.y = *reinterpret_cast<uint32_t*>(&x1);
-  acc.z = *reinterpret_cast<uint32_t*>(&x2);
-  acc.w = *reinterpret_cast<uint32_t*>(&x3);
+// shared-memory accesses by 32-bit shared-window address (no generic-address arithmetic in the loop)
+template <int H2>
+SK_DEVINL void lds_h2(uint32_t addr, uint32_t (&v)[H2]) {
+  if constexpr (H2 == 4) asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(addr) : "memory");
+  else if constexpr (H2 == 2) asm volatile("ld.shared.v2.b32 {%0,%1}, [%2];" : "=r"(v[0]), "=r"(v[1]) : "r"(addr) : "memory");
+  else asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v[0]) : "r"(addr) : "memory");
+}
+template <int H2>
+SK_DEVINL void sts_h2(uint32_t addr, const uint32_t (&v)[H2]) {
+  if constexpr (H2 == 4) asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]) : "memory");
+  else if constexpr (H2 == 2) asm volatile("st.shared.v2.b32 [%0], {%1,%2};" ::"r"(addr), "r"(v[0]), "r"(v[1]) : "memory");
+  else asm volatile("st.shared.b32 [%0], %1;" ::"r"(addr), "r"(v[0]) : "memory");
+}
+// acc = q * mult + acc per FP16 half, one rounding, subnormals kept
+SK_DEVINL uint32_t hfma2_bits(uint32_t q, uint32_t mult, uint32_t acc) {
+  uint32_t d;
+  asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(d) : "r"(q), "r"(mult), "r"(acc));
+  return d;
 }
 
-template <int ZETA, int NQ, int MAXW>
+template <int ZETA, int K>
+struct SmemLoadSet {  // destination of the K steps of loads in flight
+  float a[K][SmemGeom<ZETA>::VEC];
+  uint32_t e[K][EntRow<ZETA>::W];
+};
+template <int ZETA, int K>
+struct SmemWorkSet {  // the K steps being scattered: RN16(s*a) pairs and masked entries
+  uint32_t q[K][SmemGeom<ZETA>::H2];
+  uint32_t e[K][EntRow<ZETA>::W];
+};
+
+template <int ZETA, int K, int MAXW>
 __global__ void __launch_bounds__(MAXW * 32) k_smem(SmemArgs g) {
-  constexpr int VEC = kSmemVec, LPR = kSmemLpr, R = kSmemR;
+  using G = SmemGeom<ZETA>;
+  constexpr int R = G::R, LPR = G::LPR, VEC = G::VEC, H2 = G::H2, EW = EntRow<ZETA>::W;
   static_assert(ZETA == 1 || ZETA == 2 || ZETA == 4 || ZETA == 8, "ZETA in {1,2,4,8}");
-  static_assert(2 * NQ * R <= kSmemPadRows, "packed-array padding covers the look-ahead");
-  constexpr int RING_ROWS = NQ * R;
-  constexpr int JC = ZETA < 4 ? ZETA : 4;  // blocks handled together (bounds the accumulator registers)
-  using ent_t = typename EntRow<ZETA>::type;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const ScatterArgs& a = g.s;
   const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t r = lane / LPR, pcol = lane % LPR;
-  const uint32_t row_pitch = (uint32_t)a.n * 2u;  // bytes per sketch row in shared memory
+  const uint32_t pitch = (uint32_t)a.n * 2u;  // bytes per sketch row in shared memory
 
-  // ---- a0 (private part): zero the partial sketch
+  // ---- a0 (private part): zero the partial sketch (+ the dummy row d that absorbs out-of-range steps)
   {
     uint4* z = reinterpret_cast<uint4*>(smem_raw);
-    const uint32_t n16 = (uint32_t)g.d * row_pitch / 16u;
+    const uint32_t n16 = ((uint32_t)g.d + 1u) * pitch / 16u;
     for (uint32_t k = tid; k < n16; k += blockDim.x) z[k] = make_uint4(0, 0, 0, 0);
   }
   __syncthreads();
 
-  const int64_t cta_r0 = (int64_t)blockIdx.x * g.rows_per_cta;
-  const int64_t cta_r1 = min(a.rows, cta_r0 + g.rows_per_cta);  // a.rows is a multiple of RING_ROWS here
-  const uint32_t col0 = warp * kSmemColsPerWarp + pcol * VEC;  // first column of this lane
-  unsigned char* const my_col = smem_raw + col0 * 2u;
-  unsigned char* const my_dummy = smem_raw + (uint32_t)g.d * row_pitch + tid * 16u;  // 16 private bytes behind the sketch
+  const int64_t cta_r0 = (int64_t)blockIdx.x * g.rows_per_cta;          // multiple of R
+  const int64_t cta_r1 = min(a.rows, cta_r0 + g.rows_per_cta);
+  const uint32_t col0 = warp * kSmemColsPerWarp + pcol * VEC;            // first column of this lane
+  const uint32_t lane_base = (uint32_t)__cvta_generic_to_shared(smem_raw) + col0 * 2u;
+  const uint32_t dummy_word = (uint32_t)g.d | ((uint32_t)g.d << 16);     // every entry -> row d, sign +
 
-  // The host gives every CTA a whole number of ring iterations (rows_per_cta and the range handed to this
-  // kernel are multiples of NQ*R rows; the ragged remainder of a range goes to the flat kernel), so the
-  // loop below needs no row checks and exists in a single copy.
   if (cta_r0 < cta_r1) {
-    const int64_t iters = (cta_r1 - cta_r0) / RING_ROWS;
-    const int64_t group_stride = (int64_t)R * a.lda;
-    const float* const first_ptr = a.A + (cta_r0 + r) * a.lda + col0;        // this lane's (iteration 0, group 0)
-    const ent_t* ent_ptr = reinterpret_cast<const ent_t*>(a.packed) + (a.row_begin + cta_r0 + r);
+    const int64_t last_row = cta_r1 - 1;
+    const float* const Acol = a.A + col0;
+    const unsigned char* const ent_base = reinterpret_cast<const unsigned char*>(a.packed) + (size_t)a.row_begin * (ZETA * 2);
+    const int32_t nsteps = (int32_t)((cta_r1 - cta_r0 + R - 1) / R);
 
-    float buf[NQ][VEC];
-    ent_t ent[NQ];
-    const float* ld_ptr = first_ptr;  // walks one group per load
+    SmemLoadSet<ZETA, K> L;
+    SmemWorkSet<ZETA, K> W;
+
+    // issue the loads of the batch that starts at step s0; rows past the CTA's range re-read its last row
+    auto load_batch = [&](int32_t s0) {
 #pragma unroll
-    for (int q = 0; q < NQ; ++q) {
-      ld_stream<VEC>(ld_ptr, buf[q]);
-      ld_ptr += group_stride;
-      ent[q] = __ldg(ent_ptr + q * R);
-    }
-
-    for (int64_t it = 0; it < iters; ++it) {
-      // the last iteration has nothing left to prefetch: it re-reads iteration 0 (valid addresses, data unused)
-      if (it + 1 == iters) {
-        ld_ptr = first_ptr;
-        ent_ptr -= it * RING_ROWS + RING_ROWS;
+      for (int s = 0; s < K; ++s) {
+        const int64_t row = min(cta_r0 + (int64_t)(s0 + s) * R + r, last_row);
+        ld_stream<VEC>(Acol + row * a.lda, L.a[s]);
+        entrow_load<ZETA>(ent_base + row * (ZETA * 2), L.e[s]);
       }
+    };
+    // a3 + a4: first use of every loaded register (waits for the whole batch): q = RN16(s * a), entries of
+    // steps past the range -> dummy row.  Afterwards L is free for the next batch of loads.
+    auto cook_batch = [&](int32_t s0, uint32_t token) {
+      // `token` is 0 at run time but opaque to ptxas: it ties the conversion (and, through the registers of L,
+      // the next batch of loads) behind the last read-modify-write of the batch that has just been scattered,
+      // so the loads stay one whole scatter phase ahead of their first use instead of being interleaved
+      const float scale = __uint_as_float(__float_as_uint(a.scale) | token);
 #pragma unroll
-      for (int q = 0; q < NQ; ++q) {
-        float p[VEC];
+      for (int s = 0; s < K; ++s) {
+        const bool valid = cta_r0 + (int64_t)(s0 + s) * R + r <= last_row;
 #pragma unroll
-        for (int k = 0; k < VEC; ++k) p[k] = buf[q][k] * a.scale;
-        const ent_t my_ent = ent[q];
-        // refill this ring slot with the same group of the next iteration
-        ld_stream<VEC>(ld_ptr, buf[q]);
-        ld_ptr += group_stride;
-        ent[q] = __ldg(ent_ptr + RING_ROWS + q * R);
-
-        uint32_t qv[VEC / 2];
+        for (int k = 0; k < H2; ++k) W.q[s][k] = pack_rn(L.a[s][2 * k] * scale, L.a[s][2 * k + 1] * scale);
 #pragma unroll
-        for (int k = 0; k < VEC / 2; ++k) qv[k] = pack_rn(p[2 * k], p[2 * k + 1]);
+        for (int w = 0; w < EW; ++w) W.e[s][w] = valid ? L.e[s][w] : dummy_word;
+      }
+    };
+    // a5: zeta sub-steps per step; sub-step t of row r updates block (r + t) mod zeta
+    auto scatter_batch = [&]() -> uint32_t {
+      uint32_t last = 0;
 #pragma unroll
-        for (int jc = 0; jc < ZETA; jc += JC) {
-          unsigned char* addr[JC];
-          uint32_t mult[JC], e16[JC];
+      for (int s = 0; s < K; ++s) {
+        uint32_t addr[ZETA], mult[ZETA];
 #pragma unroll
-          for (int j = 0; j < JC; ++j) {
-            const uint32_t w = entrow_word<ZETA>(my_ent, (jc + j) >> 1);
-            e16[j] = ((jc + j) & 1) ? (w >> 16) : (w & 0xFFFFu);
-            addr[j] = my_col + (e16[j] & kE16Bucket) * row_pitch;
-            // sign bit of the entry replicated into both halves, XOR +1.0: +-1.0 in both halves
-            mult[j] = (__byte_perm(w, 0, ((jc + j) & 1) ? 0x3232 : 0x1010) & 0x80008000u) ^ 0x3C003C00u;
-          }
-          // pass 0: every (row, block) of rank 0.  No two of them share a word, so the JC read-modify-writes
-          // are independent: all loads first.  Ranked-later rows aim at the lane's private dummy word instead
-          // (no branch, no predicate on the memory operations).
-          {
-            uint4 acc[JC];
+        for (int t = 0; t < ZETA; ++t) {
+          const uint32_t w = W.e[s][t >> 1];
+          const uint32_t bucket = (t & 1) ? ((w >> 16) & 0x7FFFu) : (w & 0x7FFFu);
+          addr[t] = bucket * pitch + lane_base;
+          // sign bit of the entry replicated into both halves, XOR +1.0: +-1.0 in both halves
+          mult[t] = (__byte_perm(w, 0, (t & 1) ? 0x3232 : 0x1010) & 0x80008000u) ^ 0x3C003C00u;
+        }
 #pragma unroll
-            for (int j = 0; j < JC; ++j) {
-              unsigned char* const a0 = (e16[j] & (3u << kE16RankShift)) ? my_dummy : addr[j];
-              acc[j] = *reinterpret_cast<uint4*>(a0);
-            }
+        for (int t = 0; t < ZETA; ++t) {
+          uint32_t acc[H2];
+          lds_h2<H2>(addr[t], acc);
 #pragma unroll
-            for (int j = 0; j < JC; ++j) rmw_add(acc[j], qv, mult[j]);
-#pragma unroll
-            for (int j = 0; j < JC; ++j) {
-              unsigned char* const a0 = (e16[j] & (3u << kE16RankShift)) ? my_dummy : addr[j];
-              *reinterpret_cast<uint4*>(a0) = acc[j];
-            }
-          }
-          __syncwarp();
-          // rows that share a bucket with an earlier row of the group (~6/(d/zeta) of the groups per block):
-          // one more pass per rank; gmax is the same in every lane (the warp is one row group)
-          const uint32_t gmax = (e16[0] >> kE16GmaxShift) & 3u;
-          for (uint32_t k = 1; k <= gmax; ++k) {
-#pragma unroll
-            for (int j = 0; j < JC; ++j) {
-              if (((e16[j] >> kE16RankShift) & 3u) == k) {
-                uint4 acc = *reinterpret_cast<uint4*>(addr[j]);
-                rmw_add(acc, qv, mult[j]);
-                *reinterpret_cast<uint4*>(addr[j]) = acc;
-              }
-            }
-            __syncwarp();
-          }
+          for (int k = 0; k < H2; ++k) acc[k] = hfma2_bits(W.q[s][k], mult[t], acc[k]);
+          sts_h2<H2>(addr[t], acc);
+          if (R > 1) __syncwarp();  // the next sub-step of another row may read this word
+          last = acc[0];
         }
       }
-      ent_ptr += RING_ROWS;
+      return last & g.zero;
+    };
+
+    load_batch(0);
+    cook_batch(0, 0u);
+    load_batch(K);
+    for (int32_t s0 = 0; s0 < nsteps; s0 += K) {
+      const uint32_t token = scatter_batch();  // the loads issued one iteration ago are in flight meanwhile
+      cook_batch(s0 + K, token);               // first touch of L: everything in flight is a scatter phase old
+      load_batch(s0 + 2 * K);                  // L is free again; consumed across the back-edge
     }
   }
   __syncthreads();
@@ -225,7 +216,7 @@ __global__ void __launch_bounds__(MAXW * 32) k_smem(SmemArgs g) {
   // ---- flush: partial sketch -> B with 16-byte result-discarding REDs (layouts coincide: [d][n])
   {
     const uint4* z = reinterpret_cast<const uint4*>(smem_raw);
-    const uint32_t n16 = (uint32_t)g.d * row_pitch / 16u;
+    const uint32_t n16 = (uint32_t)g.d * pitch / 16u;
     __half* B = reinterpret_cast<__half*>(a.B);
     // stagger the start so the CTAs do not all hit the same L2 lines at once
     const uint32_t shift = (uint32_t)((blockIdx.x * 2654435761u) % n16);

@@ -15,10 +15,11 @@ cudaError_t launch_generic(const ScatterArgs& a, bool f16, int rounding, int gri
 
 // shared-memory-privatised FP16-RN scatter; wpc = warps per CTA = n / 64
 cudaError_t launch_smem_f16(const SmemArgs& g, int zeta, int wpc, int grid, size_t smem_bytes, cudaStream_t st);
-int smem_ring_rows(int zeta, int wpc);  // rows one ring iteration of that instantiation covers
-cudaError_t launch_hash_pack_ranked(uint64_t seed, int zeta, int64_t rows_padded, uint32_t db, uint16_t* out, int grid,
-                                    cudaStream_t st);
-int smem_pad_rows();
+int smem_ring_rows(int zeta, int wpc);  // rows one loop iteration (one load batch) of that instantiation covers
+int smem_step_rows(int zeta);           // R: rows per step; row ranges given to the kernel start at a multiple of it
+// a1 precomputed: 16-bit entries (bucket | sign<<15), index row*zeta + t for block (row mod R + t) mod zeta
+cudaError_t launch_hash_pack_rot(uint64_t seed, int zeta, int64_t rows, uint32_t db, uint16_t* out, int grid,
+                                 cudaStream_t st);
 int smem_max_bucket();
 
 }  // namespace sk

@@ -1,4 +1,4 @@
-// launch_smem.cu -- instantiations of the shared-memory-privatised scatter and its ranked hash-pack kernel.
+// launch_smem.cu -- instantiations of the shared-memory-privatised scatter and its hash-pack kernel.
 #include "kernel_smem.cuh"
 #include "launch.h"
 
@@ -9,12 +9,12 @@ template <int ZETA>
 cudaError_t go(const SmemArgs& g, int wpc, int grid, size_t smem_bytes, cudaStream_t st) {
   cudaError_t e;
   if (wpc <= 4) {
-    auto k = k_smem<ZETA, smem_ring_depth(ZETA, true), 4>;
+    auto k = k_smem<ZETA, smem_batch_steps(ZETA, true), 4>;
     e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     if (e != cudaSuccess) return e;
     k<<<grid, wpc * 32, smem_bytes, st>>>(g);
   } else {
-    auto k = k_smem<ZETA, smem_ring_depth(ZETA, false), 16>;
+    auto k = k_smem<ZETA, smem_batch_steps(ZETA, false), 16>;
     e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     if (e != cudaSuccess) return e;
     k<<<grid, wpc * 32, smem_bytes, st>>>(g);
@@ -34,17 +34,17 @@ cudaError_t launch_smem_f16(const SmemArgs& g, int zeta, int wpc, int grid, size
   return cudaErrorInvalidValue;
 }
 
-int smem_ring_rows(int zeta, int wpc) { return kSmemR * smem_ring_depth(zeta, wpc <= 4); }
-int smem_pad_rows() { return kSmemPadRows; }
+int smem_ring_rows(int zeta, int wpc) { return smem_rows_per_step(zeta) * smem_batch_steps(zeta, wpc <= 4); }
+int smem_step_rows(int zeta) { return smem_rows_per_step(zeta); }
 int smem_max_bucket() { return kSmemMaxBucket; }
 
-cudaError_t launch_hash_pack_ranked(uint64_t seed, int zeta, int64_t rows_padded, uint32_t db, uint16_t* out, int grid,
-                                    cudaStream_t st) {
+cudaError_t launch_hash_pack_rot(uint64_t seed, int zeta, int64_t rows, uint32_t db, uint16_t* out, int grid,
+                                 cudaStream_t st) {
   switch (zeta) {
-    case 1: k_hash_pack_ranked<1><<<grid, 256, 0, st>>>(seed, rows_padded, db, out); break;
-    case 2: k_hash_pack_ranked<2><<<grid, 256, 0, st>>>(seed, rows_padded, db, out); break;
-    case 4: k_hash_pack_ranked<4><<<grid, 256, 0, st>>>(seed, rows_padded, db, out); break;
-    case 8: k_hash_pack_ranked<8><<<grid, 256, 0, st>>>(seed, rows_padded, db, out); break;
+    case 1: k_hash_pack_rot<1><<<grid, 256, 0, st>>>(seed, rows, db, out); break;
+    case 2: k_hash_pack_rot<2><<<grid, 256, 0, st>>>(seed, rows, db, out); break;
+    case 4: k_hash_pack_rot<4><<<grid, 256, 0, st>>>(seed, rows, db, out); break;
+    case 8: k_hash_pack_rot<8><<<grid, 256, 0, st>>>(seed, rows, db, out); break;
     default: return cudaErrorInvalidValue;
   }
   return cudaGetLastError();

@@ -50,7 +50,7 @@ struct sketch {
   int smem_per_sm;
   // library-owned scratch
   void* rep;  size_t rep_bytes;        // replicated partial sketches
-  void* packed; size_t packed_bytes; int packed_width;  // 0 = none, 2 = ranked 16-bit entries, 4 = plain 32-bit
+  void* packed; size_t packed_bytes; int packed_width;  // 0 = none, 2 = 16-bit entries in sub-step order, 4 = plain 32-bit
   void* stage[2]; size_t stage_bytes;  // host-path staging
   void* bdev; size_t bdev_bytes;
   cudaStream_t st_copy, st_comp;
@@ -97,19 +97,15 @@ int ensure_scratch(void** buf, size_t* have, size_t want) {
 
 inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 inline bool zeta_templated(int z) { return z == 1 || z == 2 || z == 4 || z == 8; }
-inline bool ranked_ok(const sketch* s) { return zeta_templated(s->zeta) && s->d <= sk::smem_max_bucket(); }
-
-// smem layout: 8 lanes x 8 columns = 64 columns per warp for every zeta
-inline int smem_vec_for(int) { return 8; }
+inline bool rot_ok(const sketch* s) { return zeta_templated(s->zeta) && s->d <= sk::smem_max_bucket(); }
 
 bool smem_feasible(const sketch* s, int n, int64_t lda, const void* A, const void* B, size_t* bytes) {
-  if (!zeta_templated(s->zeta)) return false;
+  if (!rot_ok(s)) return false;
   if (n % 64 != 0 || n / 64 > 16) return false;
-  int vec = smem_vec_for(s->zeta);
+  const int vec = 2 * sk::smem_step_rows(s->zeta);  // columns per lane: 8 / 4 / 2
   if (lda % vec != 0 || !aligned(A, 4 * (size_t)vec) || !aligned(B, 16)) return false;
-  size_t b = (size_t)s->d * n * 2 + (size_t)(n / 64) * 32 * 16;  // partial sketch + one dummy 16-byte word per thread
+  size_t b = ((size_t)s->d + 1) * n * 2;  // partial sketch + the dummy row d
   if (b > (size_t)s->smem_optin) return false;
-  if ((uint64_t)s->d * (uint64_t)n * 2ull >= (1ull << 31)) return false;
   *bytes = b;
   return true;
 }
@@ -138,10 +134,11 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
   p->hash_mode = (o && o->hash_mode) ? o->hash_mode : 1;
   if (p->hash_mode != 1 && p->hash_mode != 2) return SKETCH_ERR_INVALID;
   size_t sm_bytes = 0;
-  // the privatised kernel is FP16-RN with precomputed ranked hashes; its 4-row groups must be aligned in the
-  // global row index.  Everything else (FP32, SR, odd shapes) runs the flat / generic kernels.
+  // the privatised kernel is FP16-RN with precomputed hashes; its R-row steps must be aligned in the global
+  // row index.  Everything else (FP32, SR, odd shapes) runs the flat / generic kernels.
   const int64_t rb0 = o ? o->row_begin : 0;
-  bool sm_ok = f16 && rounding == SKETCH_RN && ranked_ok(s) && (rb0 % 4 == 0) && smem_feasible(s, n, lda, A, B, &sm_bytes);
+  bool sm_ok = f16 && rounding == SKETCH_RN && smem_feasible(s, n, lda, A, B, &sm_bytes) &&
+               (rb0 % sk::smem_step_rows(s->zeta) == 0);
   int vmax = flat_vec_for(f16, n, lda, A, B, 8);
   int vpair = flat_vec_for(f16, n, lda, A, B, f16 ? 2 : 1);
   bool zt = zeta_templated(s->zeta);
@@ -159,8 +156,8 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
   p->zeta_t = s->zeta;
 
   if (v == SKETCH_VARIANT_SMEM) {
-    p->hash_mode = 2;  // always the precomputed ranked entries
-    p->vec = smem_vec_for(s->zeta);
+    p->hash_mode = 2;  // always the precomputed entries
+    p->vec = 2 * sk::smem_step_rows(s->zeta);
     p->wpc = n / 64;
     p->smem_bytes = sm_bytes;
     p->replicas = 1;
@@ -171,10 +168,10 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
     if (per_sm > 32) per_sm = 32;
     int64_t grid = (int64_t)s->sm_count * per_sm;
     if (o && o->grid_ctas > 0) grid = o->grid_ctas;
-    // every CTA gets a whole number of ring iterations; the < ring ragged rows at the end of the range are
-    // scattered by the flat kernel straight into B (apply_device)
+    // every CTA gets a whole number of loop iterations (two load batches); the kernel itself masks the
+    // steps past the end of the range
     const int64_t ring = sk::smem_ring_rows(s->zeta, p->wpc);
-    const int64_t rows_main = rows / ring * ring;
+    const int64_t rows_main = rows;
     p->rows_main = rows_main;
     int64_t rpc = (rows_main + grid - 1) / grid;
     rpc = (rpc + ring - 1) / ring * ring;
@@ -246,33 +243,28 @@ int launched(cudaError_t e, const char* what) {
   return e == cudaSuccess ? SKETCH_OK : cuda_fail(e, what);
 }
 
-// a1 in its precomputed form.  Ranked 16-bit entries (bucket | rank<<11 | group_max_rank<<13 | sign<<15, rows
-// padded to 64 beyond m) when the sketch fits them, else plain 32-bit entries.  force: re-run the pack kernel.
-
+// a1 in its precomputed form.  16-bit entries in sub-step order (kernel_smem.cuh) when zeta is templated and the
+// sketch fits the 15-bit bucket field, else plain 32-bit entries (bucket | sign<<31).  force: re-run the kernel.
 int ensure_packed(sketch* s, cudaStream_t st, bool force) {
   if (s->packed_width && !force) return SKETCH_OK;
   int rc = ensure_device(s);
   if (rc) return rc;
-  const bool ranked = ranked_ok(s);
-  const int64_t pad = sk::smem_pad_rows();
-  const int64_t rows_padded = ((s->m + 31) / 32) * 32 + pad;
-  const int64_t total = (ranked ? rows_padded : s->m) * (int64_t)s->zeta;
-  rc = ensure_scratch(&s->packed, &s->packed_bytes, (size_t)total * (ranked ? 2 : 4));
+  const bool rot = rot_ok(s);
+  const int64_t total = s->m * (int64_t)s->zeta;
+  rc = ensure_scratch(&s->packed, &s->packed_bytes, (size_t)total * (rot ? 2 : 4));
   if (rc) return rc;
   int64_t blocks = (total + 255) / 256;
   int64_t cap = (int64_t)s->sm_count * 16;
   int grid = (int)(blocks < cap ? blocks : cap);
   if (grid < 1) grid = 1;
-  if (ranked) {
-    rc = launched(sk::launch_hash_pack_ranked(s->seed, s->zeta, rows_padded, s->db, (uint16_t*)s->packed, grid, st),
-                  "k_hash_pack_ranked");
+  if (rot) {
+    rc = launched(sk::launch_hash_pack_rot(s->seed, s->zeta, s->m, s->db, (uint16_t*)s->packed, grid, st), "k_hash_pack_rot");
   } else {
     sk::k_hash_pack32<<<grid, 256, 0, st>>>(s->seed, total, (uint32_t)s->zeta, s->db, (uint32_t*)s->packed);
     rc = launch_check("k_hash_pack32");
   }
-
   if (rc) return rc;
-  s->packed_width = ranked ? 2 : 4;
+  s->packed_width = rot ? 2 : 4;
   return SKETCH_OK;
 }
 
@@ -316,18 +308,11 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
       g.s = make_args(s, A, n, lda, B, row_begin, p.rows_main, sr_seed, p.vec);
       g.rows_per_cta = p.rows_per_cta;
       g.d = s->d;
+      g.zero = 0u;
       rc = ensure_packed(s, st, false);
       if (rc) return rc;
       g.s.packed = s->packed;
       rc = launched(sk::launch_smem_f16(g, s->zeta, p.wpc, p.grid, p.smem_bytes, st), "k_smem");
-      if (rc) return rc;
-    }
-    if (p.rows_main < rows) {  // ragged tail (< one ring iteration): flat 16-byte REDs straight into B
-      const int64_t tail = rows - p.rows_main;
-      sk::ScatterArgs a = make_args(s, A + p.rows_main * lda, n, lda, B, row_begin + p.rows_main, tail, sr_seed, 8);
-      const int hb = 32 / s->zeta;
-      const int grid = (int)((((tail + hb - 1) / hb) + 7) / 8);
-      rc = launched(sk::launch_flat_f16(a, s->zeta, 8, 0, 0, grid < 1 ? 1 : grid, st), "k_flat<f16> (tail)");
       if (rc) return rc;
     }
     return SKETCH_OK;
