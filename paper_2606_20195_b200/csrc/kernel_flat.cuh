@@ -9,10 +9,10 @@
 namespace sk {
 
 // packed entry -> canonical 32-bit entry (bucket | sign<<31).  16-bit entries are the form written by
-// k_hash_pack_rot (kernel_smem.cuh): bucket in bits 0..14, sign in bit 15, stored in sub-step order.
+// k_hash_pack_rot (kernel_smem.cuh): bucket in bits 0..10, sign in bit 15, stored in sub-step order.
 template <typename PackT>
 SK_DEVINL uint32_t unpack_entry(PackT p) {
-  if constexpr (sizeof(PackT) == 2) return ((uint32_t)p & 0x7FFFu) | (((uint32_t)p >> 15) << 31);
+  if constexpr (sizeof(PackT) == 2) return ((uint32_t)p & 0x07FFu) | (((uint32_t)p >> 15) << 31);
   else return (uint32_t)p;
 }
 

@@ -11,9 +11,12 @@
 //     row index) in zeta "sub-steps": in sub-step t the lanes of row r update stack block (r + t) mod zeta.
 //     The R rows of a step therefore hit R DIFFERENT blocks in every instruction, and blocks are disjoint
 //     row ranges of the sketch: a Latin-square schedule with no same-instruction
-//     conflicts, whatever the hash says.  Two rows that share a bucket meet in different sub-steps; the
-//     sub-steps of a warp are ordered (LDS/STS issue in order, __syncwarp between them), so the second
-//     one reads what the first one wrote.  No ranks, no slow path, no divergence.
+//     conflicts, whatever the hash says.  Two rows that share a bucket meet in different sub-steps, and the
+//     sub-steps of a warp are ordered (LDS/STS issue in order, __syncwarp between them).  To overlap the
+//     shared-memory latency with the previous sub-step's HFMA2/STS, the LDS of a sub-step is issued D = 1
+//     sub-steps early; the hash stage marks the (row, sub-step) entries whose sketch row is written inside
+//     that window (probability ~D/(d/zeta)) and only those lanes repeat the LDS after the store.
+//     No ranks, no branches, no divergence.
 // The product s*a is rounded to FP16 once per element; the block sign enters as the +-1 multiplier of
 // HFMA2 (q * (+-1) + acc: the product is exact, one rounding = RN16(acc +- q)).
 // A goes straight from HBM into registers with 256-bit streaming loads (staging A through shared memory
@@ -34,7 +37,14 @@
 namespace sk {
 
 constexpr int kSmemColsPerWarp = 64;
-constexpr int kSmemMaxBucket = 32767;  // 15-bit bucket field; index d is the CTA's dummy row
+constexpr int kSmemMaxBucket = 2047;   // 11-bit bucket field; index d is the CTA's dummy row
+constexpr int kSmemDepth = 1;          // D: sub-steps whose LDS is issued ahead of the running read-modify-write
+                                       // (measured on B200, c5: D = 0 3.62 ms, D = 1 3.47, D = 2 3.54, D = 3 3.53, D = 4 3.58)
+constexpr int kSmemFlagDepth = 1;      // the reload flags cover this many earlier sub-steps (>= D)
+constexpr int kSmemHaloRows = 4;       // rows a hash-pack warp recomputes in front of its 28 output rows
+// 16-bit entry: bucket | reload<<14 | sign<<15
+constexpr uint32_t kE16Bucket = 0x07FFu;
+constexpr uint32_t kE16Reload = 0x4000u;
 
 template <int ZETA>
 struct SmemGeom {
@@ -49,19 +59,57 @@ constexpr int smem_rows_per_step(int zeta) { return zeta >= 4 ? 4 : zeta; }
 constexpr int smem_batch_steps(int zeta, bool small_cta) { return small_cta ? 8 : 2; }
 
 // ------------------------------------------------------------------------------------------------
-// a1 (precomputed form): entry (row, t) = hash of block (row mod R + t) mod ZETA.  One thread per entry.
+// a1 (precomputed form).  Entry (row, t) describes block j = (row mod R + t) mod ZETA of that row:
+//   bucket | reload<<14 | sign<<15.
+// Sub-steps are numbered u = (row / R) * ZETA + t.  `reload` is set when one of the D sub-steps before u
+// updates the same sketch row: sub-step u-k touches block j through row-slot (row mod R + k) mod ZETA (if
+// that is < R) of step floor((u-k)/ZETA).  The scatter kernel issues the LDS of sub-step u before the
+// stores of sub-steps u-D .. u-1 and repeats it after them only where `reload` is set.
+// One lane per row (ZETA hashes each); a warp covers 32 consecutive rows of which the first 4 are a halo
+// (recomputed, not written) so that every partner entry is one shuffle away.
 // ------------------------------------------------------------------------------------------------
 template <int ZETA>
 __global__ void k_hash_pack_rot(uint64_t seed, int64_t rows, uint32_t db, uint16_t* __restrict__ packed) {
-  constexpr int R = SmemGeom<ZETA>::R;
-  const int64_t total = rows * ZETA;
-  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += stride) {
-    const uint64_t row = (uint64_t)idx / ZETA;
-    const uint32_t t = (uint32_t)((uint64_t)idx % ZETA);
-    const uint32_t j = ((uint32_t)(row % R) + t) % ZETA;
-    const uint32_t e = hash_entry(seed, row * ZETA + j, j, db);
-    packed[idx] = (uint16_t)(entry_bucket(e) | ((e >> 31) << 15));
+  constexpr int R = SmemGeom<ZETA>::R, D = kSmemFlagDepth, H = kSmemHaloRows, OUT = 32 - H;
+  static_assert(H % R == 0 && H >= R * ((D + ZETA - 1) / ZETA), "halo covers D sub-steps");
+  const uint32_t lane = threadIdx.x & 31;
+  const int64_t warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+  const int64_t chunks = (rows + OUT - 1) / OUT;
+  for (int64_t c = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; c < chunks; c += warps) {
+    const int64_t row = c * OUT - H + lane;  // OUT and H are multiples of R: row mod R == lane mod R
+    const uint32_t r = lane % R;
+    uint32_t b[ZETA];  // canonical entries of this row, by block
+#pragma unroll
+    for (int j = 0; j < ZETA; ++j) b[j] = row >= 0 ? hash_entry(seed, (uint64_t)row * ZETA + j, j, db) : 0x7FFFFFFFu;
+    uint32_t e[ZETA];  // by sub-step: e[t] = b[(r + t) mod ZETA]
+#pragma unroll
+    for (int t = 0; t < ZETA; ++t) {
+      e[t] = b[t];
+#pragma unroll
+      for (int rr = 1; rr < R; ++rr) e[t] = (r == (uint32_t)rr) ? b[(rr + t) % ZETA] : e[t];
+    }
+    uint32_t out[ZETA];
+#pragma unroll
+    for (int t = 0; t < ZETA; ++t) {
+      bool reload = false;
+#pragma unroll
+      for (int k = 1; k <= D; ++k) {
+        const int ds = (t - k >= 0) ? 0 : -((k - t + ZETA - 1) / ZETA);  // step of sub-step u-k relative to this one
+        const int tk = ((t - k) % ZETA + ZETA) % ZETA;
+        const uint32_t rk = (r + k) % ZETA;                                // its row slot for this block
+        const int src = (int)lane + ds * R + (int)rk - (int)r;
+        const uint32_t pe = __shfl_sync(0xFFFFFFFFu, e[tk], src & 31);
+        reload |= (rk < (uint32_t)R) && (src >= 0) && (entry_bucket(pe) == entry_bucket(e[t]));
+      }
+      out[t] = entry_bucket(e[t]) | (reload ? kE16Reload : 0u) | ((e[t] >> 31) << 15);
+    }
+    if (lane >= (uint32_t)H && row < rows) {
+      uint16_t* dst = packed + row * ZETA;
+      if constexpr (ZETA == 1) dst[0] = (uint16_t)out[0];
+      else if constexpr (ZETA == 2) *reinterpret_cast<uint32_t*>(dst) = out[0] | (out[1] << 16);
+      else if constexpr (ZETA == 4) *reinterpret_cast<uint2*>(dst) = make_uint2(out[0] | (out[1] << 16), out[2] | (out[3] << 16));
+      else *reinterpret_cast<uint4*>(dst) = make_uint4(out[0] | (out[1] << 16), out[2] | (out[3] << 16), out[4] | (out[5] << 16), out[6] | (out[7] << 16));
+    }
   }
 }
 
@@ -97,6 +145,18 @@ SK_DEVINL void sts_h2(uint32_t addr, const uint32_t (&v)[H2]) {
   else if constexpr (H2 == 2) asm volatile("st.shared.v2.b32 [%0], {%1,%2};" ::"r"(addr), "r"(v[0]), "r"(v[1]) : "memory");
   else asm volatile("st.shared.b32 [%0], %1;" ::"r"(addr), "r"(v[0]) : "memory");
 }
+// the same load again, executed only by lanes whose `flag` is non-zero (registers keep their value elsewhere)
+template <int H2>
+SK_DEVINL void lds_h2_if(uint32_t flag, uint32_t addr, uint32_t (&v)[H2]) {
+  if constexpr (H2 == 4)
+    asm volatile("{ .reg .pred p; setp.ne.b32 p, %5, 0; @p ld.shared.v4.b32 {%0,%1,%2,%3}, [%4]; }"
+                 : "+r"(v[0]), "+r"(v[1]), "+r"(v[2]), "+r"(v[3]) : "r"(addr), "r"(flag) : "memory");
+  else if constexpr (H2 == 2)
+    asm volatile("{ .reg .pred p; setp.ne.b32 p, %3, 0; @p ld.shared.v2.b32 {%0,%1}, [%2]; }"
+                 : "+r"(v[0]), "+r"(v[1]) : "r"(addr), "r"(flag) : "memory");
+  else
+    asm volatile("{ .reg .pred p; setp.ne.b32 p, %2, 0; @p ld.shared.b32 %0, [%1]; }" : "+r"(v[0]) : "r"(addr), "r"(flag) : "memory");
+}
 // acc = q * mult + acc per FP16 half, one rounding, subnormals kept
 SK_DEVINL uint32_t hfma2_bits(uint32_t q, uint32_t mult, uint32_t acc) {
   uint32_t d;
@@ -115,7 +175,7 @@ struct SmemWorkSet {  // the K steps being scattered: RN16(s*a) pairs and masked
   uint32_t e[K][EntRow<ZETA>::W];
 };
 
-template <int ZETA, int K, int MAXW>
+template <int ZETA, int K, int MAXW, int DEPTH = kSmemDepth>
 __global__ void __launch_bounds__(MAXW * 32) k_smem(SmemArgs g) {
   using G = SmemGeom<ZETA>;
   constexpr int R = G::R, LPR = G::LPR, VEC = G::VEC, H2 = G::H2, EW = EntRow<ZETA>::W;
@@ -174,29 +234,33 @@ __global__ void __launch_bounds__(MAXW * 32) k_smem(SmemArgs g) {
         for (int w = 0; w < EW; ++w) W.e[s][w] = valid ? L.e[s][w] : dummy_word;
       }
     };
-    // a5: zeta sub-steps per step; sub-step t of row r updates block (r + t) mod zeta
+    // a5: the batch is U = K * zeta sub-steps; sub-step u = (step s, t) of row-slot r updates block (r + t) mod zeta.
+    // Software pipeline of depth D: the LDS of sub-step u is issued before the HFMA2/STS of sub-steps u-D .. u-1
+    // and repeated after them by the lanes whose entry says one of those wrote the same sketch row.
     auto scatter_batch = [&]() -> uint32_t {
+      constexpr int U = K * ZETA, D = DEPTH;
+      static_assert(D <= kSmemFlagDepth, "reload flags must cover the pipeline depth");
+      uint32_t acc[D + 1][H2];
       uint32_t last = 0;
+      auto entry = [&](int u) -> uint32_t {  // 16-bit entry of sub-step u in the low half
+        const uint32_t w = W.e[u / ZETA][(u % ZETA) >> 1];
+        return ((u % ZETA) & 1) ? (w >> 16) : (w & 0xFFFFu);
+      };
 #pragma unroll
-      for (int s = 0; s < K; ++s) {
-        uint32_t addr[ZETA], mult[ZETA];
-#pragma unroll
-        for (int t = 0; t < ZETA; ++t) {
-          const uint32_t w = W.e[s][t >> 1];
-          const uint32_t bucket = (t & 1) ? ((w >> 16) & 0x7FFFu) : (w & 0x7FFFu);
-          addr[t] = bucket * pitch + lane_base;
+      for (int u = 0; u < U + D; ++u) {
+        if (u < U) lds_h2<H2>((entry(u) & kE16Bucket) * pitch + lane_base, acc[u % (D + 1)]);
+        const int v = u - D;
+        if (v >= 0) {
+          const uint32_t ev = entry(v);
+          const uint32_t addr = (ev & kE16Bucket) * pitch + lane_base;
           // sign bit of the entry replicated into both halves, XOR +1.0: +-1.0 in both halves
-          mult[t] = (__byte_perm(w, 0, (t & 1) ? 0x3232 : 0x1010) & 0x80008000u) ^ 0x3C003C00u;
-        }
+          const uint32_t mult = (((ev & 0x8000u) * 0x10001u)) ^ 0x3C003C00u;
+          lds_h2_if<H2>(ev & kE16Reload, addr, acc[v % (D + 1)]);
 #pragma unroll
-        for (int t = 0; t < ZETA; ++t) {
-          uint32_t acc[H2];
-          lds_h2<H2>(addr[t], acc);
-#pragma unroll
-          for (int k = 0; k < H2; ++k) acc[k] = hfma2_bits(W.q[s][k], mult[t], acc[k]);
-          sts_h2<H2>(addr[t], acc);
-          if (R > 1) __syncwarp();  // the next sub-step of another row may read this word
-          last = acc[0];
+          for (int k = 0; k < H2; ++k) acc[v % (D + 1)][k] = hfma2_bits(W.q[v / ZETA][k], mult, acc[v % (D + 1)][k]);
+          sts_h2<H2>(addr, acc[v % (D + 1)]);
+          __syncwarp();  // a later sub-step of another lane may read this word
+          last = acc[v % (D + 1)][0];
         }
       }
       return last & g.zero;

@@ -253,7 +253,7 @@ int ensure_packed(sketch* s, cudaStream_t st, bool force) {
   const int64_t total = s->m * (int64_t)s->zeta;
   rc = ensure_scratch(&s->packed, &s->packed_bytes, (size_t)total * (rot ? 2 : 4));
   if (rc) return rc;
-  int64_t blocks = (total + 255) / 256;
+  int64_t blocks = rot ? (s->m / 28 + 1 + 7) / 8 : (total + 255) / 256;  // rot: one warp per 28 rows, 8 warps per block
   int64_t cap = (int64_t)s->sm_count * 16;
   int grid = (int)(blocks < cap ? blocks : cap);
   if (grid < 1) grid = 1;
