@@ -32,13 +32,20 @@ WORKLOADS = {
     "c2": (1 << 20, 64, 128, 4, 1),
     "c3": (1 << 22, 128, 256, 4, 2),
     "c4": (1 << 23, 256, 1024, 4, 3),
+    "c4-512": (1 << 23, 256, 512, 4, 3),
+    "c4-2048": (1 << 23, 256, 2048, 4, 3),
+    "c3-z1": (1 << 22, 128, 256, 1, 2),
+    "c3-z2": (1 << 22, 128, 256, 2, 2),
+    "c3-z8": (1 << 22, 128, 256, 8, 2),
     "c5": (1 << 25, 128, 256, 4, 4),
 }
 VARIANTS = {"auto": 0, "flat_pair": 1, "flat_vec": 2, "smem": 3, "generic": 4}
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` captures (profiles/*.md name the commands); None until captured.
-NCU_TRAFFIC_BYTES = {}
+# `ncu --set full` captures (profiles/*.md name the commands); None where not captured.
+NCU_TRAFFIC_BYTES = {
+    ("c5", "smem"): 17448558000 + 5222656,   # profiles/r01_smem_c5.md: 17.449 GB read (A 17.180 + packed hashes 0.268) + 5 MB written
+}
 
 
 def measured_peaks():
@@ -190,6 +197,7 @@ def run_ours(args):
 
     import paper_2606_20195_b200 as ss
     import workloads as wl
+    from paper_2606_20195_b200.sharding import all_reduce_sketch, shard_rows
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -207,7 +215,8 @@ def run_ours(args):
     dev = torch.device("cuda", local)
     seed = wl.sketch_seed(0)
     sk = ss.Sketch(m * world, d, zeta, seed)   # one map over all shards; rank r owns rows [r*m, (r+1)*m)
-    row_begin = rank * m
+    row_begin, shard = shard_rows(m * world, world, rank)
+    assert shard == m
     A = wl.gaussian_device(m, n, mseed + 7919 * rank, dev)
     out16 = torch.empty((d, n), dtype=torch.float16, device=dev)
     out32 = torch.empty((d, n), dtype=torch.float32, device=dev)
@@ -222,7 +231,7 @@ def run_ours(args):
     def apply16():
         sk.apply_f16acc(A, out=out16, variant=vid, row_begin=row_begin, rows=m, replicas=args.replicas, hash_mode=args.hash_mode)
         if dist is not None:
-            dist.all_reduce(out16)
+            all_reduce_sketch(out16, dist)
 
     def step16():
         # complete sketch ("initialization, map generation, and application"): when the scatter
@@ -234,7 +243,7 @@ def run_ours(args):
     def step32():
         sk.apply_f32acc(A, out=out32, row_begin=row_begin, rows=m)
         if dist is not None:
-            dist.all_reduce(out32)
+            all_reduce_sketch(out32, dist)
 
     def barrier():
         torch.cuda.synchronize()

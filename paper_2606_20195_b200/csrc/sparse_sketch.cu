@@ -145,7 +145,10 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
 
   int v = want;
   if (v == SKETCH_VARIANT_AUTO) {
-    if (sm_ok) v = SKETCH_VARIANT_SMEM;
+    // measured on B200 (profiles/r01_variant_sweep.md): with one contribution per element (zeta = 1) the
+    // 16-byte REDs of the flat kernel stay under the L2 atomic rate and beat the privatised kernel, whose
+    // one-row steps are issue-bound; from zeta = 2 on the privatised kernel wins wherever it fits
+    if (sm_ok && s->zeta >= 2) v = SKETCH_VARIANT_SMEM;
     else if (zt && vmax) v = SKETCH_VARIANT_FLAT_VEC;
     else v = SKETCH_VARIANT_GENERIC;
   }
@@ -191,10 +194,12 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
   }
   int P = (o && o->replicas > 0) ? o->replicas : 0;
   if (P == 0) {
-    // auto: enough partial sketches to spread same-line RED traffic over L2, capped at 16 MiB of scratch
+    // auto: enough partial sketches to spread same-line RED traffic over L2, capped at 16 MiB of scratch;
+    // launch-bound inputs (c1: 12.3 us with P = 1 vs 13.6 us with the fold kernel) RED straight into B
     size_t one = (size_t)s->d * n * (f16 ? 2 : 4);
     size_t cap = (16u << 20) / (one ? one : 1);
     P = (int)(cap < 1 ? 1 : cap > 8 ? 8 : cap);
+    if (rows * (int64_t)n <= (1 << 20)) P = 1;
   }
   if (P > 4096) P = 4096;
   p->replicas = P;
@@ -401,18 +406,25 @@ int apply_host(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void*
     }
     s->stage_bytes = chunk_bytes;
   }
-  rc = ensure_scratch(&s->bdev, &s->bdev_bytes, out_bytes);
+  // one partial sketch per row chunk (slot k mod kSlots), folded once at the end: the chunk level of the
+  // accumulation hierarchy.  Adding every chunk into ONE FP16 sketch would put #chunks x #CTAs partial sums
+  // on a single running sum (measured at c5: relF 2.5e-2 instead of 7e-3).
+  const int64_t nchunks = rows > 0 ? (rows + chunk_rows - 1) / chunk_rows : 0;
+  const int64_t kSlots = nchunks < 64 ? (nchunks > 0 ? nchunks : 1) : 64;
+  rc = ensure_scratch(&s->bdev, &s->bdev_bytes, out_bytes * (size_t)(kSlots + 1));
   if (rc) return rc;
+  char* const slots = static_cast<char*>(s->bdev);            // [kSlots][d][n]
+  char* const result = slots + out_bytes * (size_t)kSlots;     // [d][n]
   sketch_opts_t oo;
   memset(&oo, 0, sizeof(oo));
   if (o) oo = *o;
   const int user_acc = o ? o->accumulate : 0;
-  if (user_acc) CU_TRY(cudaMemcpyAsync(s->bdev, B, out_bytes, cudaMemcpyHostToDevice, s->st_comp));
-  else if (rows == 0) CU_TRY(cudaMemsetAsync(s->bdev, 0, out_bytes, s->st_comp));
-  int k = 0;
+  if (user_acc) CU_TRY(cudaMemcpyAsync(result, B, out_bytes, cudaMemcpyHostToDevice, s->st_comp));
+  if (nchunks == 0) CU_TRY(cudaMemsetAsync(slots, 0, out_bytes, s->st_comp));
+  int64_t k = 0;
   for (int64_t r0 = 0; r0 < rows; r0 += chunk_rows, ++k) {
     int64_t nr = rows - r0 < chunk_rows ? rows - r0 : chunk_rows;
-    int b = k & 1;
+    int b = (int)(k & 1);
     if (k >= 2) CU_TRY(cudaStreamWaitEvent(s->st_copy, s->ev_done[b], 0));
     const float* src = A + r0 * lda;
     if (lda == n) CU_TRY(cudaMemcpyAsync(s->stage[b], src, (size_t)nr * row_bytes, cudaMemcpyHostToDevice, s->st_copy));
@@ -421,12 +433,22 @@ int apply_host(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void*
     CU_TRY(cudaStreamWaitEvent(s->st_comp, s->ev_copied[b], 0));
     oo.row_begin = rb + r0;
     oo.rows = nr;
-    oo.accumulate = (k > 0 || user_acc) ? 1 : 0;
-    rc = apply_device(s, (const float*)s->stage[b], n, n, s->bdev, f16, rounding, sr_seed, &oo, s->st_comp);
+    oo.accumulate = k >= kSlots ? 1 : 0;
+    rc = apply_device(s, (const float*)s->stage[b], n, n, slots + out_bytes * (size_t)(k % kSlots), f16, rounding, sr_seed, &oo,
+                      s->st_comp);
     if (rc) return rc;
     CU_TRY(cudaEventRecord(s->ev_done[b], s->st_comp));
   }
-  CU_TRY(cudaMemcpyAsync(B, s->bdev, out_bytes, cudaMemcpyDeviceToHost, s->st_comp));
+  {
+    const int64_t count = (int64_t)s->d * n;
+    int grid = (int)((count + 255) / 256);
+    if (grid > s->sm_count * 8) grid = s->sm_count * 8;
+    if (f16) sk::k_reduce_replicas<true><<<grid, 256, 0, s->st_comp>>>(slots, count, (int)kSlots, result, count, user_acc);
+    else sk::k_reduce_replicas<false><<<grid, 256, 0, s->st_comp>>>(slots, count, (int)kSlots, result, count, user_acc);
+    rc = launch_check("k_reduce_replicas (chunks)");
+    if (rc) return rc;
+  }
+  CU_TRY(cudaMemcpyAsync(B, result, out_bytes, cudaMemcpyDeviceToHost, s->st_comp));
   CU_TRY(cudaStreamSynchronize(s->st_comp));
   return SKETCH_OK;
 }
