@@ -39,7 +39,7 @@ WORKLOADS = {
     "c3-z8": (1 << 22, 128, 256, 8, 2),
     "c5": (1 << 25, 128, 256, 4, 4),
 }
-VARIANTS = {"auto": 0, "flat_pair": 1, "flat_vec": 2, "smem": 3, "generic": 4}
+VARIANTS = {"auto": 0, "flat_pair": 1, "flat_vec": 2, "smem": 3, "generic": 4, "tmem": 5}
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/*.md name the commands); None where not captured.

@@ -58,6 +58,10 @@ typedef struct sketch sketch_t; /* opaque, library-owned */
 #define SKETCH_VARIANT_FLAT_VEC 2  /* widest vector RED the shape allows (16-byte REDG: 8 halves / 4 floats) */
 #define SKETCH_VARIANT_SMEM 3      /* shared-memory-privatised partial sketch per CTA, flushed with vector RED */
 #define SKETCH_VARIANT_GENERIC 4   /* any n / any alignment scalar fallback (one lane per element) */
+#define SKETCH_VARIANT_TMEM 5      /* tensor-memory-privatised partial sketch per warp (tcgen05.ld / tcgen05.st read-
+                                      modify-write), A staged by TMA, hashes computed on the fly by a producer
+                                      warp; FP16-RN, zeta in {1,2,4,8}, n = 64*X*S with X, S in {1,2,4} and
+                                      d*X <= 512, lda % 4 == 0, A and B 16-byte aligned */
 
 typedef struct sketch_opts {
   int32_t variant;    /* SKETCH_VARIANT_* */

@@ -12,6 +12,7 @@ from .binding import (  # noqa: F401
     VARIANT_FLAT_VEC,
     VARIANT_GENERIC,
     VARIANT_SMEM,
+    VARIANT_TMEM,
     VARIANT_NAMES,
     Sketch,
     SketchError,

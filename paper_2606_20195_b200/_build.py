@@ -13,8 +13,11 @@ HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 OBJ = HERE / "_obj"
 LIB = HERE / "libsparse_sketch.so"
-SOURCES = [CSRC / n for n in ("sparse_sketch.cu", "launch_flat_f16.cu", "launch_flat_f32.cu", "launch_smem.cu")]
-HEADERS = [CSRC / n for n in ("args.h", "launch.h", "device_util.cuh", "kernel_flat.cuh", "kernel_misc.cuh", "kernel_smem.cuh")]
+SOURCES = [CSRC / n for n in ("sparse_sketch.cu", "launch_flat_f16.cu", "launch_flat_f32.cu", "launch_smem.cu", "launch_tmem.cu")]
+HEADERS = [CSRC / n for n in ("args.h", "launch.h", "device_util.cuh", "kernel_flat.cuh", "kernel_misc.cuh", "kernel_smem.cuh", "kernel_tmem.cuh")]
+# (source, object stem, extra flags): launch_tmem.cu is compiled once per zeta family
+UNITS = [(src, src.stem, []) for src in SOURCES if src.name != "launch_tmem.cu"]
+UNITS += [(CSRC / "launch_tmem.cu", "launch_tmem_z%d" % z, ["-DSK_TMEM_ZETA=%d" % z]) for z in (1, 2, 4, 8)]
 HEADERS.append(HERE.parent / "include" / "sparse_sketch.h")
 
 NVCC_FLAGS = [
@@ -36,11 +39,12 @@ def _stale(target: Path, deps) -> bool:
     return any(p.stat().st_mtime > t for p in deps)
 
 
-def _compile(src: Path, force: bool) -> Path:
-    obj = OBJ / (src.stem + ".o")
+def _compile(unit, force: bool) -> Path:
+    src, stem, extra = unit
+    obj = OBJ / (stem + ".o")
     if force or _stale(obj, [src] + HEADERS):
-        res = subprocess.run([_nvcc()] + NVCC_FLAGS + ["-c", str(src), "-o", str(obj)], capture_output=True, text=True)
-        (OBJ / (src.stem + ".ptxas.log")).write_text(res.stderr)
+        res = subprocess.run([_nvcc()] + NVCC_FLAGS + extra + ["-c", str(src), "-o", str(obj)], capture_output=True, text=True)
+        (OBJ / (stem + ".ptxas.log")).write_text(res.stderr)
         if res.returncode != 0:
             sys.stderr.write(res.stdout + res.stderr)
             raise RuntimeError("nvcc failed on %s" % src.name)
@@ -51,8 +55,8 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     OBJ.mkdir(exist_ok=True)
     if not force and not _stale(LIB, SOURCES + HEADERS):
         return LIB
-    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
-        objs = list(ex.map(lambda s: _compile(s, force), SOURCES))
+    with ThreadPoolExecutor(max_workers=len(UNITS)) as ex:
+        objs = list(ex.map(lambda u: _compile(u, force), UNITS))
     tmp = LIB.with_suffix(".so.tmp%d" % os.getpid())
     res = subprocess.run([_nvcc(), "-shared", "-o", str(tmp)] + [str(o) for o in objs], capture_output=True, text=True)
     if res.returncode != 0:
@@ -60,8 +64,8 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         raise RuntimeError("link of libsparse_sketch.so failed")
     os.replace(tmp, LIB)
     if verbose:
-        for s in SOURCES:
-            sys.stderr.write((OBJ / (s.stem + ".ptxas.log")).read_text())
+        for _, stem, _ in UNITS:
+            sys.stderr.write((OBJ / (stem + ".ptxas.log")).read_text())
     return LIB
 
 

@@ -31,6 +31,11 @@ struct SmemArgs {
   uint32_t zero;  // always 0; the kernel uses it to build a scheduling dependency ptxas cannot fold away
 };
 
+struct TmemArgs {
+  ScatterArgs s;  // packed unused (the producer warp hashes on the fly); lda % 4 == 0, A and B 16-byte aligned
+  int32_t d;
+};
+
 constexpr int kFlatThreads = 256;
 
 }  // namespace sk

@@ -22,4 +22,15 @@ cudaError_t launch_hash_pack_rot(uint64_t seed, int zeta, int64_t rows, uint32_t
                                  cudaStream_t st);
 int smem_max_bucket();
 
+// tensor-memory-privatised FP16-RN scatter (kernel_tmem.cuh); n = 64 * X * S.  tmem_shape picks (X, S) for a
+// shape, returns false when the sketch does not fit the 512 TMEM columns of a warp's lane quadrant.
+bool tmem_shape(int n, int d, int* X, int* S);
+size_t tmem_smem_bytes_for(int zeta, int n);
+int tmem_rows_per_stage(int n);
+cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, int grid, cudaStream_t st);
+cudaError_t launch_tmem_z1(const TmemArgs& g, int X, int S, int grid, cudaStream_t st);
+cudaError_t launch_tmem_z2(const TmemArgs& g, int X, int S, int grid, cudaStream_t st);
+cudaError_t launch_tmem_z4(const TmemArgs& g, int X, int S, int grid, cudaStream_t st);
+cudaError_t launch_tmem_z8(const TmemArgs& g, int X, int S, int grid, cudaStream_t st);
+
 }  // namespace sk

@@ -110,6 +110,14 @@ bool smem_feasible(const sketch* s, int n, int64_t lda, const void* A, const voi
   return true;
 }
 
+bool tmem_feasible(const sketch* s, int n, int64_t lda, const void* A, const void* B) {
+  if (!zeta_templated(s->zeta)) return false;
+  int X = 0, S = 0;
+  if (!sk::tmem_shape(n, s->d, &X, &S)) return false;
+  if (lda % 4 != 0 || !aligned(A, 16) || !aligned(B, 16)) return false;  // TMA bulk copies: 16-byte granules
+  return sk::tmem_smem_bytes_for(s->zeta, n) <= (size_t)s->smem_optin;
+}
+
 int flat_vec_for(bool f16, int n, int64_t lda, const void* A, const void* B, int want_max) {
   const int cands_h[3] = {8, 4, 2};
   const int cands_f[4] = {4, 2, 1, 0};  // FP32: one 16-byte RED per lane is the widest single transaction
@@ -130,7 +138,7 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
   if (rc) return rc;
   memset(p, 0, sizeof(*p));
   int want = o ? o->variant : SKETCH_VARIANT_AUTO;
-  if (want < 0 || want > SKETCH_VARIANT_GENERIC) return SKETCH_ERR_INVALID;
+  if (want < 0 || want > SKETCH_VARIANT_TMEM) return SKETCH_ERR_INVALID;
   p->hash_mode = (o && o->hash_mode) ? o->hash_mode : 1;
   if (p->hash_mode != 1 && p->hash_mode != 2) return SKETCH_ERR_INVALID;
   size_t sm_bytes = 0;
@@ -139,6 +147,7 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
   const int64_t rb0 = o ? o->row_begin : 0;
   bool sm_ok = f16 && rounding == SKETCH_RN && smem_feasible(s, n, lda, A, B, &sm_bytes) &&
                (rb0 % sk::smem_step_rows(s->zeta) == 0);
+  bool tm_ok = f16 && rounding == SKETCH_RN && tmem_feasible(s, n, lda, A, B);
   int vmax = flat_vec_for(f16, n, lda, A, B, 8);
   int vpair = flat_vec_for(f16, n, lda, A, B, f16 ? 2 : 1);
   bool zt = zeta_templated(s->zeta);
@@ -148,15 +157,32 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
     // measured on B200 (profiles/r01_variant_sweep.md): with one contribution per element (zeta = 1) the
     // 16-byte REDs of the flat kernel stay under the L2 atomic rate and beat the privatised kernel, whose
     // one-row steps are issue-bound; from zeta = 2 on the privatised kernel wins wherever it fits
-    if (sm_ok && s->zeta >= 2) v = SKETCH_VARIANT_SMEM;
+    // the tensor-memory kernel (profiles/r01_tmem_*.md) beats both wherever it fits; below ~4 MiB of A the
+    // launch is latency-bound and the lighter kernels win
+    if (tm_ok && rows * (int64_t)n > (1 << 20)) v = SKETCH_VARIANT_TMEM;
+    else if (sm_ok && s->zeta >= 2) v = SKETCH_VARIANT_SMEM;
     else if (zt && vmax) v = SKETCH_VARIANT_FLAT_VEC;
     else v = SKETCH_VARIANT_GENERIC;
   }
   if (v == SKETCH_VARIANT_SMEM && !sm_ok) return SKETCH_ERR_UNSUPPORTED;
+  if (v == SKETCH_VARIANT_TMEM && !tm_ok) return SKETCH_ERR_UNSUPPORTED;
   if (v == SKETCH_VARIANT_FLAT_VEC && !(zt && vmax)) return SKETCH_ERR_UNSUPPORTED;
   if (v == SKETCH_VARIANT_FLAT_PAIR && !(zt && vpair)) return SKETCH_ERR_UNSUPPORTED;
   p->variant = v;
   p->zeta_t = s->zeta;
+
+  if (v == SKETCH_VARIANT_TMEM) {
+    p->hash_mode = 1;  // the producer warp hashes on the fly
+    p->replicas = 1;
+    p->wpc = 5;
+    p->smem_bytes = sk::tmem_smem_bytes_for(s->zeta, n);
+    int64_t stages = (rows + sk::tmem_rows_per_stage(n) - 1) / sk::tmem_rows_per_stage(n);
+    int64_t grid = stages < s->sm_count ? stages : s->sm_count;  // one CTA per SM: it owns all 512 TMEM columns
+    if (o && o->grid_ctas > 0) grid = o->grid_ctas;
+    if (grid < 1) grid = 1;
+    p->grid = (int)grid;
+    return SKETCH_OK;
+  }
 
   if (v == SKETCH_VARIANT_SMEM) {
     p->hash_mode = 2;  // always the precomputed entries
@@ -305,6 +331,18 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
   const int accumulate = o ? o->accumulate : 0;
   const size_t elem = f16 ? 2 : 4;
   const size_t out_bytes = (size_t)s->d * n * elem;
+
+  if (p.variant == SKETCH_VARIANT_TMEM) {
+    if (!accumulate) CU_TRY(cudaMemsetAsync(B, 0, out_bytes, st));  // a0
+    if (rows > 0) {
+      sk::TmemArgs g;
+      g.s = make_args(s, A, n, lda, B, row_begin, rows, sr_seed, 1);
+      g.d = s->d;
+      rc = launched(sk::launch_tmem_f16(g, s->zeta, p.grid, st), "k_tmem");
+      if (rc) return rc;
+    }
+    return SKETCH_OK;
+  }
 
   if (p.variant == SKETCH_VARIANT_SMEM) {
     if (!accumulate) CU_TRY(cudaMemsetAsync(B, 0, out_bytes, st));  // a0

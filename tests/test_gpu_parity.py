@@ -37,9 +37,9 @@ def bits(t):
     return b
 
 
-F16_VARIANTS = ["auto", "flat_pair", "flat_vec", "smem", "generic"]
+F16_VARIANTS = ["auto", "flat_pair", "flat_vec", "smem", "tmem", "generic"]
 F32_VARIANTS = ["auto", "flat_pair", "flat_vec", "generic"]
-VID = {"auto": 0, "flat_pair": 1, "flat_vec": 2, "smem": 3, "generic": 4}
+VID = {"auto": 0, "flat_pair": 1, "flat_vec": 2, "smem": 3, "generic": 4, "tmem": 5}
 
 
 def apply16(ss, sk, A, variant="auto", **kw):
@@ -275,10 +275,11 @@ def test_row_ranges_accumulate_and_lda(ss, variant):
     assert np.array_equal(oracle.half_bits_to_f64(bits(out)), want)
     if variant == "auto":   # auto falls back to the flat kernel for a range that starts off the 4-row grid
         assert sk.plan(n, row_begin=37, rows=100)["variant"] == "flat_vec" and sk.plan(n, row_begin=36, rows=100)["variant"] == "smem"
+        assert sk.plan(n)["variant"] == "tmem"          # large enough ranges go to tensor memory, any row_begin
     out32 = None
     for k, (r0, r1) in enumerate(((0, 37), (37, 12001), (12001, m))):
         out32 = sk.apply_f32acc(Ap[r0:r1, :n], out=out32, row_begin=r0, accumulate=k > 0,
-                                variant=VID[variant] if variant != "smem" else 0)
+                                variant=VID[variant] if variant not in ("smem", "tmem") else 0)
     assert np.array_equal(out32.cpu().numpy().astype(np.float64), want)
 
 
@@ -341,9 +342,10 @@ def test_replica_counts_and_grids(ss):
         for grid in (0, 1, 5, 333):
             got = sk.apply_f16acc(Ad, variant=VID["flat_vec"], replicas=P, grid_ctas=grid)
             assert np.array_equal(oracle.half_bits_to_f64(bits(got)), want), (P, grid)
-    for grid in (1, 3, 148, 1000):
-        got = sk.apply_f16acc(Ad, variant=VID["smem"], grid_ctas=grid)
-        assert np.array_equal(oracle.half_bits_to_f64(bits(got)), want), grid
+    for variant in ("smem", "tmem"):
+        for grid in (1, 3, 148, 1000):
+            got = sk.apply_f16acc(Ad, variant=VID[variant], grid_ctas=grid)
+            assert np.array_equal(oracle.half_bits_to_f64(bits(got)), want), (variant, grid)
 
 
 def test_tiny_and_degenerate_inputs(ss):
@@ -387,7 +389,7 @@ def test_subnormal_scale_is_exact_in_any_order(ss):
     assert np.abs(mag).max() < 2048 and np.count_nonzero(want) > 0.9 * want.size
     sk = ss.Sketch(m, d, zeta, seed)
     want[want == 0x8000] = 0
-    for variant in ("smem", "flat_vec", "flat_pair"):
+    for variant in ("tmem", "smem", "flat_vec", "flat_pair"):
         assert np.array_equal(bits(sk.apply_f16acc(dev(A), variant=VID[variant])), want), variant
 
 
@@ -405,7 +407,7 @@ def test_overflow_saturates_like_the_oracle(ss):
     # the exact sums have std ~ 2^12 * 0.5 * sqrt(2048) = 9.3e4 > 65504: a large share overflows
     assert 0.2 < over_want < 0.95
     B = oracle.f64_sketch(seed, d, zeta, A)
-    for variant, kw in (("smem", {}), ("flat_vec", {"replicas": 1}), ("flat_vec", {"replicas": 8})):
+    for variant, kw in (("tmem", {}), ("smem", {}), ("flat_vec", {"replicas": 1}), ("flat_vec", {"replicas": 8})):
         got = oracle.half_bits_to_f64(bits(sk.apply_f16acc(dev(A), variant=VID[variant], **kw)))
         over = (~np.isfinite(got)).mean()
         assert abs(over - over_want) < 0.3, (variant, over, over_want)
