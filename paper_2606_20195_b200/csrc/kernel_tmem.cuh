@@ -26,8 +26,19 @@
 //               store the chain's final value) -- the bucket is warp-uniform, so this is a select, not
 //               divergence.  tcgen05.wait::st orders a group's LDTMs behind the previous group's STTMs.
 //   flush     : LDTM.x8 -> result-discarding vector REDs into B.
+//
+// Sketches larger than one warp's 512 TMEM columns (d * X > 512) are split two ways:
+//   BQ bucket groups : the zeta stack blocks are cut into BQ groups of ZB = zeta / BQ consecutive blocks
+//               (disjoint sketch-row ranges); a warp of group b holds only the d / BQ sketch
+//               rows of its blocks and adds only those contributions.  Every row is then converted by BQ
+//               warps, which costs shared-memory reads and F2FPs but no tensor-memory capacity.
+//   CS column slices : gridDim.y CTAs share a row range, CTA y takes the features [y * N, (y + 1) * N) of every
+//               row (N = 64 * X * S); its A tile is fetched row by row (N * 4 bytes each), the hashes are
+//               recomputed per slice.  d = 1024, n = 256: X = 2, BQ = 4, CS = 2;  d = 2048: X = 1, BQ = 4, CS = 4.
 // Accumulation is FP16 RN throughout; the hierarchy is (warp-private partial) -> RED into B.
 #pragma once
+
+#include <cuda.h>  // CUtensorMap (type only; the encoder is fetched with cudaGetDriverEntryPoint)
 
 #include "args.h"
 #include "device_util.cuh"
@@ -70,6 +81,13 @@ SK_DEVINL void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t 
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(policy) : "memory");
 }
 
+// TMA tiled copy of a {N features x T rows} box at (column c0, row c1) of the 2-D tensor map; rows and
+// columns outside the tensor are zero-filled and still counted in the transaction bytes
+SK_DEVINL void tensor_g2s(uint32_t dst, const CUtensorMap* tmap, int32_t c0, int32_t c1, uint32_t bar, uint64_t policy) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3}], [%4], %5;"
+               ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(c0), "r"(c1), "r"(bar), "l"(policy) : "memory");
+}
+
 template <int X> SK_DEVINL void tmem_ld(uint32_t taddr, uint32_t (&v)[X]) {
   static_assert(X == 1 || X == 2 || X == 4, "X");
   if constexpr (X == 1) asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(v[0]) : "r"(taddr));
@@ -110,14 +128,20 @@ SK_DEVINL uint32_t hfma2_u32(uint32_t q, uint32_t mult, uint32_t acc) {
 }
 
 // ---------------------------------------------------------------------------------------- geometry
-template <int ZETA, int X, int S, int NW, int T>
+template <int ZETA, int X, int S, int BQ, int NW, int T>
 struct TmemGeom {
-  static_assert(NW % 4 == 0 && NW % S == 0, "consumer warps: whole lane quadrants, whole slice sets");
-  static constexpr int RS = NW / S;            // row-sets per stage
+  static_assert(NW % 4 == 0 && NW % (S * BQ) == 0, "consumer warps: whole lane quadrants, whole slice x bucket-group sets");
+  static_assert(ZETA % BQ == 0, "bucket groups are whole stack blocks");
+  static constexpr int ZB = ZETA / BQ;         // stack blocks one warp accumulates
+  static constexpr int RS = NW / (S * BQ);     // row-sets per stage
   static constexpr int TR = T / RS;            // rows of a stage one warp processes
-  static constexpr int G = ZETA >= 4 ? 2 : 4;  // rows per group (LDTMs in flight = G * ZETA)
+  #ifndef SK_TMEM_G_SMALL
+#define SK_TMEM_G_SMALL 4
+#endif
+  static constexpr int G = (ZB >= 4 || (BQ > 1 && ZB >= 2)) ? 2 : SK_TMEM_G_SMALL;  // rows per group (LDTMs in flight = G * ZB)
   static_assert(TR % G == 0, "whole groups");
-  static constexpr int N = 64 * X * S;         // features
+  static constexpr int N = 64 * X * S;         // features of the CTA's column slice
+  static constexpr int WC = kTmemCols / (NW / 4);  // tensor-memory columns of one warp's private region
   static constexpr int A_BYTES = T * N * 4;
   static constexpr int E_BYTES = T * ZETA * 8;
   static constexpr int STAGE_BYTES = A_BYTES + E_BYTES;
@@ -131,11 +155,11 @@ constexpr size_t tmem_smem_bytes(int zeta, int n) {
 }
 
 // ---------------------------------------------------------------------------------------- the kernel
-template <int ZETA, int X, int S, int NW>
-__global__ void __launch_bounds__((NW + 1) * 32, 1) k_tmem(TmemArgs g) {
+template <int ZETA, int X, int S, int BQ, int NW>
+__global__ void __launch_bounds__((NW + 1) * 32, 1) k_tmem(TmemArgs g, const __grid_constant__ CUtensorMap tmap) {
   constexpr int T = tmem_stage_rows(64 * X * S), NS = tmem_stages(64 * X * S);
-  using Geo = TmemGeom<ZETA, X, S, NW, T>;
-  constexpr int TR = Geo::TR, G = Geo::G, N = Geo::N;
+  using Geo = TmemGeom<ZETA, X, S, BQ, NW, T>;
+  constexpr int TR = Geo::TR, G = Geo::G, N = Geo::N, ZB = Geo::ZB;
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const ScatterArgs& a = g.s;
   const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -163,11 +187,13 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_tmem(TmemArgs g) {
   const uint32_t tbase = *tbase_p;
 
   const int64_t nstages = (a.rows + T - 1) / T;
+  const int64_t col0 = (int64_t)blockIdx.y * N;   // first feature of this CTA's column slice
+  const uint32_t dloc = (uint32_t)g.d / BQ;        // sketch rows one warp holds
 
   if (warp == NW) {
     // ================================================================ producer: TMA + hash stage (a1, a2)
     const uint64_t policy = l2_evict_first_policy();
-    const bool contiguous = (a.lda == N);
+    const bool contiguous = (a.lda == N);          // implies a single column slice
     uint32_t it = 0;
     for (int64_t st = blockIdx.x; st < nstages; st += gridDim.x, ++it) {
       const uint32_t slot = it % NS, ph = (it / NS) & 1;
@@ -176,27 +202,30 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_tmem(TmemArgs g) {
       mbar_wait(empty, ph ^ 1);                // passes at once the first time round the ring
       const int64_t row0 = st * T;
       const int32_t nrows = (int32_t)min((int64_t)T, a.rows - row0);
-      if (lane == 0) mbar_expect_tx(full, (uint32_t)nrows * N * 4);
-      __syncwarp();
       if (contiguous) {
-        if (lane == 0) bulk_g2s(sA, a.A + row0 * a.lda, (uint32_t)nrows * N * 4, full, policy);
-      } else {
-        for (int32_t r = lane; r < nrows; r += 32) bulk_g2s(sA + r * N * 4, a.A + (row0 + r) * a.lda, N * 4, full, policy);
+        if (lane == 0) {
+          mbar_expect_tx(full, (uint32_t)nrows * N * 4);
+          bulk_g2s(sA, a.A + row0 * a.lda, (uint32_t)nrows * N * 4, full, policy);
+        }
+      } else if (lane == 0) {                  // strided rows / column slice: one tiled TMA copy per stage
+        mbar_expect_tx(full, (uint32_t)T * N * 4);
+        tensor_g2s(sA, &tmap, (int32_t)col0, (int32_t)row0, full, policy);
       }
-      if (nrows < T) {                         // last stage of the matrix: rows past the end contribute +0
+      if (contiguous && nrows < T) {           // last stage of the matrix: rows past the end contribute +0
         const uint32_t z0 = sA + nrows * N * 4, z1 = sA + Geo::A_BYTES;
         for (uint32_t p = z0 + lane * 16; p < z1; p += 32 * 16) asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(p), "r"(0u) : "memory");
       }
-      // a1: entries of rows lane, lane + 32, ...: {bucket * X, +-1.0 | +-1.0}
+      // a1: entries of rows lane, lane + 32, ...: {(bucket - first sketch row of the block's group) * X, +-1.0 | +-1.0}
 #pragma unroll
-      for (int rr = 0; rr < T / 32; ++rr) {
+      for (int rr = 0; rr < (T + 31) / 32; ++rr) {
         const int32_t r = rr * 32 + (int32_t)lane;
+        if (T % 32 != 0 && r >= T) break;      // stages of 16 rows (n >= 512): half a warp hashes
         const uint64_t ctr0 = (uint64_t)(a.row_begin + row0 + r) * ZETA;
         uint32_t w[2 * ZETA];
 #pragma unroll
         for (int j = 0; j < ZETA; ++j) {
           const uint32_t e = hash_entry(a.seed, ctr0 + j, j, a.db);
-          w[2 * j] = entry_bucket(e) * X;
+          w[2 * j] = (entry_bucket(e) - (uint32_t)(j / ZB) * dloc) * X;
           w[2 * j + 1] = 0x3C003C00u ^ entry_signmask_h2(e);
         }
         const uint32_t p = sE + r * (ZETA * 8);
@@ -212,15 +241,15 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_tmem(TmemArgs g) {
     }
   } else {
     // ================================================================ consumers: a3, a4, a5 in tensor memory
-    const uint32_t slice = warp % S, rowset = warp / S;
-    const uint32_t region = tbase + (((warp & 3u) * 32u) << 16) + (warp >> 2) * (uint32_t)(g.d * X);
-    const uint32_t ncols = (uint32_t)g.d * X;  // multiple of 8 (host check)
+    const uint32_t slice = warp % S, bgrp = (warp / S) % BQ, rowset = warp / (S * BQ);
+    const uint32_t region = tbase + (((warp & 3u) * 32u) << 16) + (warp >> 2) * (uint32_t)Geo::WC;
+    const uint32_t ncols = dloc * X;  // multiple of 8, <= WC (host check)
     for (uint32_t c = 0; c < ncols; c += 8) tmem_st8_zero(region + c);   // a0 (private part)
     tmem_wait_st();
 
     const float scale = a.scale;
     const uint32_t a_off = (rowset * TR) * (N * 4) + (slice * 64 * X + lane * 2 * X) * 4;
-    const uint32_t e_off = (rowset * TR) * (ZETA * 8);
+    const uint32_t e_off = (rowset * TR) * (ZETA * 8) + bgrp * (ZB * 8);
     uint32_t it = 0;
     for (int64_t st = blockIdx.x; st < nstages; st += gridDim.x, ++it) {
       const uint32_t slot = it % NS, ph = (it / NS) & 1;
@@ -229,7 +258,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_tmem(TmemArgs g) {
       mbar_wait(bars + 8 * slot, ph);
 #pragma unroll
       for (int g0 = 0; g0 < TR; g0 += G) {
-        uint32_t q[G][X], col[G][ZETA], mul[G][ZETA];
+        uint32_t q[G][X], col[G][ZB], mul[G][ZB];
 #pragma unroll
         for (int r = 0; r < G; ++r) {
           // a2 (from the staged tile), a3, a4: q = RN16(s * a), two features per word
@@ -246,31 +275,31 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_tmem(TmemArgs g) {
 #pragma unroll
           for (int k = 0; k < X; ++k) q[r][k] = pack_rn(v[2 * k] * scale, v[2 * k + 1] * scale);
           const unsigned char* pe = sE + (g0 + r) * (ZETA * 8);
-          if constexpr (ZETA == 1) { const uint2 t = *reinterpret_cast<const uint2*>(pe); col[r][0] = t.x; mul[r][0] = t.y; }
+          if constexpr (ZB == 1) { const uint2 t = *reinterpret_cast<const uint2*>(pe); col[r][0] = t.x; mul[r][0] = t.y; }
           else {
 #pragma unroll
-            for (int k = 0; k < ZETA / 2; ++k) {
+            for (int k = 0; k < ZB / 2; ++k) {
               const uint4 t = *reinterpret_cast<const uint4*>(pe + 16 * k);
               col[r][2 * k] = t.x; mul[r][2 * k] = t.y; col[r][2 * k + 1] = t.z; mul[r][2 * k + 1] = t.w;
             }
           }
         }
-        // a5: read-modify-write of G x ZETA sketch rows in tensor memory
-        uint32_t acc[G][ZETA][X];
+        // a5: read-modify-write of G x ZB sketch rows in tensor memory
+        uint32_t acc[G][ZB][X];
         tmem_wait_st();                        // the previous group's stores are in TMEM
 #pragma unroll
         for (int r = 0; r < G; ++r)
 #pragma unroll
-          for (int j = 0; j < ZETA; ++j) tmem_ld<X>(region + col[r][j], acc[r][j]);
+          for (int j = 0; j < ZB; ++j) tmem_ld<X>(region + col[r][j], acc[r][j]);
         tmem_wait_ld();
 #pragma unroll
         for (int r = 0; r < G; ++r)
 #pragma unroll
-          for (int j = 0; j < ZETA; ++j)
+          for (int j = 0; j < ZB; ++j)
 #pragma unroll
             for (int k = 0; k < X; ++k) tmem_tie(acc[r][j][k]);
 #pragma unroll
-        for (int j = 0; j < ZETA; ++j) {
+        for (int j = 0; j < ZB; ++j) {
 #pragma unroll
           for (int r = 0; r < G; ++r) {
             // chain onto the latest earlier row of the group that hit the same sketch row
@@ -304,7 +333,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_tmem(TmemArgs g) {
 
     // ---- flush: private partial sketch -> B with result-discarding vector REDs (a5's last level)
     tmem_wait_st();
-    __half* const Bw = reinterpret_cast<__half*>(a.B) + slice * 64 * X + lane * 2 * X;
+    __half* const Bw = reinterpret_cast<__half*>(a.B) + (size_t)(bgrp * dloc) * a.n + col0 + slice * 64 * X + lane * 2 * X;
     for (uint32_t c = 0; c < ncols; c += 8) {
       uint32_t v[8];
       tmem_ld8(region + c, v);
@@ -313,7 +342,7 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_tmem(TmemArgs g) {
       for (int k = 0; k < 8; ++k) tmem_tie(v[k]);
 #pragma unroll
       for (int b = 0; b < 8 / X; ++b) {
-        __half* dst = Bw + (size_t)(c / X + b) * N;
+        __half* dst = Bw + (size_t)(c / X + b) * a.n;
         if constexpr (X == 1) { if (v[b] != 0u) red_h2(dst, v[b]); }
         else if constexpr (X == 2) { if ((v[2 * b] | v[2 * b + 1]) != 0u) red_h4(dst, v[2 * b], v[2 * b + 1]); }
         else { if ((v[4 * b] | v[4 * b + 1] | v[4 * b + 2] | v[4 * b + 3]) != 0u) red_h8(dst, v[4 * b], v[4 * b + 1], v[4 * b + 2], v[4 * b + 3]); }

@@ -2,6 +2,7 @@
 // Each returns the launch status (cudaGetLastError) or cudaErrorInvalidValue for an unsupported combination.
 #pragma once
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include "args.h"
@@ -22,15 +23,19 @@ cudaError_t launch_hash_pack_rot(uint64_t seed, int zeta, int64_t rows, uint32_t
                                  cudaStream_t st);
 int smem_max_bucket();
 
-// tensor-memory-privatised FP16-RN scatter (kernel_tmem.cuh); n = 64 * X * S.  tmem_shape picks (X, S) for a
-// shape, returns false when the sketch does not fit the 512 TMEM columns of a warp's lane quadrant.
-bool tmem_shape(int n, int d, int* X, int* S);
-size_t tmem_smem_bytes_for(int zeta, int n);
-int tmem_rows_per_stage(int n);
-cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, int grid, cudaStream_t st);
-cudaError_t launch_tmem_z1(const TmemArgs& g, int X, int S, int grid, cudaStream_t st);
-cudaError_t launch_tmem_z2(const TmemArgs& g, int X, int S, int grid, cudaStream_t st);
-cudaError_t launch_tmem_z4(const TmemArgs& g, int X, int S, int grid, cudaStream_t st);
-cudaError_t launch_tmem_z8(const TmemArgs& g, int X, int S, int grid, cudaStream_t st);
+// tensor-memory-privatised FP16-RN scatter (kernel_tmem.cuh).  Geometry: n = 64 * X * S * CS; lane holds X half2
+// words, S feature slices and BQ bucket groups per CTA, CS column slices across CTAs (gridDim.y), NW consumer warps.
+// tmem_shape picks it, returns false when no geometry fits the 512 TMEM columns of a warp's lane quadrant.
+struct TmemShape {
+  int X, S, BQ, CS, NW;
+};
+bool tmem_shape(int n, int d, int zeta, TmemShape* out);
+size_t tmem_smem_bytes_for(int zeta, int n_cta);  // n_cta = n / CS
+int tmem_rows_per_stage(int n_cta);
+cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, const TmemShape& h, int grid, cudaStream_t st);
+cudaError_t launch_tmem_z1(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st);
+cudaError_t launch_tmem_z2(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st);
+cudaError_t launch_tmem_z4(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st);
+cudaError_t launch_tmem_z8(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st);
 
 }  // namespace sk

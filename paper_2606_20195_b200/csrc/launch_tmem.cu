@@ -1,6 +1,8 @@
 // launch_tmem.cu -- instantiations of the tensor-memory-privatised scatter.  Compiled once per zeta
 // (-DSK_TMEM_ZETA=1|2|4|8) so the four families build in parallel; the zeta = 4 unit also holds the
 // shape logic and the dispatcher.
+#include <cstring>
+
 #include "kernel_tmem.cuh"
 #include "launch.h"
 
@@ -11,28 +13,43 @@
 namespace sk {
 namespace {
 
-template <int X, int S>
-cudaError_t go(const TmemArgs& g, int grid, cudaStream_t st) {
-  constexpr int Z = SK_TMEM_ZETA, NW = 4, N = 64 * X * S;
-  auto k = k_tmem<Z, X, S, NW>;
-  const size_t smem = tmem_smem_bytes(Z, N);
-  cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
-  k<<<grid, (NW + 1) * 32, smem, st>>>(g);
-  return cudaGetLastError();
+template <int X, int S, int BQ, int NW>
+cudaError_t go(const TmemArgs& g, const CUtensorMap& tmap, int grid, int cs, cudaStream_t st) {
+  constexpr int Z = SK_TMEM_ZETA, N = 64 * X * S;
+  if constexpr (Z % BQ != 0) {
+    return cudaErrorInvalidValue;
+  } else {
+    auto k = k_tmem<Z, X, S, BQ, NW>;
+    const size_t smem = tmem_smem_bytes(Z, N);
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k<<<dim3((unsigned)grid, (unsigned)cs), (NW + 1) * 32, smem, st>>>(g, tmap);
+    return cudaGetLastError();
+  }
 }
 
-cudaError_t dispatch(const TmemArgs& g, int X, int S, int grid, cudaStream_t st) {
-  switch (X * 10 + S) {
-    case 11: return go<1, 1>(g, grid, st);
-    case 12: return go<1, 2>(g, grid, st);
-    case 14: return go<1, 4>(g, grid, st);
-    case 21: return go<2, 1>(g, grid, st);
-    case 22: return go<2, 2>(g, grid, st);
-    case 24: return go<2, 4>(g, grid, st);
-    case 41: return go<4, 1>(g, grid, st);
-    case 42: return go<4, 2>(g, grid, st);
-    case 44: return go<4, 4>(g, grid, st);
+cudaError_t dispatch(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st) {
+  if (h.NW == 4) {
+    switch (h.X * 100 + h.S * 10 + h.BQ) {
+      case 111: return go<1, 1, 1, 4>(g, tmap, grid, h.CS, st);
+      case 121: return go<1, 2, 1, 4>(g, tmap, grid, h.CS, st);
+      case 141: return go<1, 4, 1, 4>(g, tmap, grid, h.CS, st);
+      case 211: return go<2, 1, 1, 4>(g, tmap, grid, h.CS, st);
+      case 221: return go<2, 2, 1, 4>(g, tmap, grid, h.CS, st);
+      case 241: return go<2, 4, 1, 4>(g, tmap, grid, h.CS, st);
+      case 411: return go<4, 1, 1, 4>(g, tmap, grid, h.CS, st);
+      case 421: return go<4, 2, 1, 4>(g, tmap, grid, h.CS, st);
+      case 441: return go<4, 4, 1, 4>(g, tmap, grid, h.CS, st);
+      case 112: return go<1, 1, 2, 4>(g, tmap, grid, h.CS, st);
+      case 122: return go<1, 2, 2, 4>(g, tmap, grid, h.CS, st);
+      case 212: return go<2, 1, 2, 4>(g, tmap, grid, h.CS, st);
+      case 222: return go<2, 2, 2, 4>(g, tmap, grid, h.CS, st);
+      case 412: return go<4, 1, 2, 4>(g, tmap, grid, h.CS, st);
+      case 422: return go<4, 2, 2, 4>(g, tmap, grid, h.CS, st);
+      case 114: return go<1, 1, 4, 4>(g, tmap, grid, h.CS, st);
+      case 214: return go<2, 1, 4, 4>(g, tmap, grid, h.CS, st);
+      case 414: return go<4, 1, 4, 4>(g, tmap, grid, h.CS, st);
+    }
   }
   return cudaErrorInvalidValue;
 }
@@ -40,39 +57,88 @@ cudaError_t dispatch(const TmemArgs& g, int X, int S, int grid, cudaStream_t st)
 }  // namespace
 
 #if SK_TMEM_ZETA == 1
-cudaError_t launch_tmem_z1(const TmemArgs& g, int X, int S, int grid, cudaStream_t st) { return dispatch(g, X, S, grid, st); }
+cudaError_t launch_tmem_z1(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st) { return dispatch(g, h, tmap, grid, st); }
 #elif SK_TMEM_ZETA == 2
-cudaError_t launch_tmem_z2(const TmemArgs& g, int X, int S, int grid, cudaStream_t st) { return dispatch(g, X, S, grid, st); }
+cudaError_t launch_tmem_z2(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st) { return dispatch(g, h, tmap, grid, st); }
 #elif SK_TMEM_ZETA == 8
-cudaError_t launch_tmem_z8(const TmemArgs& g, int X, int S, int grid, cudaStream_t st) { return dispatch(g, X, S, grid, st); }
+cudaError_t launch_tmem_z8(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st) { return dispatch(g, h, tmap, grid, st); }
 #elif SK_TMEM_ZETA == 4
-cudaError_t launch_tmem_z4(const TmemArgs& g, int X, int S, int grid, cudaStream_t st) { return dispatch(g, X, S, grid, st); }
+cudaError_t launch_tmem_z4(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st) { return dispatch(g, h, tmap, grid, st); }
 
-// widest X (fewest instructions per byte) whose d * X columns fit one lane quadrant; S = n / (64 X) in {1, 2, 4}
-bool tmem_shape(int n, int d, int* X, int* S) {
-  if (n <= 0 || d <= 0 || n % 64 != 0) return false;
-  for (int x = 4; x >= 1; x >>= 1) {
-    if ((int64_t)d * x > kTmemCols || (d * x) % 8 != 0 || n % (64 * x) != 0) continue;
-    const int s = n / (64 * x);
-    if (s != 1 && s != 2 && s != 4) continue;
-    *X = x;
-    *S = s;
-    return true;
+// Geometry for an n-feature, d-row, zeta-block sketch: the fewest column slices CS that fit at all, then
+// the (X, S, BQ) with the fewest issued instructions per KiB of A.  Model (from the SASS of the main loop,
+// profiles/r02_tmem_shapes.md): a row slice of 256 X bytes costs 1 + 3 X instructions to load and convert
+// (in each of the BQ warps that need it) and 5.25 + 2 X per stack block to read-modify-write.
+bool tmem_shape(int n, int d, int zeta, TmemShape* out) {
+  if (n <= 0 || d <= 0 || zeta <= 0 || n % 64 != 0 || d % zeta != 0) return false;
+  const int NW = 4;
+  for (int cs = 1; cs <= 4; cs *= 2) {
+    if (n % (64 * cs) != 0) break;
+    const int nc = n / cs;
+    double best = 0.0;
+    bool found = false;
+    for (int x = 4; x >= 1; x >>= 1) {
+      if (nc % (64 * x) != 0) continue;
+      const int s = nc / (64 * x);
+      if (s != 1 && s != 2 && s != 4) continue;
+      for (int bq = 1; bq <= 4; bq *= 2) {
+        if (s * bq > NW || zeta % bq != 0 || d % bq != 0) continue;
+        const int64_t cols = (int64_t)(d / bq) * x;
+        if (cols > kTmemCols / (NW / 4) || cols % 8 != 0) continue;
+        const double cost = bq * (4.0 / x + 12.0) + zeta * (21.0 / x + 8.0);
+        if (!found || cost < best - 1e-9) {
+          found = true;
+          best = cost;
+          out->X = x; out->S = s; out->BQ = bq; out->CS = cs; out->NW = NW;
+        }
+      }
+    }
+    if (found) return true;
   }
   return false;
 }
 
-size_t tmem_smem_bytes_for(int zeta, int n) { return tmem_smem_bytes(zeta, n); }
-int tmem_rows_per_stage(int n) { return tmem_stage_rows(n); }
+size_t tmem_smem_bytes_for(int zeta, int n_cta) { return tmem_smem_bytes(zeta, n_cta); }
+int tmem_rows_per_stage(int n_cta) { return tmem_stage_rows(n_cta); }
 
-cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, int grid, cudaStream_t st) {
-  int X = 0, S = 0;
-  if (!tmem_shape(g.s.n, g.d, &X, &S)) return cudaErrorInvalidValue;
+// 2-D tensor map over the row range: {n features, rows} FP32, row pitch lda, box {n / CS features, T rows}
+cudaError_t make_tensor_map(const TmemArgs& g, int n_cta, CUtensorMap* out) {
+  typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static encode_fn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q);
+    if (e != cudaSuccess) return e;
+    if (q != cudaDriverEntryPointSuccess || !p) return cudaErrorNotSupported;
+    fn = reinterpret_cast<encode_fn>(p);
+  }
+  const cuuint64_t dims[2] = {(cuuint64_t)g.s.n, (cuuint64_t)g.s.rows};
+  const cuuint64_t strides[1] = {(cuuint64_t)g.s.lda * 4};
+  const cuuint32_t box[2] = {(cuuint32_t)n_cta, (cuuint32_t)tmem_stage_rows(n_cta)};
+  const cuuint32_t estr[2] = {1, 1};
+  CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(g.s.A), dims, strides, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, const TmemShape& h, int grid, cudaStream_t st) {
+  if (64 * h.X * h.S * h.CS != g.s.n) return cudaErrorInvalidValue;
+  CUtensorMap tmap;
+  memset(&tmap, 0, sizeof(tmap));
+  if (g.s.lda != g.s.n / h.CS) {   // the kernel's non-contiguous path
+    if (g.s.rows > 0x7FFFFFFF) return cudaErrorInvalidValue;
+    cudaError_t e = make_tensor_map(g, g.s.n / h.CS, &tmap);
+    if (e != cudaSuccess) return e;
+  }
   switch (zeta) {
-    case 1: return launch_tmem_z1(g, X, S, grid, st);
-    case 2: return launch_tmem_z2(g, X, S, grid, st);
-    case 4: return launch_tmem_z4(g, X, S, grid, st);
-    case 8: return launch_tmem_z8(g, X, S, grid, st);
+    case 1: return launch_tmem_z1(g, h, tmap, grid, st);
+    case 2: return launch_tmem_z2(g, h, tmap, grid, st);
+    case 4: return launch_tmem_z4(g, h, tmap, grid, st);
+    case 8: return launch_tmem_z8(g, h, tmap, grid, st);
   }
   return cudaErrorInvalidValue;
 }

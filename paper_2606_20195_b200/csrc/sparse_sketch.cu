@@ -65,6 +65,7 @@ struct Plan {
   size_t smem_bytes;
   int64_t rows_per_cta;
   int64_t rows_main;  // smem variant: rows handled by k_smem (multiple of its ring rows); the rest go to k_flat
+  sk::TmemShape tm;   // tmem variant: geometry
 };
 
 int ensure_device(sketch* s) {
@@ -110,12 +111,11 @@ bool smem_feasible(const sketch* s, int n, int64_t lda, const void* A, const voi
   return true;
 }
 
-bool tmem_feasible(const sketch* s, int n, int64_t lda, const void* A, const void* B) {
+bool tmem_feasible(const sketch* s, int n, int64_t lda, const void* A, const void* B, sk::TmemShape* h) {
   if (!zeta_templated(s->zeta)) return false;
-  int X = 0, S = 0;
-  if (!sk::tmem_shape(n, s->d, &X, &S)) return false;
+  if (!sk::tmem_shape(n, s->d, s->zeta, h)) return false;
   if (lda % 4 != 0 || !aligned(A, 16) || !aligned(B, 16)) return false;  // TMA bulk copies: 16-byte granules
-  return sk::tmem_smem_bytes_for(s->zeta, n) <= (size_t)s->smem_optin;
+  return sk::tmem_smem_bytes_for(s->zeta, n / h->CS) <= (size_t)s->smem_optin;
 }
 
 int flat_vec_for(bool f16, int n, int64_t lda, const void* A, const void* B, int want_max) {
@@ -147,7 +147,8 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
   const int64_t rb0 = o ? o->row_begin : 0;
   bool sm_ok = f16 && rounding == SKETCH_RN && smem_feasible(s, n, lda, A, B, &sm_bytes) &&
                (rb0 % sk::smem_step_rows(s->zeta) == 0);
-  bool tm_ok = f16 && rounding == SKETCH_RN && tmem_feasible(s, n, lda, A, B);
+  sk::TmemShape tm = {0, 0, 0, 0, 0};
+  bool tm_ok = f16 && rounding == SKETCH_RN && tmem_feasible(s, n, lda, A, B, &tm);
   int vmax = flat_vec_for(f16, n, lda, A, B, 8);
   int vpair = flat_vec_for(f16, n, lda, A, B, f16 ? 2 : 1);
   bool zt = zeta_templated(s->zeta);
@@ -174,11 +175,15 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
   if (v == SKETCH_VARIANT_TMEM) {
     p->hash_mode = 1;  // the producer warp hashes on the fly
     p->replicas = 1;
-    p->wpc = 5;
-    p->smem_bytes = sk::tmem_smem_bytes_for(s->zeta, n);
-    int64_t stages = (rows + sk::tmem_rows_per_stage(n) - 1) / sk::tmem_rows_per_stage(n);
-    int64_t grid = stages < s->sm_count ? stages : s->sm_count;  // one CTA per SM: it owns all 512 TMEM columns
-    if (o && o->grid_ctas > 0) grid = o->grid_ctas;
+    p->tm = tm;
+    p->wpc = tm.NW + 1;
+    p->smem_bytes = sk::tmem_smem_bytes_for(s->zeta, n / tm.CS);
+    const int T = sk::tmem_rows_per_stage(n / tm.CS);
+    int64_t stages = (rows + T - 1) / T;
+    // one CTA per SM (it owns all 512 TMEM columns); gridDim.y = CS column slices share a row range
+    int64_t grid = s->sm_count / tm.CS;
+    if (o && o->grid_ctas > 0) grid = (o->grid_ctas + tm.CS - 1) / tm.CS;
+    if (grid > stages) grid = stages;
     if (grid < 1) grid = 1;
     p->grid = (int)grid;
     return SKETCH_OK;
@@ -338,7 +343,7 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
       sk::TmemArgs g;
       g.s = make_args(s, A, n, lda, B, row_begin, rows, sr_seed, 1);
       g.d = s->d;
-      rc = launched(sk::launch_tmem_f16(g, s->zeta, p.grid, st), "k_tmem");
+      rc = launched(sk::launch_tmem_f16(g, s->zeta, p.tm, p.grid, st), "k_tmem");
       if (rc) return rc;
     }
     return SKETCH_OK;
@@ -618,7 +623,7 @@ int sketch_plan(const sketch_t* cs, int32_t n, int64_t lda, int is_f16, int roun
   if (variant_out) *variant_out = p.variant;
   if (replicas_out) *replicas_out = p.replicas;
   if (hash_mode_out) *hash_mode_out = p.hash_mode;
-  if (grid_out) *grid_out = p.grid;
+  if (grid_out) *grid_out = p.variant == SKETCH_VARIANT_TMEM ? p.grid * p.tm.CS : p.grid;
   return SKETCH_OK;
 }
 

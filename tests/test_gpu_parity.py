@@ -96,6 +96,9 @@ SHAPES_EXACT = [
     # (m, n, d, zeta)   -- config 1, then shapes spanning several tiles with ragged tails
     (4096, 16, 32, 4), (4096, 16, 32, 1), (10007, 64, 128, 4), (33333, 128, 256, 4), (9999, 128, 256, 1),
     (5001, 256, 64, 4), (777, 24, 16, 4), (3000, 8, 8, 1),
+    # config-4 shaped sketches (256 KiB - 1 MiB): bucket groups and column slices of the tensor-memory kernel
+    (6007, 256, 512, 4), (6007, 256, 1024, 4), (4099, 256, 2048, 4), (5003, 512, 512, 4), (7001, 128, 1024, 4),
+    (3001, 512, 128, 1),
 ]
 
 
@@ -281,6 +284,30 @@ def test_row_ranges_accumulate_and_lda(ss, variant):
         out32 = sk.apply_f32acc(Ap[r0:r1, :n], out=out32, row_begin=r0, accumulate=k > 0,
                                 variant=VID[variant] if variant not in ("smem", "tmem") else 0)
     assert np.array_equal(out32.cpu().numpy().astype(np.float64), want)
+
+
+@pytest.mark.parametrize("d", [512, 1024, 2048])
+def test_tmem_column_slices_row_ranges_accumulate_and_lda(ss, d):
+    # config-4 shaped sketches: bucket groups (d = 512) and column slices across CTAs (d = 1024, 2048) of the
+    # tensor-memory kernel, on a padded leading dimension, in three row ranges accumulated into one sketch
+    m, n, zeta = 9001, 256, 4
+    A = wl.integer_valued(m, n, 13)
+    seed = sketch_seed(56 + d)
+    want = oracle.f64_sketch(seed, d, zeta, A)
+    sk = ss.Sketch(m, d, zeta, seed)
+    assert sk.plan(n)["variant"] == "tmem"
+    Ap = torch.full((m, n + 12), float("nan"), device="cuda")
+    Ap[:, :n] = dev(A)
+    out = None
+    for k, (r0, r1) in enumerate(((0, 37), (37, 4001), (4001, m))):
+        out = apply16(ss, sk, Ap[r0:r1, :n], "tmem", out=out, row_begin=r0, accumulate=k > 0)
+    assert np.array_equal(oracle.half_bits_to_f64(bits(out)), want)
+    # Gaussian input: north-star tolerances
+    G = wl.gaussian(m, n, 14)
+    B = oracle.f64_sketch(seed, d, zeta, G)
+    ref = ev.rel_fro(oracle.half_bits_to_f64(oracle.seq16_sketch(seed, d, zeta, G)), B)
+    got = ev.rel_fro(oracle.half_bits_to_f64(bits(apply16(ss, sk, dev(G), "tmem"))), B)
+    assert got <= 1.5 * ref and got <= 5e-2, (got, ref)
 
 
 def test_odd_n_and_poor_alignment_take_the_generic_path(ss):
