@@ -115,8 +115,10 @@ template <int X> SK_DEVINL void tmem_st(uint32_t taddr, const uint32_t (&v)[X]) 
 SK_DEVINL void tmem_st8_zero(uint32_t taddr) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1};" ::"r"(taddr), "r"(0u));
 }
-SK_DEVINL void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-SK_DEVINL void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// no "memory" clobber: these order tensor-memory traffic only (volatile asms keep their mutual order), so the
+// compiler may hoist the next group's shared-memory loads above them
+SK_DEVINL void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;"); }
+SK_DEVINL void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;"); }
 // tcgen05.ld writes its registers asynchronously: every use must be ordered behind tcgen05.wait::ld.  An
 // empty volatile asm that "modifies" the register gives the compiler that dependency at no cost.
 SK_DEVINL void tmem_tie(uint32_t& v) { asm volatile("" : "+r"(v)); }
@@ -128,43 +130,163 @@ SK_DEVINL uint32_t hfma2_u32(uint32_t q, uint32_t mult, uint32_t acc) {
 }
 
 // ---------------------------------------------------------------------------------------- geometry
-template <int ZETA, int X, int S, int BQ, int NW, int T>
-struct TmemGeom {
-  static_assert(NW % 4 == 0 && NW % (S * BQ) == 0, "consumer warps: whole lane quadrants, whole slice x bucket-group sets");
-  static_assert(ZETA % BQ == 0, "bucket groups are whole stack blocks");
-  static constexpr int ZB = ZETA / BQ;         // stack blocks one warp accumulates
-  static constexpr int RS = NW / (S * BQ);     // row-sets per stage
-  static constexpr int TR = T / RS;            // rows of a stage one warp processes
-  #ifndef SK_TMEM_G_SMALL
-#define SK_TMEM_G_SMALL 4
-#endif
-  static constexpr int G = (ZB >= 4 || (BQ > 1 && ZB >= 2)) ? 2 : SK_TMEM_G_SMALL;  // rows per group (LDTMs in flight = G * ZB)
-  static_assert(TR % G == 0, "whole groups");
-  static constexpr int N = 64 * X * S;         // features of the CTA's column slice
-  static constexpr int WC = kTmemCols / (NW / 4);  // tensor-memory columns of one warp's private region
-  static constexpr int A_BYTES = T * N * 4;
-  static constexpr int E_BYTES = T * ZETA * 8;
-  static constexpr int STAGE_BYTES = A_BYTES + E_BYTES;
-};
-
 // rows per stage: 32 KiB of A per stage (16 KiB at n = 64), at least 16 rows
 __host__ __device__ constexpr int tmem_stage_rows(int n) { return n <= 128 ? 64 : n == 256 ? 32 : 16; }
 __host__ __device__ constexpr int tmem_stages(int n) { return n <= 512 ? 4 : 3; }
-constexpr size_t tmem_smem_bytes(int zeta, int n) {
-  return (size_t)tmem_stages(n) * ((size_t)tmem_stage_rows(n) * n * 4 + (size_t)tmem_stage_rows(n) * zeta * 8) + 16 * 8 + 16;
+// bytes of one (row, bucket group) record / side-list item of the deferral modes: {q offset | row, 0, then (col, mul) x ZB}
+__host__ __device__ constexpr int tmem_rec_bytes(int zb) { return zb == 1 ? 16 : 16 + 8 * zb; }
+
+// GM = group mode: how two rows of one group that hit the same sketch row are kept from losing an update.
+//   0      groups of G = 2 (4 for short block lists) rows; same-bucket rows are chained in registers.  Works for any
+//          d, costs O(G^2) compares and selects per block, so G stays small and few LDTMs are in flight.
+//   1, 2   DEFERRAL, groups of 4 / 8 rows, bucket-group kernels only (BQ > 1).  The producer finds every row that
+//          shares a sketch row with a LATER row of its group (rare when d / zeta >> G^2), points that row's main-loop
+//          record at an all-zero FP16 row and, in the clashing blocks, at a substitute sketch row that no row of the
+//          group touches (adding +0 there changes nothing), and appends the row to a per-stage side list that the
+//          consumers apply one row at a time after the main loop.  The main loop then has pairwise distinct TMEM
+//          addresses within a group by construction: no compares, no selects, 8 read-modify-writes in flight.
+template <int ZETA, int X, int S, int BQ, int NW, int GM, int T>
+struct TmemGeom {
+  static_assert(NW % 4 == 0 && NW % (S * BQ) == 0, "consumer warps: whole lane quadrants, whole slice x bucket-group sets");
+  static_assert(ZETA % BQ == 0, "bucket groups are whole stack blocks");
+  static_assert(GM == 0 || BQ > 1, "deferral needs the shared FP16 tile of the bucket-group kernels");
+  static constexpr int ZB = ZETA / BQ;         // stack blocks one warp accumulates
+  static constexpr int RS = NW / (S * BQ);     // row-sets per stage
+  static constexpr int TR = T / RS;            // rows of a stage one warp processes
+  static constexpr bool DEF = GM != 0;
+  static constexpr int G = GM == 1 ? 4 : GM == 2 ? 8 : (ZB >= 4 || (BQ > 1 && ZB >= 2)) ? 2 : 4;  // rows per group (LDTMs in flight = G * ZB)
+  static_assert(TR % G == 0 && 32 % G == 0, "whole groups");
+  static constexpr int N = 64 * X * S;         // features of the CTA's column slice
+  static constexpr int WC = kTmemCols / (NW / 4);  // tensor-memory columns of one warp's private region
+  static constexpr int A_BYTES = T * N * 4;
+  // chained modes: entries [row][zeta] {col, mul}.  Deferral: records [row][BQ] of RB bytes, then per (chunk phase,
+  // bucket group) a side list of up to T items of RB bytes, then the NPC * BQ item counts.
+  static constexpr int RB = tmem_rec_bytes(ZB);
+  static constexpr int E_BYTES = DEF ? T * BQ * RB : T * ZETA * 8;
+  // producer warps: one in the chained modes; the deferral bookkeeping triples the hash stage's work, so there the
+  // stage's 32-row chunks go to NPC warps and the bucket groups of a chunk to NPB warps
+  static constexpr int CH = (T + 31) / 32;
+  static constexpr int NPC = DEF ? (CH >= 2 ? 2 : 1) : 1;
+  static constexpr int NPB = DEF ? (BQ < 4 / NPC ? BQ : 4 / NPC) : 1;
+  static constexpr int NP = NPC * NPB;
+  static constexpr int L_BYTES = DEF ? NPC * BQ * T * RB + 128 : 0;
+  static constexpr int STAGE_BYTES = A_BYTES + E_BYTES + L_BYTES;
+  static_assert(STAGE_BYTES % 128 == 0, "TMA destination alignment");
+  // bucket groups: every row is needed by BQ warps, so the consumer warps first convert the stage ONCE into a
+  // shared FP16 tile (a3, a4), meet at a named barrier, and then each scatters its own blocks from that tile.
+  // Two tiles (stage parity); the deferral modes append one all-zero row to each.
+  static constexpr bool SHQ = BQ > 1;
+  static constexpr int Q_ROW = N * 2;
+  static constexpr int Q_BYTES = T * Q_ROW + (DEF ? Q_ROW : 0);
+  static_assert((T * N / 4) % (NW * 32) == 0, "whole conversion passes");
+};
+
+__host__ __device__ constexpr int tmem_producers(int n, int bq, int gm) {
+  return gm == 0 ? 1 : (tmem_stage_rows(n) >= 64 ? 2 : 1) * (bq < (tmem_stage_rows(n) >= 64 ? 2 : 4) ? bq : (tmem_stage_rows(n) >= 64 ? 2 : 4));
+}
+// ring of stages | barriers + TMEM base (256 B) | with bucket groups: two converted (FP16) tiles | deferral: 2 KiB of
+// producer scratch (the sketch rows of a 32-row chunk, one 128-byte line per producer warp and block)
+constexpr size_t tmem_smem_bytes(int zeta, int n, int bq, int gm) {
+  const size_t t = (size_t)tmem_stage_rows(n);
+  const size_t rb = (size_t)tmem_rec_bytes(zeta / bq);
+  const size_t e = gm ? t * bq * rb + 2 * bq * t * rb + 128 : t * zeta * 8;
+  return (size_t)tmem_stages(n) * (t * n * 4 + e) + 256 + (bq > 1 ? 2 * (t * n * 2 + (gm ? (size_t)n * 2 : 0)) : 0) + (gm ? 2048 : 0);
+}
+
+// a5 for R rows x ZB stack blocks of one warp: LDTM, one RN16 add per half (fma.rn.f16x2 by +-1), STTM.
+// CHAIN: two rows of the call that hit the same sketch row are chained in registers (the later row adds onto
+// the earlier row's result and both store the chain's final value; the bucket is warp-uniform, so this is a
+// select, not divergence).  Without CHAIN the caller guarantees distinct sketch rows within a block.
+template <int R, int ZB, int X, bool CHAIN>
+SK_DEVINL void tmem_rmw(uint32_t region, const uint32_t (*q)[X], const uint32_t (*col)[ZB], const uint32_t (*mul)[ZB]) {
+  uint32_t acc[R][ZB][X];
+  tmem_wait_st();                              // the previous stores are in TMEM
+#pragma unroll
+  for (int r = 0; r < R; ++r)
+#pragma unroll
+    for (int j = 0; j < ZB; ++j) tmem_ld<X>(region + col[r][j], acc[r][j]);
+  tmem_wait_ld();
+#pragma unroll
+  for (int r = 0; r < R; ++r)
+#pragma unroll
+    for (int j = 0; j < ZB; ++j)
+#pragma unroll
+      for (int k = 0; k < X; ++k) tmem_tie(acc[r][j][k]);
+#pragma unroll
+  for (int j = 0; j < ZB; ++j) {
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      if constexpr (CHAIN) {
+#pragma unroll
+        for (int p = 0; p < r; ++p) {
+          const bool same = col[p][j] == col[r][j];
+#pragma unroll
+          for (int k = 0; k < X; ++k) acc[r][j][k] = same ? acc[p][j][k] : acc[r][j][k];
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < X; ++k) acc[r][j][k] = hfma2_u32(q[r][k], mul[r][j], acc[r][j][k]);
+    }
+    if constexpr (CHAIN) {
+#pragma unroll
+      for (int r = R - 2; r >= 0; --r) {
+#pragma unroll
+        for (int p = R - 1; p > r; --p) {
+          const bool same = col[p][j] == col[r][j];
+#pragma unroll
+          for (int k = 0; k < X; ++k) acc[r][j][k] = same ? acc[p][j][k] : acc[r][j][k];
+        }
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) tmem_st<X>(region + col[r][j], acc[r][j]);
+  }
+}
+
+// FP16 words of one lane (X half2) from the shared converted tile
+template <int X> SK_DEVINL void lds_q(const unsigned char* p, uint32_t (&q)[X]) {
+  if constexpr (X == 1) q[0] = *reinterpret_cast<const uint32_t*>(p);
+  else if constexpr (X == 2) { const uint2 t = *reinterpret_cast<const uint2*>(p); q[0] = t.x; q[1] = t.y; }
+  else { const uint4 t = *reinterpret_cast<const uint4*>(p); q[0] = t.x; q[1] = t.y; q[2] = t.z; q[3] = t.w; }
+}
+// record / side-list item of the deferral modes -> head word (q offset or row), (col, mul) x ZB
+template <int ZB> SK_DEVINL void lds_rec(const unsigned char* p, uint32_t& head, uint32_t (&col)[ZB], uint32_t (&mul)[ZB]) {
+  const uint4 t = *reinterpret_cast<const uint4*>(p);
+  head = t.x;
+  if constexpr (ZB == 1) { col[0] = t.z; mul[0] = t.w; }
+  else {
+#pragma unroll
+    for (int k = 0; k < ZB / 2; ++k) {
+      const uint4 u = *reinterpret_cast<const uint4*>(p + 16 + 16 * k);
+      col[2 * k] = u.x; mul[2 * k] = u.y; col[2 * k + 1] = u.z; mul[2 * k + 1] = u.w;
+    }
+  }
+}
+template <int ZB> SK_DEVINL void sts_rec(uint32_t p, uint32_t head, const uint32_t (&col)[ZB], const uint32_t (&mul)[ZB]) {
+  if constexpr (ZB == 1) {
+    asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p), "r"(head), "r"(0u), "r"(col[0]), "r"(mul[0]) : "memory");
+  } else {
+    asm volatile("st.shared.v4.b32 [%0], {%1,%2,%2,%2};" ::"r"(p), "r"(head), "r"(0u) : "memory");
+#pragma unroll
+    for (int k = 0; k < ZB / 2; ++k)
+      asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p + 16 + 16 * k), "r"(col[2 * k]), "r"(mul[2 * k]), "r"(col[2 * k + 1]), "r"(mul[2 * k + 1]) : "memory");
+  }
 }
 
 // ---------------------------------------------------------------------------------------- the kernel
-template <int ZETA, int X, int S, int BQ, int NW>
-__global__ void __launch_bounds__((NW + 1) * 32, 1) k_tmem(TmemArgs g, const __grid_constant__ CUtensorMap tmap) {
+template <int ZETA, int X, int S, int BQ, int NW, int GM>
+__global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM)) * 32, 1) k_tmem(TmemArgs g, const __grid_constant__ CUtensorMap tmap) {
   constexpr int T = tmem_stage_rows(64 * X * S), NS = tmem_stages(64 * X * S);
-  using Geo = TmemGeom<ZETA, X, S, BQ, NW, T>;
-  constexpr int TR = Geo::TR, G = Geo::G, N = Geo::N, ZB = Geo::ZB;
+  using Geo = TmemGeom<ZETA, X, S, BQ, NW, GM, T>;
+  constexpr int TR = Geo::TR, G = Geo::G, N = Geo::N, ZB = Geo::ZB, RB = Geo::RB, NP = Geo::NP, NPC = Geo::NPC, NPB = Geo::NPB;
+  static_assert(NP == tmem_producers(N, BQ, GM), "producer warps");
+  constexpr int JB = ZETA / NPB;                     // stack blocks one producer warp hashes
+  constexpr uint32_t Q0 = NS * Geo::STAGE_BYTES + 256;   // first converted tile
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const ScatterArgs& a = g.s;
   const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
-  // shared-memory carve-up: [NS][A tile | entries] then the barriers
+  // shared-memory carve-up: [NS][A tile | entries or records | side lists] then the barriers, then the FP16 tiles
   const uint32_t smem0 = smem_u32(smem_raw);
   const uint32_t bars = smem0 + NS * Geo::STAGE_BYTES;     // full[NS], empty[NS], 8 B each
   uint32_t* const tbase_p = reinterpret_cast<uint32_t*>(smem_raw + NS * Geo::STAGE_BYTES + 16 * NS);
@@ -175,11 +297,17 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_tmem(TmemArgs g, const __g
   }
   if (tid == 32) {
     for (int k = 0; k < NS; ++k) {
-      mbar_init(bars + 8 * k, 1);              // full: the producer's arrive (+ the TMA transaction bytes)
+      mbar_init(bars + 8 * k, NP);             // full: one arrive per producer warp (+ the TMA transaction bytes)
       mbar_init(bars + 8 * (NS + k), NW);      // empty: one arrive per consumer warp
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async;" ::: "memory");
+  }
+  if constexpr (Geo::DEF) {                    // the all-zero row behind each converted tile
+    for (uint32_t i = tid * 4; i < 2u * Geo::Q_ROW; i += (NW + NP) * 32 * 4) {
+      const uint32_t tile = i / Geo::Q_ROW, off = i % Geo::Q_ROW;
+      *reinterpret_cast<uint32_t*>(smem_raw + Q0 + tile * Geo::Q_BYTES + T * Geo::Q_ROW + off) = 0u;
+    }
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
@@ -190,19 +318,24 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_tmem(TmemArgs g, const __g
   const int64_t col0 = (int64_t)blockIdx.y * N;   // first feature of this CTA's column slice
   const uint32_t dloc = (uint32_t)g.d / BQ;        // sketch rows one warp holds
 
-  if (warp == NW) {
-    // ================================================================ producer: TMA + hash stage (a1, a2)
+  if (warp >= NW) {
+    // ================================================================ producers: TMA + hash stage (a1, a2)
+    const uint32_t pw = warp - NW;                 // producer warp pw: 32-row chunks cp, cp + NPC, ...; stack blocks [j0, j0 + JB)
+    const uint32_t cp = pw % NPC, j0 = (pw / NPC) * JB, b0 = j0 / ZB;
+    unsigned char* const scr = smem_raw + Q0 + 2 * Geo::Q_BYTES + pw * (JB * 128);   // deferral: [JB][32] sketch rows
+    static_assert(!Geo::DEF || NP * JB * 128 <= 2048, "producer scratch");
     const uint64_t policy = l2_evict_first_policy();
     const bool contiguous = (a.lda == N);          // implies a single column slice
     uint32_t it = 0;
     for (int64_t st = blockIdx.x; st < nstages; st += gridDim.x, ++it) {
       const uint32_t slot = it % NS, ph = (it / NS) & 1;
-      const uint32_t sA = smem0 + slot * Geo::STAGE_BYTES, sE = sA + Geo::A_BYTES;
+      const uint32_t sA = smem0 + slot * Geo::STAGE_BYTES, sE = sA + Geo::A_BYTES, sL = sE + Geo::E_BYTES;
       const uint32_t full = bars + 8 * slot, empty = bars + 8 * (NS + slot);
       mbar_wait(empty, ph ^ 1);                // passes at once the first time round the ring
       const int64_t row0 = st * T;
       const int32_t nrows = (int32_t)min((int64_t)T, a.rows - row0);
-      if (contiguous) {
+      if (pw != 0) {
+      } else if (contiguous) {
         if (lane == 0) {
           mbar_expect_tx(full, (uint32_t)nrows * N * 4);
           bulk_g2s(sA, a.A + row0 * a.lda, (uint32_t)nrows * N * 4, full, policy);
@@ -211,30 +344,103 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_tmem(TmemArgs g, const __g
         mbar_expect_tx(full, (uint32_t)T * N * 4);
         tensor_g2s(sA, &tmap, (int32_t)col0, (int32_t)row0, full, policy);
       }
-      if (contiguous && nrows < T) {           // last stage of the matrix: rows past the end contribute +0
+      if (pw == 0 && contiguous && nrows < T) {           // last stage of the matrix: rows past the end contribute +0
         const uint32_t z0 = sA + nrows * N * 4, z1 = sA + Geo::A_BYTES;
         for (uint32_t p = z0 + lane * 16; p < z1; p += 32 * 16) asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(p), "r"(0u) : "memory");
       }
-      // a1: entries of rows lane, lane + 32, ...: {(bucket - first sketch row of the block's group) * X, +-1.0 | +-1.0}
+      // a1: rows lane, lane + 32, ... of the stage
+      uint32_t cnt[BQ];                        // deferral: side-list lengths (warp-uniform)
 #pragma unroll
-      for (int rr = 0; rr < (T + 31) / 32; ++rr) {
+      for (int b = 0; b < BQ; ++b) cnt[b] = 0;
+#pragma unroll
+      for (int rr = (int)cp; rr < (T + 31) / 32; rr += NPC) {
         const int32_t r = rr * 32 + (int32_t)lane;
-        if (T % 32 != 0 && r >= T) break;      // stages of 16 rows (n >= 512): half a warp hashes
+        const bool live = (T % 32 == 0) || r < T;   // stages of 16 rows (n >= 512): half a warp's rows exist
         const uint64_t ctr0 = (uint64_t)(a.row_begin + row0 + r) * ZETA;
-        uint32_t w[2 * ZETA];
+        uint32_t bk[JB], mulw[JB];             // sketch row, +-1.0 | +-1.0 of blocks j0 + j
 #pragma unroll
-        for (int j = 0; j < ZETA; ++j) {
-          const uint32_t e = hash_entry(a.seed, ctr0 + j, j, a.db);
-          w[2 * j] = (entry_bucket(e) - (uint32_t)(j / ZB) * dloc) * X;
-          w[2 * j + 1] = 0x3C003C00u ^ entry_signmask_h2(e);
+        for (int j = 0; j < JB; ++j) {
+          const uint32_t e = hash_entry(a.seed, ctr0 + j0 + j, j0 + j, a.db);
+          bk[j] = entry_bucket(e);
+          mulw[j] = 0x3C003C00u ^ entry_signmask_h2(e);
         }
-        const uint32_t p = sE + r * (ZETA * 8);
-        if constexpr (ZETA == 1) asm volatile("st.shared.v2.b32 [%0], {%1,%2};" ::"r"(p), "r"(w[0]), "r"(w[1]) : "memory");
-        else {
+        if constexpr (!Geo::DEF) {
+          // entries {(bucket - first sketch row of the block's group) * X, multiplier}
+          if (live) {
+            const uint32_t p = sE + r * (ZETA * 8);
+            if constexpr (ZETA == 1) asm volatile("st.shared.v2.b32 [%0], {%1,%2};" ::"r"(p), "r"(bk[0] * X), "r"(mulw[0]) : "memory");
+            else {
 #pragma unroll
-          for (int k = 0; k < ZETA / 2; ++k)
-            asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p + 16 * k), "r"(w[4 * k]), "r"(w[4 * k + 1]), "r"(w[4 * k + 2]), "r"(w[4 * k + 3]) : "memory");
+              for (int k = 0; k < ZETA / 2; ++k)
+                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p + 16 * k),
+                             "r"((bk[2 * k] - (uint32_t)((2 * k) / ZB) * dloc) * X), "r"(mulw[2 * k]),
+                             "r"((bk[2 * k + 1] - (uint32_t)((2 * k + 1) / ZB) * dloc) * X), "r"(mulw[2 * k + 1]) : "memory");
+            }
+          }
+        } else {
+          // deferral (see TmemGeom): ls bit j = a later row of my group of G rows has my sketch row in block j
+          // the group's sketch rows go through shared memory (one store, G/4 broadcast loads per block; a MATCH.ANY
+          // over 32 distinct keys costs ~200 cycles, G - 1 shuffles about as many instructions)
+          const uint32_t pg = lane % G;
+          uint32_t ls = 0, og[JB][G];
+          __syncwarp();
+#pragma unroll
+          for (int j = 0; j < JB; ++j) reinterpret_cast<uint32_t*>(scr + j * 128)[lane] = bk[j];
+          __syncwarp();
+#pragma unroll
+          for (int j = 0; j < JB; ++j) {
+#pragma unroll
+            for (int k = 0; k < G / 4; ++k) {
+              const uint4 t = *reinterpret_cast<const uint4*>(scr + j * 128 + (lane - pg) * 4 + 16 * k);
+              og[j][4 * k] = t.x; og[j][4 * k + 1] = t.y; og[j][4 * k + 2] = t.z; og[j][4 * k + 3] = t.w;
+            }
+            uint32_t eq = 0;                     // bit i: row i of my group has my sketch row
+#pragma unroll
+            for (int i = 0; i < G; ++i) eq |= (og[j][i] == bk[j] ? 1u : 0u) << i;
+            if ((eq >> (pg + 1)) != 0u) ls |= 1u << j;
+          }
+          if (!live) ls = 0;
+          uint32_t fb[JB];                     // sketch row the main loop touches
+#pragma unroll
+          for (int j = 0; j < JB; ++j) fb[j] = bk[j];
+          // substitute sketch row in a clashing block: first of j*db + pg, + G, + 2G, ... that no row of the group
+          // hashed to.  Different rows of a group draw from different residue classes mod G, so two substitutes never
+          // coincide; at most G candidates are taken, hence the host requires d / zeta >= G * (G + 1).
+#pragma unroll
+          for (int j = 0; j < JB; ++j) {
+            if (__any_sync(0xFFFFFFFFu, (ls >> j) & 1u)) {
+              const uint32_t base = (j0 + (uint32_t)j) * a.db + pg;
+              uint32_t taken = 0;              // bit t: candidate base + t*G is some row's sketch row
+#pragma unroll
+              for (int k = 0; k < G; ++k) {
+                const uint32_t diff = og[j][k] - base;   // wraps to a huge value when that row lies below base
+                if ((diff % G) == 0u && diff / G <= (uint32_t)G) taken |= 1u << (diff / G);
+              }
+              if ((ls >> j) & 1u) fb[j] = base + (uint32_t)(__ffs((int)~taken) - 1) * G;
+            }
+          }
+#pragma unroll
+          for (int bb = 0; bb < BQ / NPB; ++bb) {  // my bucket groups b0 + bb
+            const uint32_t b = b0 + bb;
+            const bool def = ((ls >> (bb * ZB)) & ((1u << ZB) - 1u)) != 0u;
+            uint32_t cm[ZB], co[ZB], mm[ZB];
+#pragma unroll
+            for (int jj = 0; jj < ZB; ++jj) {
+              cm[jj] = (fb[bb * ZB + jj] - b * dloc) * X;
+              co[jj] = (bk[bb * ZB + jj] - b * dloc) * X;
+              mm[jj] = mulw[bb * ZB + jj];
+            }
+            if (live) sts_rec<ZB>(sE + ((uint32_t)r * BQ + b) * RB, def ? (uint32_t)(T * Geo::Q_ROW) : (uint32_t)r * Geo::Q_ROW, cm, mm);
+            const uint32_t m = __ballot_sync(0xFFFFFFFFu, def);
+            if (def) sts_rec<ZB>(sL + ((cp * BQ + b) * T + cnt[bb] + __popc(m & ((1u << lane) - 1u))) * RB, (uint32_t)r, co, mm);
+            cnt[bb] += __popc(m);
+          }
         }
+      }
+      if constexpr (Geo::DEF) {
+#pragma unroll
+        for (int bb = 0; bb < BQ / NPB; ++bb)
+          if (lane == bb) asm volatile("st.shared.b32 [%0], %1;" ::"r"(sL + NPC * BQ * T * RB + (cp * BQ + b0 + bb) * 4), "r"(cnt[bb]) : "memory");
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(full);
@@ -249,82 +455,88 @@ __global__ void __launch_bounds__((NW + 1) * 32, 1) k_tmem(TmemArgs g, const __g
 
     const float scale = a.scale;
     const uint32_t a_off = (rowset * TR) * (N * 4) + (slice * 64 * X + lane * 2 * X) * 4;
-    const uint32_t e_off = (rowset * TR) * (ZETA * 8) + bgrp * (ZB * 8);
+    const uint32_t e_off = Geo::DEF ? ((rowset * TR) * BQ + bgrp) * RB : (rowset * TR) * (ZETA * 8) + bgrp * (ZB * 8);
     uint32_t it = 0;
     for (int64_t st = blockIdx.x; st < nstages; st += gridDim.x, ++it) {
       const uint32_t slot = it % NS, ph = (it / NS) & 1;
       const unsigned char* const sA = smem_raw + slot * Geo::STAGE_BYTES + a_off;
       const unsigned char* const sE = smem_raw + slot * Geo::STAGE_BYTES + Geo::A_BYTES + e_off;
       mbar_wait(bars + 8 * slot, ph);
+      const unsigned char* qlane = nullptr;    // this lane's words of row 0 of the converted tile
+      if constexpr (Geo::SHQ) {
+        // a3, a4 once per element: the whole stage -> FP16 tile `it & 1` (row pitch N * 2 bytes)
+        const float4* const tile = reinterpret_cast<const float4*>(smem_raw + slot * Geo::STAGE_BYTES);
+        unsigned char* const qb = smem_raw + Q0 + (it & 1u) * Geo::Q_BYTES;
+        constexpr int CI = (T * N / 4) / (NW * 32), CB = CI < 8 ? CI : 8;   // loads in batches of CB (the stores may alias for all the compiler knows)
+#pragma unroll
+        for (int i0 = 0; i0 < CI; i0 += CB) {
+          float4 t[CB];
+#pragma unroll
+          for (int i = 0; i < CB; ++i) t[i] = tile[(uint32_t)(i0 + i) * (NW * 32) + tid];
+#pragma unroll
+          for (int i = 0; i < CB; ++i)
+            reinterpret_cast<uint2*>(qb)[(uint32_t)(i0 + i) * (NW * 32) + tid] =
+                make_uint2(pack_rn(t[i].x * scale, t[i].y * scale), pack_rn(t[i].z * scale, t[i].w * scale));
+        }
+        // all consumer warps: tile `it & 1` is complete, and every warp is done scattering tile `(it - 1) & 1`
+        asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
+        qlane = qb + (slice * 64 * X + lane * 2 * X) * 2;
+      }
 #pragma unroll
       for (int g0 = 0; g0 < TR; g0 += G) {
         uint32_t q[G][X], col[G][ZB], mul[G][ZB];
 #pragma unroll
         for (int r = 0; r < G; ++r) {
-          // a2 (from the staged tile), a3, a4: q = RN16(s * a), two features per word
-          float v[2 * X];
-          const unsigned char* pa = sA + (g0 + r) * (N * 4);
-          if constexpr (X == 1) { const float2 t = *reinterpret_cast<const float2*>(pa); v[0] = t.x; v[1] = t.y; }
-          else {
+          if constexpr (Geo::DEF) {
+            uint32_t qoff;
+            lds_rec<ZB>(sE + (g0 + r) * (BQ * RB), qoff, col[r], mul[r]);
+            lds_q<X>(qlane + qoff, q[r]);
+          } else {
+            if constexpr (Geo::SHQ) {
+              lds_q<X>(qlane + (rowset * TR + g0 + r) * Geo::Q_ROW, q[r]);
+            } else {
+              // a2 (from the staged tile), a3, a4: q = RN16(s * a), two features per word
+              float v[2 * X];
+              const unsigned char* pa = sA + (g0 + r) * (N * 4);
+              if constexpr (X == 1) { const float2 t = *reinterpret_cast<const float2*>(pa); v[0] = t.x; v[1] = t.y; }
+              else {
 #pragma unroll
-            for (int k = 0; k < X / 2; ++k) {
-              const float4 t = *reinterpret_cast<const float4*>(pa + 16 * k);
-              v[4 * k] = t.x; v[4 * k + 1] = t.y; v[4 * k + 2] = t.z; v[4 * k + 3] = t.w;
+                for (int k = 0; k < X / 2; ++k) {
+                  const float4 t = *reinterpret_cast<const float4*>(pa + 16 * k);
+                  v[4 * k] = t.x; v[4 * k + 1] = t.y; v[4 * k + 2] = t.z; v[4 * k + 3] = t.w;
+                }
+              }
+#pragma unroll
+              for (int k = 0; k < X; ++k) q[r][k] = pack_rn(v[2 * k] * scale, v[2 * k + 1] * scale);
             }
-          }
+            const unsigned char* pe = sE + (g0 + r) * (ZETA * 8);
+            if constexpr (ZB == 1) { const uint2 t = *reinterpret_cast<const uint2*>(pe); col[r][0] = t.x; mul[r][0] = t.y; }
+            else {
 #pragma unroll
-          for (int k = 0; k < X; ++k) q[r][k] = pack_rn(v[2 * k] * scale, v[2 * k + 1] * scale);
-          const unsigned char* pe = sE + (g0 + r) * (ZETA * 8);
-          if constexpr (ZB == 1) { const uint2 t = *reinterpret_cast<const uint2*>(pe); col[r][0] = t.x; mul[r][0] = t.y; }
-          else {
-#pragma unroll
-            for (int k = 0; k < ZB / 2; ++k) {
-              const uint4 t = *reinterpret_cast<const uint4*>(pe + 16 * k);
-              col[r][2 * k] = t.x; mul[r][2 * k] = t.y; col[r][2 * k + 1] = t.z; mul[r][2 * k + 1] = t.w;
+              for (int k = 0; k < ZB / 2; ++k) {
+                const uint4 t = *reinterpret_cast<const uint4*>(pe + 16 * k);
+                col[r][2 * k] = t.x; mul[r][2 * k] = t.y; col[r][2 * k + 1] = t.z; mul[r][2 * k + 1] = t.w;
+              }
             }
           }
         }
         // a5: read-modify-write of G x ZB sketch rows in tensor memory
-        uint32_t acc[G][ZB][X];
-        tmem_wait_st();                        // the previous group's stores are in TMEM
-#pragma unroll
-        for (int r = 0; r < G; ++r)
-#pragma unroll
-          for (int j = 0; j < ZB; ++j) tmem_ld<X>(region + col[r][j], acc[r][j]);
-        tmem_wait_ld();
-#pragma unroll
-        for (int r = 0; r < G; ++r)
-#pragma unroll
-          for (int j = 0; j < ZB; ++j)
-#pragma unroll
-            for (int k = 0; k < X; ++k) tmem_tie(acc[r][j][k]);
-#pragma unroll
-        for (int j = 0; j < ZB; ++j) {
-#pragma unroll
-          for (int r = 0; r < G; ++r) {
-            // chain onto the latest earlier row of the group that hit the same sketch row
-#pragma unroll
-            for (int p = 0; p < r; ++p) {
-              const bool same = col[p][j] == col[r][j];
-#pragma unroll
-              for (int k = 0; k < X; ++k) acc[r][j][k] = same ? acc[p][j][k] : acc[r][j][k];
-            }
-#pragma unroll
-            for (int k = 0; k < X; ++k) acc[r][j][k] = hfma2_u32(q[r][k], mul[r][j], acc[r][j][k]);
+        tmem_rmw<G, ZB, X, !Geo::DEF>(region, q, col, mul);
+      }
+      if constexpr (Geo::DEF) {
+        // the deferred rows of this stage (TmemGeom): original sketch rows, one row at a time
+        const unsigned char* const sL = smem_raw + slot * Geo::STAGE_BYTES + Geo::A_BYTES + Geo::E_BYTES;
+#pragma unroll 1
+        for (uint32_t pl = 0; pl < (uint32_t)NPC; ++pl) {
+          const uint32_t cnt = *reinterpret_cast<const uint32_t*>(sL + NPC * BQ * T * RB + (pl * BQ + bgrp) * 4);
+#pragma unroll 1
+          for (uint32_t i = 0; i < cnt; ++i) {
+            uint32_t row, q1[1][X], c1[1][ZB], m1[1][ZB];
+            lds_rec<ZB>(sL + ((pl * BQ + bgrp) * T + i) * RB, row, c1[0], m1[0]);
+            if (row / TR != rowset) continue;
+            lds_q<X>(qlane + row * Geo::Q_ROW, q1[0]);
+            tmem_rmw<1, ZB, X, false>(region, q1, c1, m1);
           }
-          // rows of the group that share a sketch row all store the chain's final value: the stores need
-          // no predicate and their order does not matter
-#pragma unroll
-          for (int r = G - 2; r >= 0; --r) {
-#pragma unroll
-            for (int p = G - 1; p > r; --p) {
-              const bool same = col[p][j] == col[r][j];
-#pragma unroll
-              for (int k = 0; k < X; ++k) acc[r][j][k] = same ? acc[p][j][k] : acc[r][j][k];
-            }
-          }
-#pragma unroll
-          for (int r = 0; r < G; ++r) tmem_st<X>(region + col[r][j], acc[r][j]);
         }
       }
       __syncwarp();

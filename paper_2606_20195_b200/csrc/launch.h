@@ -27,10 +27,10 @@ int smem_max_bucket();
 // words, S feature slices and BQ bucket groups per CTA, CS column slices across CTAs (gridDim.y), NW consumer warps.
 // tmem_shape picks it, returns false when no geometry fits the 512 TMEM columns of a warp's lane quadrant.
 struct TmemShape {
-  int X, S, BQ, CS, NW;
+  int X, S, BQ, CS, NW, GM;
 };
 bool tmem_shape(int n, int d, int zeta, TmemShape* out);
-size_t tmem_smem_bytes_for(int zeta, int n_cta);  // n_cta = n / CS
+size_t tmem_smem_bytes_for(int zeta, int n_cta, int bq, int gm);  // n_cta = n / CS
 int tmem_rows_per_stage(int n_cta);
 cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, const TmemShape& h, int grid, cudaStream_t st);
 cudaError_t launch_tmem_z1(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st);

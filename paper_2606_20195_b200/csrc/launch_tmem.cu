@@ -1,6 +1,7 @@
 // launch_tmem.cu -- instantiations of the tensor-memory-privatised scatter.  Compiled once per zeta
 // (-DSK_TMEM_ZETA=1|2|4|8) so the four families build in parallel; the zeta = 4 unit also holds the
 // shape logic and the dispatcher.
+#include <cstdlib>
 #include <cstring>
 
 #include "kernel_tmem.cuh"
@@ -13,17 +14,17 @@
 namespace sk {
 namespace {
 
-template <int X, int S, int BQ, int NW>
+template <int X, int S, int BQ, int NW, int GM>
 cudaError_t go(const TmemArgs& g, const CUtensorMap& tmap, int grid, int cs, cudaStream_t st) {
   constexpr int Z = SK_TMEM_ZETA, N = 64 * X * S;
   if constexpr (Z % BQ != 0) {
     return cudaErrorInvalidValue;
   } else {
-    auto k = k_tmem<Z, X, S, BQ, NW>;
-    const size_t smem = tmem_smem_bytes(Z, N);
+    auto k = k_tmem<Z, X, S, BQ, NW, GM>;
+    const size_t smem = tmem_smem_bytes(Z, N, BQ, GM);
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k<<<dim3((unsigned)grid, (unsigned)cs), (NW + 1) * 32, smem, st>>>(g, tmap);
+    k<<<dim3((unsigned)grid, (unsigned)cs), (NW + tmem_producers(N, BQ, GM)) * 32, smem, st>>>(g, tmap);
     return cudaGetLastError();
   }
 }
@@ -31,24 +32,24 @@ cudaError_t go(const TmemArgs& g, const CUtensorMap& tmap, int grid, int cs, cud
 cudaError_t dispatch(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st) {
   if (h.NW == 4) {
     switch (h.X * 100 + h.S * 10 + h.BQ) {
-      case 111: return go<1, 1, 1, 4>(g, tmap, grid, h.CS, st);
-      case 121: return go<1, 2, 1, 4>(g, tmap, grid, h.CS, st);
-      case 141: return go<1, 4, 1, 4>(g, tmap, grid, h.CS, st);
-      case 211: return go<2, 1, 1, 4>(g, tmap, grid, h.CS, st);
-      case 221: return go<2, 2, 1, 4>(g, tmap, grid, h.CS, st);
-      case 241: return go<2, 4, 1, 4>(g, tmap, grid, h.CS, st);
-      case 411: return go<4, 1, 1, 4>(g, tmap, grid, h.CS, st);
-      case 421: return go<4, 2, 1, 4>(g, tmap, grid, h.CS, st);
-      case 441: return go<4, 4, 1, 4>(g, tmap, grid, h.CS, st);
-      case 112: return go<1, 1, 2, 4>(g, tmap, grid, h.CS, st);
-      case 122: return go<1, 2, 2, 4>(g, tmap, grid, h.CS, st);
-      case 212: return go<2, 1, 2, 4>(g, tmap, grid, h.CS, st);
-      case 222: return go<2, 2, 2, 4>(g, tmap, grid, h.CS, st);
-      case 412: return go<4, 1, 2, 4>(g, tmap, grid, h.CS, st);
-      case 422: return go<4, 2, 2, 4>(g, tmap, grid, h.CS, st);
-      case 114: return go<1, 1, 4, 4>(g, tmap, grid, h.CS, st);
-      case 214: return go<2, 1, 4, 4>(g, tmap, grid, h.CS, st);
-      case 414: return go<4, 1, 4, 4>(g, tmap, grid, h.CS, st);
+      case 111: return go<1, 1, 1, 4, 0>(g, tmap, grid, h.CS, st);
+      case 121: return go<1, 2, 1, 4, 0>(g, tmap, grid, h.CS, st);
+      case 141: return go<1, 4, 1, 4, 0>(g, tmap, grid, h.CS, st);
+      case 211: return go<2, 1, 1, 4, 0>(g, tmap, grid, h.CS, st);
+      case 221: return go<2, 2, 1, 4, 0>(g, tmap, grid, h.CS, st);
+      case 241: return go<2, 4, 1, 4, 0>(g, tmap, grid, h.CS, st);
+      case 411: return go<4, 1, 1, 4, 0>(g, tmap, grid, h.CS, st);
+      case 421: return go<4, 2, 1, 4, 0>(g, tmap, grid, h.CS, st);
+      case 441: return go<4, 4, 1, 4, 0>(g, tmap, grid, h.CS, st);
+      case 112: return h.GM == 1 ? go<1, 1, 2, 4, 1>(g, tmap, grid, h.CS, st) : h.GM == 2 ? go<1, 1, 2, 4, 2>(g, tmap, grid, h.CS, st) : go<1, 1, 2, 4, 0>(g, tmap, grid, h.CS, st);
+      case 122: return h.GM == 1 ? go<1, 2, 2, 4, 1>(g, tmap, grid, h.CS, st) : h.GM == 2 ? go<1, 2, 2, 4, 2>(g, tmap, grid, h.CS, st) : go<1, 2, 2, 4, 0>(g, tmap, grid, h.CS, st);
+      case 212: return h.GM == 1 ? go<2, 1, 2, 4, 1>(g, tmap, grid, h.CS, st) : h.GM == 2 ? go<2, 1, 2, 4, 2>(g, tmap, grid, h.CS, st) : go<2, 1, 2, 4, 0>(g, tmap, grid, h.CS, st);
+      case 222: return h.GM == 1 ? go<2, 2, 2, 4, 1>(g, tmap, grid, h.CS, st) : h.GM == 2 ? go<2, 2, 2, 4, 2>(g, tmap, grid, h.CS, st) : go<2, 2, 2, 4, 0>(g, tmap, grid, h.CS, st);
+      case 412: return h.GM == 1 ? go<4, 1, 2, 4, 1>(g, tmap, grid, h.CS, st) : h.GM == 2 ? go<4, 1, 2, 4, 2>(g, tmap, grid, h.CS, st) : go<4, 1, 2, 4, 0>(g, tmap, grid, h.CS, st);
+      case 422: return h.GM == 1 ? go<4, 2, 2, 4, 1>(g, tmap, grid, h.CS, st) : h.GM == 2 ? go<4, 2, 2, 4, 2>(g, tmap, grid, h.CS, st) : go<4, 2, 2, 4, 0>(g, tmap, grid, h.CS, st);
+      case 114: return h.GM == 1 ? go<1, 1, 4, 4, 1>(g, tmap, grid, h.CS, st) : h.GM == 2 ? go<1, 1, 4, 4, 2>(g, tmap, grid, h.CS, st) : go<1, 1, 4, 4, 0>(g, tmap, grid, h.CS, st);
+      case 214: return h.GM == 1 ? go<2, 1, 4, 4, 1>(g, tmap, grid, h.CS, st) : h.GM == 2 ? go<2, 1, 4, 4, 2>(g, tmap, grid, h.CS, st) : go<2, 1, 4, 4, 0>(g, tmap, grid, h.CS, st);
+      case 414: return h.GM == 1 ? go<4, 1, 4, 4, 1>(g, tmap, grid, h.CS, st) : h.GM == 2 ? go<4, 1, 4, 4, 2>(g, tmap, grid, h.CS, st) : go<4, 1, 4, 4, 0>(g, tmap, grid, h.CS, st);
     }
   }
   return cudaErrorInvalidValue;
@@ -90,6 +91,15 @@ bool tmem_shape(int n, int d, int zeta, TmemShape* out) {
           found = true;
           best = cost;
           out->X = x; out->S = s; out->BQ = bq; out->CS = cs; out->NW = NW;
+          // group mode (kernel_tmem.cuh): deferral with groups of 8 / 4 rows where few groups hold two rows with one
+          // sketch row -- expected deferred rows per group ZB * C(G,2) / (d/zeta) <= 0.15 -- and substitutes exist
+          // (d/zeta >= G (G+1)); only the bucket-group kernels have it.  Else chained groups.
+          const double zb = (double)zeta / bq, dbk = (double)d / zeta;
+          out->GM = bq == 1 ? 0 : (zb * 28.0 / dbk <= 0.15 && dbk >= 72) ? 2 : (zb * 6.0 / dbk <= 0.15 && dbk >= 20) ? 1 : 0;
+          if (const char* ev = getenv("SK_TMEM_GM")) {   // experiments only
+            const int gm = atoi(ev);
+            if (bq > 1 && (gm == 0 || (gm == 1 && dbk >= 20) || (gm == 2 && dbk >= 72))) out->GM = gm;
+          }
         }
       }
     }
@@ -98,7 +108,7 @@ bool tmem_shape(int n, int d, int zeta, TmemShape* out) {
   return false;
 }
 
-size_t tmem_smem_bytes_for(int zeta, int n_cta) { return tmem_smem_bytes(zeta, n_cta); }
+size_t tmem_smem_bytes_for(int zeta, int n_cta, int bq, int gm) { return tmem_smem_bytes(zeta, n_cta, bq, gm); }
 int tmem_rows_per_stage(int n_cta) { return tmem_stage_rows(n_cta); }
 
 // 2-D tensor map over the row range: {n features, rows} FP32, row pitch lda, box {n / CS features, T rows}

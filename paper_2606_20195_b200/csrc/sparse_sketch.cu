@@ -115,7 +115,7 @@ bool tmem_feasible(const sketch* s, int n, int64_t lda, const void* A, const voi
   if (!zeta_templated(s->zeta)) return false;
   if (!sk::tmem_shape(n, s->d, s->zeta, h)) return false;
   if (lda % 4 != 0 || !aligned(A, 16) || !aligned(B, 16)) return false;  // TMA bulk copies: 16-byte granules
-  return sk::tmem_smem_bytes_for(s->zeta, n / h->CS) <= (size_t)s->smem_optin;
+  return sk::tmem_smem_bytes_for(s->zeta, n / h->CS, h->BQ, h->GM) <= (size_t)s->smem_optin;
 }
 
 int flat_vec_for(bool f16, int n, int64_t lda, const void* A, const void* B, int want_max) {
@@ -147,7 +147,7 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
   const int64_t rb0 = o ? o->row_begin : 0;
   bool sm_ok = f16 && rounding == SKETCH_RN && smem_feasible(s, n, lda, A, B, &sm_bytes) &&
                (rb0 % sk::smem_step_rows(s->zeta) == 0);
-  sk::TmemShape tm = {0, 0, 0, 0, 0};
+  sk::TmemShape tm = {0, 0, 0, 0, 0, 0};
   bool tm_ok = f16 && rounding == SKETCH_RN && tmem_feasible(s, n, lda, A, B, &tm);
   int vmax = flat_vec_for(f16, n, lda, A, B, 8);
   int vpair = flat_vec_for(f16, n, lda, A, B, f16 ? 2 : 1);
@@ -177,7 +177,7 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
     p->replicas = 1;
     p->tm = tm;
     p->wpc = tm.NW + 1;
-    p->smem_bytes = sk::tmem_smem_bytes_for(s->zeta, n / tm.CS);
+    p->smem_bytes = sk::tmem_smem_bytes_for(s->zeta, n / tm.CS, tm.BQ, tm.GM);
     const int T = sk::tmem_rows_per_stage(n / tm.CS);
     int64_t stages = (rows + T - 1) / T;
     // one CTA per SM (it owns all 512 TMEM columns); gridDim.y = CS column slices share a row range
