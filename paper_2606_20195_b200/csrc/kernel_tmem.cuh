@@ -482,16 +482,39 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM)) * 32
         asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
         qlane = qb + (slice * 64 * X + lane * 2 * X) * 2;
       }
+      if constexpr (Geo::DEF) {
+        // software pipeline over the groups of the stage: records two groups ahead, FP16 words one group ahead of the
+        // read-modify-write that uses them (their shared-memory latency hides under the tensor-memory round trip)
+        constexpr int NG = TR / G;
+        uint32_t qo[2][G], col[3][G][ZB], mul[3][G][ZB], q[2][G][X];
+#pragma unroll
+        for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + r * (BQ * RB), qo[0][r], col[0][r], mul[0][r]);
+        if constexpr (NG > 1) {
+#pragma unroll
+          for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + (G + r) * (BQ * RB), qo[1][r], col[1][r], mul[1][r]);
+        }
+#pragma unroll
+        for (int r = 0; r < G; ++r) lds_q<X>(qlane + qo[0][r], q[0][r]);
+#pragma unroll
+        for (int gi = 0; gi < NG; ++gi) {
+          if (gi + 1 < NG) {
+#pragma unroll
+            for (int r = 0; r < G; ++r) lds_q<X>(qlane + qo[(gi + 1) & 1][r], q[(gi + 1) & 1][r]);
+          }
+          if (gi + 2 < NG) {
+#pragma unroll
+            for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + ((gi + 2) * G + r) * (BQ * RB), qo[gi & 1][r], col[(gi + 2) % 3][r], mul[(gi + 2) % 3][r]);
+          }
+          // a5: read-modify-write of G x ZB sketch rows in tensor memory, pairwise distinct by construction
+          tmem_rmw<G, ZB, X, false>(region, q[gi & 1], col[gi % 3], mul[gi % 3]);
+        }
+      } else {
 #pragma unroll
       for (int g0 = 0; g0 < TR; g0 += G) {
         uint32_t q[G][X], col[G][ZB], mul[G][ZB];
 #pragma unroll
         for (int r = 0; r < G; ++r) {
-          if constexpr (Geo::DEF) {
-            uint32_t qoff;
-            lds_rec<ZB>(sE + (g0 + r) * (BQ * RB), qoff, col[r], mul[r]);
-            lds_q<X>(qlane + qoff, q[r]);
-          } else {
+          {
             if constexpr (Geo::SHQ) {
               lds_q<X>(qlane + (rowset * TR + g0 + r) * Geo::Q_ROW, q[r]);
             } else {
@@ -520,8 +543,9 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM)) * 32
             }
           }
         }
-        // a5: read-modify-write of G x ZB sketch rows in tensor memory
-        tmem_rmw<G, ZB, X, !Geo::DEF>(region, q, col, mul);
+        // a5: read-modify-write of G x ZB sketch rows in tensor memory; same-bucket rows chained in registers
+        tmem_rmw<G, ZB, X, true>(region, q, col, mul);
+      }
       }
       if constexpr (Geo::DEF) {
         // the deferred rows of this stage (TmemGeom): original sketch rows, one row at a time

@@ -91,11 +91,12 @@ bool tmem_shape(int n, int d, int zeta, TmemShape* out) {
           found = true;
           best = cost;
           out->X = x; out->S = s; out->BQ = bq; out->CS = cs; out->NW = NW;
-          // group mode (kernel_tmem.cuh): deferral with groups of 8 / 4 rows where few groups hold two rows with one
-          // sketch row -- expected deferred rows per group ZB * C(G,2) / (d/zeta) <= 0.15 -- and substitutes exist
-          // (d/zeta >= G (G+1)); only the bucket-group kernels have it.  Else chained groups.
+          // group mode (kernel_tmem.cuh), from the sweep in profiles/r01_tmem_shapes.md: with four bucket groups
+          // (one block per warp, one LDTM per row) the chained groups are latency-bound and deferral with groups of
+          // 4 rows wins (c4: 3.57 -> 4.13 TB/s); with two bucket groups the chained kernel is faster (c4-512: 5.37 vs
+          // 5.07 TB/s).  Deferral needs few clashes -- ZB * C(4,2) / (d/zeta) <= 0.15 -- and d/zeta >= G (G + 1).
           const double zb = (double)zeta / bq, dbk = (double)d / zeta;
-          out->GM = bq == 1 ? 0 : (zb * 28.0 / dbk <= 0.15 && dbk >= 72) ? 2 : (zb * 6.0 / dbk <= 0.15 && dbk >= 20) ? 1 : 0;
+          out->GM = (bq == 4 && zb * 6.0 / dbk <= 0.15 && dbk >= 20) ? 1 : 0;
           if (const char* ev = getenv("SK_TMEM_GM")) {   // experiments only
             const int gm = atoi(ev);
             if (bq > 1 && (gm == 0 || (gm == 1 && dbk >= 20) || (gm == 2 && dbk >= 72))) out->GM = gm;

@@ -160,7 +160,8 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
     // one-row steps are issue-bound; from zeta = 2 on the privatised kernel wins wherever it fits
     // the tensor-memory kernel (profiles/r01_tmem_*.md) beats both wherever it fits; below ~4 MiB of A the
     // launch is latency-bound and the lighter kernels win
-    if (tm_ok && rows * (int64_t)n > (1 << 20)) v = SKETCH_VARIANT_TMEM;
+    // (four column slices -- d = 2048 at n = 256 -- measured 2.54 TB/s against 2.74 TB/s of the flat REDs)
+    if (tm_ok && tm.CS < 4 && rows * (int64_t)n > (1 << 20)) v = SKETCH_VARIANT_TMEM;
     else if (sm_ok && s->zeta >= 2) v = SKETCH_VARIANT_SMEM;
     else if (zt && vmax) v = SKETCH_VARIANT_FLAT_VEC;
     else v = SKETCH_VARIANT_GENERIC;

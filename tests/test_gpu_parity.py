@@ -295,7 +295,8 @@ def test_tmem_column_slices_row_ranges_accumulate_and_lda(ss, d):
     seed = sketch_seed(56 + d)
     want = oracle.f64_sketch(seed, d, zeta, A)
     sk = ss.Sketch(m, d, zeta, seed)
-    assert sk.plan(n)["variant"] == "tmem"
+    # AUTO: tensor memory up to two column slices; four (d = 2048) measured slower than the flat 16-byte REDs
+    assert sk.plan(n)["variant"] == ("tmem" if d <= 1024 else "flat_vec")
     Ap = torch.full((m, n + 12), float("nan"), device="cuda")
     Ap[:, :n] = dev(A)
     out = None
