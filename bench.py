@@ -38,7 +38,12 @@ WORKLOADS = {
     "c3-z2": (1 << 22, 128, 256, 2, 2),
     "c3-z8": (1 << 22, 128, 256, 8, 2),
     "c5": (1 << 25, 128, 256, 4, 4),
+    # the paper's own headline point (Fig. 2): m = 2^21, n = 1024, d = 2n, zeta = 4, dense input;
+    # BASELINE.md holds its H200 number for exactly this workload (7.11 ms complete sketch = 1208 GB/s of A)
+    "e1": (1 << 21, 1024, 2048, 4, 5),
 }
+PAPER_GBPS = {"e1": (1 << 21) * 1024 * 4 / 7.11e-3 / 1e9}   # PAPER.md:322, H200 NVL (another machine: context)
+L2_RED_PAYLOAD_GBPS = 6000.0   # measured with sketch_red_probe on this pool's B200 (profiles/r01_red_probe.md)
 VARIANTS = {"auto": 0, "flat_pair": 1, "flat_vec": 2, "smem": 3, "generic": 4, "tmem": 5}
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
@@ -337,7 +342,8 @@ def run_ours(args):
     red_ops = zeta * m * n // 2
     line = {
         "metric": "sketch_A_read_GBps", "value": gbs, "unit": "GB/s", "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms16, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "warmup": args.warmup, "ms_per_step": ms16, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": (gbs / world / PAPER_GBPS[args.workload]) if args.workload in PAPER_GBPS else None,
         "dtype": "f16", "data": "synthetic",
         "config": {"workload": "%s: SparseStack zeta=%d, m=%d, n=%d, d=%d (d=2n), A FP32 row-major N(0,1) %.2f GiB per GPU, FP16-RN accumulate"
                                % (args.workload, zeta, m, n, d, m * n * 4 / 2**30),
@@ -362,6 +368,12 @@ def run_ours(args):
         "per_step_ms": per16,
         "paper_context": "H200 NVL (PAPER.md:320-322): FP16 SS zeta=4 7.11 ms for 8 GiB (1.21 TB/s), up to 1.91x its FP32 scatter",
     }
+    if plan16["variant"] in ("flat_vec", "flat_pair", "generic"):
+        # a flat scatter is bound by the L2 atomic units, not by HBM: 2 bytes of RED payload per contribution
+        payload = 2.0 * zeta * m * n / (ms16_apply * 1e-3) / 1e9
+        line["roofline"]["l2_atomic"] = {"achieved": payload, "peak": L2_RED_PAYLOAD_GBPS, "unit": "GB/s of RED payload",
+                                         "frac": payload / L2_RED_PAYLOAD_GBPS,
+                                         "note": "second roofline term (SURVEY 8d): the slower of HBM and L2-atomic bounds this variant"}
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(args.workload)
     print(json.dumps(line))
