@@ -443,3 +443,60 @@ def test_overflow_saturates_like_the_oracle(ss):
             assert not np.isnan(got).any()
         fin = np.isfinite(got)
         assert fin.sum() > 0 and ev.rel_fro(got[fin], B[fin]) < 0.2
+
+
+# ------------------------------------------------------------------------------------ full sizes
+# BASELINE.json's full shapes in the launch configuration bench.py times (AUTO through the C ABI, resident input).
+# The oracle cannot redo 16 GiB in seconds, so it recomputes SAMPLED COLUMNS of the sketch (S acts on every column
+# independently: column c of S A is S applied to column c of A) from the same bytes, copied back from the device.
+FULL_SIZES = [
+    # (name, m, n, d, zeta, expected AUTO variant)
+    ("c5", 1 << 25, 128, 256, 4, "tmem"),
+    ("c4-512", 1 << 23, 256, 512, 4, "tmem"),
+    ("c4", 1 << 23, 256, 1024, 4, "tmem"),
+    ("c4-2048", 1 << 23, 256, 2048, 4, "flat_vec"),
+    ("c3", 1 << 22, 128, 256, 4, "tmem"),
+]
+
+
+def _sample_cols(n):
+    # both halves of a half2 pair, lane and warp / column-slice boundaries, the last pair
+    c = sorted({0, 1, 62, 63, 64, 65, n // 2 - 1, n // 2, n - 2, n - 1})
+    return [x for x in c if 0 <= x < n]
+
+
+@pytest.mark.parametrize("name,m,n,d,zeta,variant", FULL_SIZES)
+def test_full_size_sampled_columns(ss, name, m, n, d, zeta, variant):
+    free, _ = torch.cuda.mem_get_info()
+    if free < m * n * 4 * 1.3:
+        pytest.skip("not enough device memory for %s" % name)
+    seed = sketch_seed(900 + d)
+    sk = ss.Sketch(m, d, zeta, seed)
+    assert sk.plan(n)["variant"] == variant
+    cols = _sample_cols(n)
+    threads = min(32, __import__("os").cpu_count() or 1)
+    # (1) integer-valued sparse input: every FP16 partial sum exact in any order -> bit-exact on the sampled columns,
+    #     FP16 and FP32 paths; the unsampled columns must at least agree between the two GPU paths exactly
+    A = wl.sparse_signs_device(m, n, 31, torch.device("cuda"))
+    got16 = sk.apply_f16acc(A)
+    got32 = sk.apply_f32acc(A)
+    Ac = np.ascontiguousarray(A[:, cols].cpu().numpy())
+    want = oracle.f64_sketch(seed, d, zeta, Ac, threads=threads)
+    assert np.abs(want).max() < 1024
+    assert np.array_equal(oracle.half_bits_to_f64(bits(got16[:, cols])), want)
+    assert np.array_equal(got32[:, cols].cpu().numpy().astype(np.float64), want)
+    assert bool((got16.float() == got32).all())
+    del got16, got32
+    # (2) Gaussian input: north-star ceilings on the sampled columns
+    A.normal_(generator=torch.Generator(device="cuda").manual_seed(32))
+    got16 = sk.apply_f16acc(A)
+    got32 = sk.apply_f32acc(A)
+    Ac = np.ascontiguousarray(A[:, cols].cpu().numpy())
+    B = oracle.f64_sketch(seed, d, zeta, Ac, threads=threads)
+    r16 = ev.rel_fro(oracle.half_bits_to_f64(bits(got16[:, cols])), B)
+    r32 = ev.rel_fro(got32[:, cols].cpu().numpy(), B)
+    print("%s: relF f16 %.3e, f32 %.3e on %d sampled columns" % (name, r16, r32, len(cols)))
+    assert r32 <= 1e-5, r32
+    # FP16: never above 5e-2 (north star).  The flat kernel keeps one running sum per entry and replica, the
+    # privatised kernels a two-level hierarchy; both stay far below at these depths (L = 2^14 .. 2^19)
+    assert r16 <= 5e-2, r16

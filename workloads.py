@@ -106,6 +106,22 @@ def integer_valued_device(m: int, n: int, seed: int, device, lo: int = -3, hi: i
     return torch.randint(lo, hi + 1, (m, n), generator=g, device=device).to(torch.float32)
 
 
+def sparse_signs_device(m: int, n: int, seed: int, device, density: float = 1.0 / 64, chunk_rows: int = 1 << 22):
+    """Entries +-1 with probability `density`, else 0, FP32 [m, n] on `device`: integer-valued AND sparse, so that the
+    sums of even 2^19-deep buckets stay far below 1024 and every FP16 partial sum is exact in any order."""
+    import torch
+
+    g = torch.Generator(device=device)
+    g.manual_seed(seed)
+    A = torch.empty((m, n), dtype=torch.float32, device=device)
+    for r0 in range(0, m, chunk_rows):
+        r1 = min(m, r0 + chunk_rows)
+        u = torch.rand((r1 - r0, n), generator=g, device=device)
+        A[r0:r1] = (u < density / 2).to(torch.float32) - (u > 1.0 - density / 2).to(torch.float32)
+        del u
+    return A
+
+
 def heavy_rows_device(m: int, n: int, alpha: float, seed: int, device):
     import torch
 
