@@ -382,6 +382,68 @@ def run_ours(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------- range study
+def run_range_study(args):
+    """BASELINE.json configs[4] (Fig. 7): A = N(0,1) * 2^k, k in {-24,-16,0,+8,+12}, RN vs SR.
+    Per (k, rounding): sketch GB/s at the workload's full size, non-finite outputs, error against the FP64 oracle on
+    sampled columns (entries finite in both, R18), and the oracle's per-contribution range counts on a row
+    sample.  One JSON line; not the driver's bench line."""
+    import numpy as np
+    import torch
+
+    import evaluation as ev
+    import oracle
+    import paper_2606_20195_b200 as ss
+    import workloads as wl
+
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    m, n, d, zeta, mseed = WORKLOADS[args.workload]
+    seed = wl.sketch_seed(0)
+    sk = ss.Sketch(m, d, zeta, seed)
+    A = wl.gaussian_device(m, n, mseed, dev)
+    cols = sorted({0, 1, n // 2 - 1, n // 2, n - 2, n - 1})
+    threads = min(os.cpu_count() or 1, 64)
+    oracle.build()
+    B0 = oracle.f64_sketch(seed, d, zeta, np.ascontiguousarray(A[:, cols].cpu().numpy()), threads=threads)  # k = 0; S(2^k A) = 2^k S A exactly
+    sample = np.ascontiguousarray(A[: 1 << 16].cpu().numpy())
+    out = torch.empty((d, n), dtype=torch.float16, device=dev)
+    rows_out, prev = [], 0
+    for k in (-24, -16, 0, 8, 12):
+        A.mul_(float(2.0 ** (k - prev)))      # exact in FP32
+        prev = k
+        counts = oracle.range_counts(zeta, sample * np.float32(2.0 ** k))
+        for rname, rmode in (("RN", ss.RN), ("SR", ss.SR)):
+            kw = dict(out=out, rounding=rmode, sr_seed=wl.sketch_seed(77))
+            for _ in range(2):
+                sk.apply_f16acc(A, **kw)
+            torch.cuda.synchronize()
+            reps = 5 if rmode == ss.RN else 2
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(reps):
+                sk.apply_f16acc(A, **kw)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / reps
+            got = out[:, cols].float().cpu().numpy().astype(np.float64)
+            want = B0 * 2.0 ** k
+            fin = np.isfinite(got)
+            rel = ev.rel_fro(got[fin], want[fin]) if fin.any() else None
+            rows_out.append({
+                "k": k, "rounding": rname, "variant": sk.plan(n, rounding=rmode)["variant"], "ms": ms,
+                "GBps": m * n * 4 / (ms * 1e-3) / 1e9,
+                "nonfinite_outputs": int((~torch.isfinite(out)).sum().item()), "nan_outputs": int(torch.isnan(out).sum().item()),
+                "zero_outputs": int((out == 0).sum().item()), "outputs": d * n,
+                "relF_vs_f64_sampled_cols_finite": rel,
+                "oracle_contribution_counts_first_65536_rows": {kk: int(v) for kk, v in counts.items()},
+            })
+    A.mul_(float(2.0 ** (-prev)))
+    print(json.dumps({"study": "range (BASELINE.json configs[4])", "workload": "%s: m=%d n=%d d=%d zeta=%d, N(0,1) * 2^k" % (args.workload, m, n, d, zeta),
+                      "sampled_columns": cols, "rows": rows_out}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -392,6 +454,7 @@ def main():
     ap.add_argument("--variant", default="auto", choices=sorted(VARIANTS))
     ap.add_argument("--replicas", type=int, default=0)
     ap.add_argument("--hash-mode", type=int, default=0)
+    ap.add_argument("--study", default=None, choices=["range"], help="extra report: config-5 range / rounding study")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-rows", type=int, default=1 << 21, help="rows per step of the reference arm's bounded sample")
@@ -400,6 +463,8 @@ def main():
         args.warmup = 3                           # timing rule: W >= 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.study == "range":
+        return run_range_study(args)
     return run_ours(args)
 
 
