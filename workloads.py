@@ -82,6 +82,32 @@ def ls_system(m: int, n: int, seed: int, sigma_min: float = 1e-4, noise: float =
     return A, b, xstar
 
 
+def ls_paper_low_coherence(m: int, n: int, seed: int):
+    """The paper's low-coherence least-squares family: singular values decreasing linearly from 100 to 1,
+    b = A 1 + nu, nu_i ~ N(0, 0.1^2).  Built as A = (G / sqrt(m)) diag(sigma): for m >> n the Gaussian factor has
+    nearly orthonormal columns, so the singular values are sigma up to O(sqrt(n/m))."""
+    rng = np.random.default_rng(seed)
+    sigma = np.linspace(100.0, 1.0, n)
+    A = (rng.standard_normal((m, n), dtype=np.float32) * (sigma / np.sqrt(m)).astype(np.float32)[None, :]).astype(np.float32)
+    b = (A.astype(np.float64) @ np.ones(n) + 0.1 * rng.standard_normal(m)).astype(np.float32)
+    return A, b
+
+
+def ls_paper_coherent(m: int, n: int, seed: int):
+    """The paper's coherent family: A = [I_n; T], T = 1e-3 G / sqrt(m - n), b = [x0 + nu; T x0] with
+    Gaussian G, x0, head noise nu_i ~ N(0, 0.5^2), and a common row permutation."""
+    rng = np.random.default_rng(seed)
+    A = np.empty((m, n), dtype=np.float32)
+    A[:n] = np.eye(n, dtype=np.float32)
+    A[n:] = rng.standard_normal((m - n, n), dtype=np.float32) * np.float32(1e-3 / np.sqrt(m - n))
+    x0 = rng.standard_normal(n)
+    b = np.empty(m, dtype=np.float64)
+    b[:n] = x0 + 0.5 * rng.standard_normal(n)
+    b[n:] = A[n:].astype(np.float64) @ x0
+    pi = rng.permutation(m)
+    return np.ascontiguousarray(A[pi]), b[pi].astype(np.float32)
+
+
 # ----------------------------------------------------------------------------- torch (device)
 def gaussian_device(m: int, n: int, seed: int, device, pow2: int = 0, chunk_rows: int = 1 << 22):
     """N(0,1) FP32 [m, n] generated on `device` in row chunks (no 2x peak memory)."""
