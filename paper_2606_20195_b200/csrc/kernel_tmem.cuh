@@ -130,8 +130,9 @@ SK_DEVINL uint32_t hfma2_u32(uint32_t q, uint32_t mult, uint32_t acc) {
 }
 
 // ---------------------------------------------------------------------------------------- geometry
-// rows per stage: 32 KiB of A per stage (16 KiB at n = 64), at least 16 rows
-__host__ __device__ constexpr int tmem_stage_rows(int n) { return n <= 128 ? 64 : n == 256 ? 32 : 16; }
+// rows per stage: 32 KiB of A per stage, at least 16 rows (4 stages x 32 KiB x 148 SMs = 19 MB in flight; with 16 KiB
+// stages at n = 64 the consumers waited for data 36 % of their time, profiles/r01_tmem_shapes.md)
+__host__ __device__ constexpr int tmem_stage_rows(int n) { return n <= 64 ? 128 : n <= 128 ? 64 : n == 256 ? 32 : 16; }
 __host__ __device__ constexpr int tmem_stages(int n) { return n <= 512 ? 4 : 3; }
 // bytes of one (row, bucket group) record / side-list item of the deferral modes: {q offset | row, 0, then (col, mul) x ZB}
 __host__ __device__ constexpr int tmem_rec_bytes(int zb) { return zb == 1 ? 16 : 16 + 8 * zb; }
@@ -163,10 +164,10 @@ struct TmemGeom {
   // bucket group) a side list of up to T items of RB bytes, then the NPC * BQ item counts.
   static constexpr int RB = tmem_rec_bytes(ZB);
   static constexpr int E_BYTES = DEF ? T * BQ * RB : T * ZETA * 8;
-  // producer warps: one in the chained modes; the deferral bookkeeping triples the hash stage's work, so there the
+  // producer warps: one in the chained modes (two at n = 64); the deferral bookkeeping triples the hash stage's work, so there the
   // stage's 32-row chunks go to NPC warps and the bucket groups of a chunk to NPB warps
   static constexpr int CH = (T + 31) / 32;
-  static constexpr int NPC = DEF ? (CH >= 2 ? 2 : 1) : 1;
+  static constexpr int NPC = DEF ? (CH >= 2 ? 2 : 1) : (CH >= 4 ? 2 : 1);   // n = 64: 4 hashes per 256 B of A, two hash warps
   static constexpr int NPB = DEF ? (BQ < 4 / NPC ? BQ : 4 / NPC) : 1;
   static constexpr int NP = NPC * NPB;
   static constexpr int L_BYTES = DEF ? NPC * BQ * T * RB + 128 : 0;
@@ -182,7 +183,8 @@ struct TmemGeom {
 };
 
 __host__ __device__ constexpr int tmem_producers(int n, int bq, int gm) {
-  return gm == 0 ? 1 : (tmem_stage_rows(n) >= 64 ? 2 : 1) * (bq < (tmem_stage_rows(n) >= 64 ? 2 : 4) ? bq : (tmem_stage_rows(n) >= 64 ? 2 : 4));
+  return gm == 0 ? (tmem_stage_rows(n) >= 128 ? 2 : 1)
+                 : (tmem_stage_rows(n) >= 64 ? 2 : 1) * (bq < (tmem_stage_rows(n) >= 64 ? 2 : 4) ? bq : (tmem_stage_rows(n) >= 64 ? 2 : 4));
 }
 // ring of stages | barriers + TMEM base (256 B) | with bucket groups: two converted (FP16) tiles | deferral: 2 KiB of
 // producer scratch (the sketch rows of a 32-row chunk, one 128-byte line per producer warp and block)
