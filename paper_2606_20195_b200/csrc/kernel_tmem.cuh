@@ -132,7 +132,8 @@ SK_DEVINL uint32_t hfma2_u32(uint32_t q, uint32_t mult, uint32_t acc) {
 // ---------------------------------------------------------------------------------------- geometry
 // rows per stage: 32 KiB of A per stage, at least 16 rows (4 stages x 32 KiB x 148 SMs = 19 MB in flight; with 16 KiB
 // stages at n = 64 the consumers waited for data 36 % of their time, profiles/r01_tmem_shapes.md)
-__host__ __device__ constexpr int tmem_stage_rows(int n) { return n <= 64 ? 128 : n <= 128 ? 64 : n == 256 ? 32 : 16; }
+// (bucket-group kernels keep 64 rows at n = 64: their records, side lists and FP16 tiles fill the rest of shared memory)
+__host__ __device__ constexpr int tmem_stage_rows(int n, int bq) { return n <= 64 ? (bq == 1 ? 128 : 64) : n <= 128 ? 64 : n == 256 ? 32 : 16; }
 __host__ __device__ constexpr int tmem_stages(int n) { return n <= 512 ? 4 : 3; }
 // bytes of one (row, bucket group) record / side-list item of the deferral modes: {q offset | row, 0, then (col, mul) x ZB}
 __host__ __device__ constexpr int tmem_rec_bytes(int zb) { return zb == 1 ? 16 : 16 + 8 * zb; }
@@ -155,6 +156,7 @@ struct TmemGeom {
   static constexpr int RS = NW / (S * BQ);     // row-sets per stage
   static constexpr int TR = T / RS;            // rows of a stage one warp processes
   static constexpr bool DEF = GM != 0;
+  static constexpr bool ABS = S == 1 && BQ == 1;   // entries hold absolute tensor-memory addresses (see the producer)
   static constexpr int G = GM == 1 ? 4 : GM == 2 ? 8 : (ZB >= 4 || (BQ > 1 && ZB >= 2)) ? 2 : 4;  // rows per group (LDTMs in flight = G * ZB)
   static_assert(TR % G == 0 && 32 % G == 0, "whole groups");
   static constexpr int N = 64 * X * S;         // features of the CTA's column slice
@@ -183,13 +185,13 @@ struct TmemGeom {
 };
 
 __host__ __device__ constexpr int tmem_producers(int n, int bq, int gm) {
-  return gm == 0 ? (tmem_stage_rows(n) >= 128 ? 2 : 1)
-                 : (tmem_stage_rows(n) >= 64 ? 2 : 1) * (bq < (tmem_stage_rows(n) >= 64 ? 2 : 4) ? bq : (tmem_stage_rows(n) >= 64 ? 2 : 4));
+  return gm == 0 ? (tmem_stage_rows(n, bq) >= 128 ? 2 : 1)
+                 : (tmem_stage_rows(n, bq) >= 64 ? 2 : 1) * (bq < (tmem_stage_rows(n, bq) >= 64 ? 2 : 4) ? bq : (tmem_stage_rows(n, bq) >= 64 ? 2 : 4));
 }
 // ring of stages | barriers + TMEM base (256 B) | with bucket groups: two converted (FP16) tiles | deferral: 2 KiB of
 // producer scratch (the sketch rows of a 32-row chunk, one 128-byte line per producer warp and block)
 constexpr size_t tmem_smem_bytes(int zeta, int n, int bq, int gm) {
-  const size_t t = (size_t)tmem_stage_rows(n);
+  const size_t t = (size_t)tmem_stage_rows(n, bq);
   const size_t rb = (size_t)tmem_rec_bytes(zeta / bq);
   const size_t e = gm ? t * bq * rb + 2 * bq * t * rb + 128 : t * zeta * 8;
   return (size_t)tmem_stages(n) * (t * n * 4 + e) + 256 + (bq > 1 ? 2 * (t * n * 2 + (gm ? (size_t)n * 2 : 0)) : 0) + (gm ? 2048 : 0);
@@ -278,7 +280,7 @@ template <int ZB> SK_DEVINL void sts_rec(uint32_t p, uint32_t head, const uint32
 // ---------------------------------------------------------------------------------------- the kernel
 template <int ZETA, int X, int S, int BQ, int NW, int GM>
 __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM)) * 32, 1) k_tmem(TmemArgs g, const __grid_constant__ CUtensorMap tmap) {
-  constexpr int T = tmem_stage_rows(64 * X * S), NS = tmem_stages(64 * X * S);
+  constexpr int T = tmem_stage_rows(64 * X * S, BQ), NS = tmem_stages(64 * X * S);
   using Geo = TmemGeom<ZETA, X, S, BQ, NW, GM, T>;
   constexpr int TR = Geo::TR, G = Geo::G, N = Geo::N, ZB = Geo::ZB, RB = Geo::RB, NP = Geo::NP, NPC = Geo::NPC, NPB = Geo::NPB;
   static_assert(NP == tmem_producers(N, BQ, GM), "producer warps");
@@ -367,16 +369,20 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM)) * 32
           mulw[j] = 0x3C003C00u ^ entry_signmask_h2(e);
         }
         if constexpr (!Geo::DEF) {
-          // entries {(bucket - first sketch row of the block's group) * X, multiplier}
+          // entries {(bucket - first sketch row of the block's group) * X, multiplier}.  With one slice and one bucket
+          // group a row is read by exactly one consumer warp (its row-set), so the entry carries that warp's complete
+          // tensor-memory address and the consumer saves an add per (row, block)
+          const uint32_t rw = Geo::ABS ? (uint32_t)r / TR : 0u;
+          const uint32_t abase = Geo::ABS ? tbase + (((rw & 3u) * 32u) << 16) + (rw >> 2) * (uint32_t)Geo::WC : 0u;
           if (live) {
             const uint32_t p = sE + r * (ZETA * 8);
-            if constexpr (ZETA == 1) asm volatile("st.shared.v2.b32 [%0], {%1,%2};" ::"r"(p), "r"(bk[0] * X), "r"(mulw[0]) : "memory");
+            if constexpr (ZETA == 1) asm volatile("st.shared.v2.b32 [%0], {%1,%2};" ::"r"(p), "r"(abase + bk[0] * X), "r"(mulw[0]) : "memory");
             else {
 #pragma unroll
               for (int k = 0; k < ZETA / 2; ++k)
                 asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p + 16 * k),
-                             "r"((bk[2 * k] - (uint32_t)((2 * k) / ZB) * dloc) * X), "r"(mulw[2 * k]),
-                             "r"((bk[2 * k + 1] - (uint32_t)((2 * k + 1) / ZB) * dloc) * X), "r"(mulw[2 * k + 1]) : "memory");
+                             "r"(abase + (bk[2 * k] - (uint32_t)((2 * k) / ZB) * dloc) * X), "r"(mulw[2 * k]),
+                             "r"(abase + (bk[2 * k + 1] - (uint32_t)((2 * k + 1) / ZB) * dloc) * X), "r"(mulw[2 * k + 1]) : "memory");
             }
           }
         } else {
@@ -546,7 +552,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM)) * 32
           }
         }
         // a5: read-modify-write of G x ZB sketch rows in tensor memory; same-bucket rows chained in registers
-        tmem_rmw<G, ZB, X, true>(region, q, col, mul);
+        tmem_rmw<G, ZB, X, true>(Geo::ABS ? 0u : region, q, col, mul);
       }
       }
       if constexpr (Geo::DEF) {

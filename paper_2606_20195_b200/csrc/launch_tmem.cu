@@ -110,10 +110,10 @@ bool tmem_shape(int n, int d, int zeta, TmemShape* out) {
 }
 
 size_t tmem_smem_bytes_for(int zeta, int n_cta, int bq, int gm) { return tmem_smem_bytes(zeta, n_cta, bq, gm); }
-int tmem_rows_per_stage(int n_cta) { return tmem_stage_rows(n_cta); }
+int tmem_rows_per_stage(int n_cta, int bq) { return tmem_stage_rows(n_cta, bq); }
 
 // 2-D tensor map over the row range: {n features, rows} FP32, row pitch lda, box {n / CS features, T rows}
-cudaError_t make_tensor_map(const TmemArgs& g, int n_cta, CUtensorMap* out) {
+cudaError_t make_tensor_map(const TmemArgs& g, int n_cta, int bq, CUtensorMap* out) {
   typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -128,7 +128,7 @@ cudaError_t make_tensor_map(const TmemArgs& g, int n_cta, CUtensorMap* out) {
   }
   const cuuint64_t dims[2] = {(cuuint64_t)g.s.n, (cuuint64_t)g.s.rows};
   const cuuint64_t strides[1] = {(cuuint64_t)g.s.lda * 4};
-  const cuuint32_t box[2] = {(cuuint32_t)n_cta, (cuuint32_t)tmem_stage_rows(n_cta)};
+  const cuuint32_t box[2] = {(cuuint32_t)n_cta, (cuuint32_t)tmem_stage_rows(n_cta, bq)};
   const cuuint32_t estr[2] = {1, 1};
   CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(g.s.A), dims, strides, box, estr,
                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -142,7 +142,7 @@ cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, const TmemShape& h, int
   memset(&tmap, 0, sizeof(tmap));
   if (g.s.lda != g.s.n / h.CS) {   // the kernel's non-contiguous path
     if (g.s.rows > 0x7FFFFFFF) return cudaErrorInvalidValue;
-    cudaError_t e = make_tensor_map(g, g.s.n / h.CS, &tmap);
+    cudaError_t e = make_tensor_map(g, g.s.n / h.CS, h.BQ, &tmap);
     if (e != cudaSuccess) return e;
   }
   switch (zeta) {

@@ -179,7 +179,7 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
     p->tm = tm;
     p->wpc = tm.NW + 1;
     p->smem_bytes = sk::tmem_smem_bytes_for(s->zeta, n / tm.CS, tm.BQ, tm.GM);
-    const int T = sk::tmem_rows_per_stage(n / tm.CS);
+    const int T = sk::tmem_rows_per_stage(n / tm.CS, tm.BQ);
     int64_t stages = (rows + T - 1) / T;
     // one CTA per SM (it owns all 512 TMEM columns); gridDim.y = CS column slices share a row range
     int64_t grid = s->sm_count / tm.CS;
