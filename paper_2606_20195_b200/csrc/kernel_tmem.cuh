@@ -156,7 +156,7 @@ struct TmemGeom {
   static constexpr int RS = NW / (S * BQ);     // row-sets per stage
   static constexpr int TR = T / RS;            // rows of a stage one warp processes
   static constexpr bool DEF = GM != 0;
-  static constexpr bool ABS = S == 1 && BQ == 1;   // entries hold absolute tensor-memory addresses (see the producer)
+  static constexpr bool ABS = S == 1;             // entries hold absolute tensor-memory addresses (see the producer)
   static constexpr int G = GM == 1 ? 4 : GM == 2 ? 8 : (ZB >= 4 || (BQ > 1 && ZB >= 2)) ? 2 : 4;  // rows per group (LDTMs in flight = G * ZB)
   static_assert(TR % G == 0 && 32 % G == 0, "whole groups");
   static constexpr int N = 64 * X * S;         // features of the CTA's column slice
@@ -368,21 +368,25 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM)) * 32
           bk[j] = entry_bucket(e);
           mulw[j] = 0x3C003C00u ^ entry_signmask_h2(e);
         }
+        // region of the consumer warp that owns (this row, bucket group b) when there is one feature slice
+        auto abase = [&](uint32_t b) -> uint32_t {
+          if constexpr (!Geo::ABS) return 0u;
+          const uint32_t w = b + (uint32_t)BQ * ((uint32_t)r / TR);
+          return tbase + (((w & 3u) * 32u) << 16) + (w >> 2) * (uint32_t)Geo::WC;
+        };
         if constexpr (!Geo::DEF) {
-          // entries {(bucket - first sketch row of the block's group) * X, multiplier}.  With one slice and one bucket
-          // group a row is read by exactly one consumer warp (its row-set), so the entry carries that warp's complete
-          // tensor-memory address and the consumer saves an add per (row, block)
-          const uint32_t rw = Geo::ABS ? (uint32_t)r / TR : 0u;
-          const uint32_t abase = Geo::ABS ? tbase + (((rw & 3u) * 32u) << 16) + (rw >> 2) * (uint32_t)Geo::WC : 0u;
+          // entries {(bucket - first sketch row of the block's group) * X, multiplier}.  With one feature slice the
+          // entry of (row, bucket group) is read by exactly one consumer warp, so it carries that warp's complete
+          // tensor-memory address (abase) and the consumer saves an add per (row, block)
           if (live) {
             const uint32_t p = sE + r * (ZETA * 8);
-            if constexpr (ZETA == 1) asm volatile("st.shared.v2.b32 [%0], {%1,%2};" ::"r"(p), "r"(abase + bk[0] * X), "r"(mulw[0]) : "memory");
+            if constexpr (ZETA == 1) asm volatile("st.shared.v2.b32 [%0], {%1,%2};" ::"r"(p), "r"(abase(0) + bk[0] * X), "r"(mulw[0]) : "memory");
             else {
 #pragma unroll
               for (int k = 0; k < ZETA / 2; ++k)
                 asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p + 16 * k),
-                             "r"(abase + (bk[2 * k] - (uint32_t)((2 * k) / ZB) * dloc) * X), "r"(mulw[2 * k]),
-                             "r"(abase + (bk[2 * k + 1] - (uint32_t)((2 * k + 1) / ZB) * dloc) * X), "r"(mulw[2 * k + 1]) : "memory");
+                             "r"(abase((2 * k) / ZB) + (bk[2 * k] - (uint32_t)((2 * k) / ZB) * dloc) * X), "r"(mulw[2 * k]),
+                             "r"(abase((2 * k + 1) / ZB) + (bk[2 * k + 1] - (uint32_t)((2 * k + 1) / ZB) * dloc) * X), "r"(mulw[2 * k + 1]) : "memory");
             }
           }
         } else {
@@ -434,8 +438,8 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM)) * 32
             uint32_t cm[ZB], co[ZB], mm[ZB];
 #pragma unroll
             for (int jj = 0; jj < ZB; ++jj) {
-              cm[jj] = (fb[bb * ZB + jj] - b * dloc) * X;
-              co[jj] = (bk[bb * ZB + jj] - b * dloc) * X;
+              cm[jj] = abase(b) + (fb[bb * ZB + jj] - b * dloc) * X;
+              co[jj] = abase(b) + (bk[bb * ZB + jj] - b * dloc) * X;
               mm[jj] = mulw[bb * ZB + jj];
             }
             if (live) sts_rec<ZB>(sE + ((uint32_t)r * BQ + b) * RB, def ? (uint32_t)(T * Geo::Q_ROW) : (uint32_t)r * Geo::Q_ROW, cm, mm);
@@ -514,7 +518,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM)) * 32
             for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + ((gi + 2) * G + r) * (BQ * RB), qo[gi & 1][r], col[(gi + 2) % 3][r], mul[(gi + 2) % 3][r]);
           }
           // a5: read-modify-write of G x ZB sketch rows in tensor memory, pairwise distinct by construction
-          tmem_rmw<G, ZB, X, false>(region, q[gi & 1], col[gi % 3], mul[gi % 3]);
+          tmem_rmw<G, ZB, X, false>(Geo::ABS ? 0u : region, q[gi & 1], col[gi % 3], mul[gi % 3]);
         }
       } else {
 #pragma unroll
@@ -567,7 +571,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM)) * 32
             lds_rec<ZB>(sL + ((pl * BQ + bgrp) * T + i) * RB, row, c1[0], m1[0]);
             if (row / TR != rowset) continue;
             lds_q<X>(qlane + row * Geo::Q_ROW, q1[0]);
-            tmem_rmw<1, ZB, X, false>(region, q1, c1, m1);
+            tmem_rmw<1, ZB, X, false>(Geo::ABS ? 0u : region, q1, c1, m1);
           }
         }
       }
