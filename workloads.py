@@ -177,3 +177,22 @@ def ls_system_device(m: int, n: int, seed: int, device, sigma_min: float = 1e-4,
         e = torch.randn(r1 - r0, generator=g, device=device, dtype=torch.float64)
         b[r0:r1] = (A[r0:r1].to(torch.float64) @ xstar + noise * e).to(torch.float32)
     return A, b, xstar
+
+
+def ls_paper_low_coherence_device(m: int, n: int, seed: int, device):
+    """Device form of `ls_paper_low_coherence`: A = (G / sqrt(m)) diag(sigma), sigma linear 100 -> 1,
+    b = A 1 + 0.1 N(0,1).  Returns (A [m, n] FP32, b [m, 1] FP32)."""
+    import torch
+
+    g = torch.Generator(device=device)
+    g.manual_seed(seed)
+    sigma = torch.linspace(100.0, 1.0, n, dtype=torch.float64, device=device) / float(np.sqrt(m))
+    A = gaussian_device(m, n, seed + 3000003, device)
+    A.mul_(sigma.to(torch.float32)[None, :])
+    b = torch.empty((m, 1), dtype=torch.float32, device=device)
+    step = 1 << 18
+    for r0 in range(0, m, step):
+        r1 = min(m, r0 + step)
+        e = torch.randn(r1 - r0, generator=g, device=device, dtype=torch.float64)
+        b[r0:r1, 0] = (A[r0:r1].double().sum(dim=1) + 0.1 * e).to(torch.float32)
+    return A, b
