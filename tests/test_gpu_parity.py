@@ -500,3 +500,32 @@ def test_full_size_sampled_columns(ss, name, m, n, d, zeta, variant):
     # FP16: never above 5e-2 (north star).  The flat kernel keeps one running sum per entry and replica, the
     # privatised kernels a two-level hierarchy; both stay far below at these depths (L = 2^14 .. 2^19)
     assert r16 <= 5e-2, r16
+
+
+# ------------------------------------------------------------------------------------ geometry sweep
+def _geometry_cases():
+    rng = np.random.default_rng(20260611)
+    cases = []
+    for n in (64, 128, 192, 256, 512, 1024):     # 192 = 3 x 64 has no geometry: skipped, like sketches beyond TMEM
+        for zeta in (1, 2, 4, 8):
+            for d_over_zeta in (8, 32, 64, 128, 256, 512):
+                cases.append((int(rng.integers(600, 2600)), n, zeta * d_over_zeta, zeta))
+    idx = rng.permutation(len(cases))[:72]
+    return [cases[i] for i in sorted(idx)]
+
+
+@pytest.mark.parametrize("m,n,d,zeta", _geometry_cases())
+def test_tmem_geometry_sweep(ss, m, n, d, zeta):
+    # every geometry the tensor-memory kernel can take (X, S, bucket groups, column slices, chained / deferral groups,
+    # 16- to 128-row stages), forced, against the oracle: bit-exact where the arithmetic is exact in any order
+    # (zeta in {1, 4}), within 2e-3 of FP64 where the scale is irrational (zeta in {2, 8}; L <= 64 terms)
+    seed = sketch_seed(7000 + m + d)
+    sk = ss.Sketch(m, d, zeta, seed)
+    exact = zeta in (1, 4)
+    A = wl.integer_valued(m, n, m) if exact else wl.gaussian(m, n, m)
+    got = apply16(ss, sk, dev(A), "tmem")
+    want = oracle.f64_sketch(seed, d, zeta, A)
+    if exact:
+        assert np.array_equal(oracle.half_bits_to_f64(bits(got)), want)
+    else:
+        assert ev.rel_fro(oracle.half_bits_to_f64(bits(got)), want) <= 2e-3
