@@ -41,6 +41,9 @@ WORKLOADS = {
     # the paper's own headline point (Fig. 2): m = 2^21, n = 1024, d = 2n, zeta = 4, dense input;
     # BASELINE.md holds its H200 number for exactly this workload (7.11 ms complete sketch = 1208 GB/s of A)
     "e1": (1 << 21, 1024, 2048, 4, 5),
+    # widths that are not 64 * 2^k (three column slices of the tensor-memory kernel)
+    "w192": (1 << 22, 192, 384, 4, 6),
+    "w384": (1 << 22, 384, 768, 4, 6),
 }
 PAPER_GBPS = {"e1": (1 << 21) * 1024 * 4 / 7.11e-3 / 1e9}   # PAPER.md:322, H200 NVL (another machine: context)
 L2_RED_PAYLOAD_GBPS = 6000.0   # measured with sketch_red_probe on this pool's B200 (profiles/r01_red_probe.md)

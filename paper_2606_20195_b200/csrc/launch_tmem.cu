@@ -73,8 +73,8 @@ cudaError_t launch_tmem_z4(const TmemArgs& g, const TmemShape& h, const CUtensor
 bool tmem_shape(int n, int d, int zeta, TmemShape* out) {
   if (n <= 0 || d <= 0 || zeta <= 0 || n % 64 != 0 || d % zeta != 0) return false;
   const int NW = 4;
-  for (int cs = 1; cs <= 4; cs *= 2) {
-    if (n % (64 * cs) != 0) break;
+  for (int cs = 1; cs <= 4; ++cs) {   // 3 column slices serve the widths 64 * 3 * 2^k (192, 384, 768)
+    if (n % (64 * cs) != 0) continue;
     const int nc = n / cs;
     double best = 0.0;
     bool found = false;

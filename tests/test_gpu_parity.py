@@ -506,7 +506,7 @@ def test_full_size_sampled_columns(ss, name, m, n, d, zeta, variant):
 def _geometry_cases():
     rng = np.random.default_rng(20260611)
     cases = []
-    for n in (64, 128, 192, 256, 512, 1024):     # 192 = 3 x 64 has no geometry: skipped, like sketches beyond TMEM
+    for n in (64, 128, 192, 256, 384, 512, 1024):   # 192, 384: three column slices; sketches beyond TMEM are skipped
         for zeta in (1, 2, 4, 8):
             for d_over_zeta in (8, 32, 64, 128, 256, 512):
                 cases.append((int(rng.integers(600, 2600)), n, zeta * d_over_zeta, zeta))
