@@ -44,6 +44,10 @@ WORKLOADS = {
     # widths that are not 64 * 2^k (three column slices of the tensor-memory kernel)
     "w192": (1 << 22, 192, 384, 4, 6),
     "w384": (1 << 22, 384, 768, 4, 6),
+    # the paper's width with sketches that still fit tensor memory (d < 2n: not a paper point)
+    "n1024-d512": (1 << 21, 1024, 512, 4, 6),
+    "n1024-d1024": (1 << 21, 1024, 1024, 4, 6),
+    "w320": (1 << 22, 320, 640, 4, 6),
 }
 PAPER_GBPS = {"e1": (1 << 21) * 1024 * 4 / 7.11e-3 / 1e9}   # PAPER.md:322, H200 NVL (another machine: context)
 L2_RED_PAYLOAD_GBPS = 6000.0   # measured with sketch_red_probe on this pool's B200 (profiles/r01_red_probe.md)

@@ -29,7 +29,7 @@ int smem_max_bucket();
 struct TmemShape {
   int X, S, BQ, CS, NW, GM;
 };
-bool tmem_shape(int n, int d, int zeta, TmemShape* out);
+bool tmem_shape(int n, int d, int zeta, int64_t lda, TmemShape* out);
 size_t tmem_smem_bytes_for(int zeta, int n_cta, int bq, int gm);  // n_cta = n / CS
 int tmem_rows_per_stage(int n_cta, int bq);
 cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, const TmemShape& h, int grid, cudaStream_t st);

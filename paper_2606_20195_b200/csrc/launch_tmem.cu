@@ -70,12 +70,13 @@ cudaError_t launch_tmem_z4(const TmemArgs& g, const TmemShape& h, const CUtensor
 // the (X, S, BQ) with the fewest issued instructions per KiB of A.  Model (from the SASS of the main loop,
 // profiles/r02_tmem_shapes.md): a row slice of 256 X bytes costs 1 + 3 X instructions to load and convert
 // (in each of the BQ warps that need it) and 5.25 + 2 X per stack block to read-modify-write.
-bool tmem_shape(int n, int d, int zeta, TmemShape* out) {
+bool tmem_shape(int n, int d, int zeta, int64_t lda, TmemShape* out) {
   if (n <= 0 || d <= 0 || zeta <= 0 || n % 64 != 0 || d % zeta != 0) return false;
   const int NW = 4;
-  for (int cs = 1; cs <= 4; ++cs) {   // 3 column slices serve the widths 64 * 3 * 2^k (192, 384, 768)
+  for (int cs = 1; cs <= 8; ++cs) {   // odd slice counts serve the widths that are not 64 * 2^k (192, 320, 384, ...)
     if (n % (64 * cs) != 0) continue;
     const int nc = n / cs;
+    if (lda != nc && nc > 256) continue;   // strided tiles come through a tensor-map box of at most 256 elements a side
     double best = 0.0;
     bool found = false;
     for (int x = 4; x >= 1; x >>= 1) {

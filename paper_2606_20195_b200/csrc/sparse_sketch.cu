@@ -113,7 +113,7 @@ bool smem_feasible(const sketch* s, int n, int64_t lda, const void* A, const voi
 
 bool tmem_feasible(const sketch* s, int n, int64_t lda, const void* A, const void* B, sk::TmemShape* h) {
   if (!zeta_templated(s->zeta)) return false;
-  if (!sk::tmem_shape(n, s->d, s->zeta, h)) return false;
+  if (!sk::tmem_shape(n, s->d, s->zeta, lda, h)) return false;
   if (lda % 4 != 0 || !aligned(A, 16) || !aligned(B, 16)) return false;  // TMA bulk copies: 16-byte granules
   return sk::tmem_smem_bytes_for(s->zeta, n / h->CS, h->BQ, h->GM) <= (size_t)s->smem_optin;
 }
@@ -160,8 +160,10 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
     // one-row steps are issue-bound; from zeta = 2 on the privatised kernel wins wherever it fits
     // the tensor-memory kernel (profiles/r01_tmem_*.md) beats both wherever it fits; below ~4 MiB of A the
     // launch is latency-bound and the lighter kernels win
-    // (four column slices -- d = 2048 at n = 256 -- measured 2.54 TB/s against 2.74 TB/s of the flat REDs)
-    if (tm_ok && tm.CS < 4 && rows * (int64_t)n > (1 << 20)) v = SKETCH_VARIANT_TMEM;
+    // (64-feature column slices cut into bucket groups -- d = 2048 at n = 256, d = 640 at n = 320 -- measured 2.5-2.7 TB/s
+    // against 2.7-2.8 TB/s of the flat REDs: one LDTM per row and warp, hashes recomputed for every 256 bytes of a row;
+    // without bucket groups -- d = 384 at n = 192 -- the same slices run at 4.65 TB/s)
+    if (tm_ok && !(tm.X * tm.S == 1 && tm.BQ > 1) && rows * (int64_t)n > (1 << 20)) v = SKETCH_VARIANT_TMEM;
     else if (sm_ok && s->zeta >= 2) v = SKETCH_VARIANT_SMEM;
     else if (zt && vmax) v = SKETCH_VARIANT_FLAT_VEC;
     else v = SKETCH_VARIANT_GENERIC;

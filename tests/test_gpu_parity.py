@@ -99,6 +99,8 @@ SHAPES_EXACT = [
     # config-4 shaped sketches (256 KiB - 1 MiB): bucket groups and column slices of the tensor-memory kernel
     (6007, 256, 512, 4), (6007, 256, 1024, 4), (4099, 256, 2048, 4), (5003, 512, 512, 4), (7001, 128, 1024, 4),
     (3001, 512, 128, 1),
+    # up to eight column slices: the paper's width n = 1024 while the sketch fits, widths that are not 64 * 2^k
+    (2501, 1024, 512, 4), (2501, 1024, 1024, 4), (2503, 384, 768, 4), (2503, 320, 640, 4), (2503, 192, 96, 1),
 ]
 
 
@@ -309,6 +311,22 @@ def test_tmem_column_slices_row_ranges_accumulate_and_lda(ss, d):
     ref = ev.rel_fro(oracle.half_bits_to_f64(oracle.seq16_sketch(seed, d, zeta, G)), B)
     got = ev.rel_fro(oracle.half_bits_to_f64(bits(apply16(ss, sk, dev(G), "tmem"))), B)
     assert got <= 1.5 * ref and got <= 5e-2, (got, ref)
+
+
+def test_tmem_wide_rows_on_a_padded_leading_dimension(ss):
+    # strided tiles come through a 2-D tensor map whose box is at most 256 elements wide: n = 512 / 1024 with lda > n must
+    # pick more column slices than the contiguous case does, and still be exact
+    m, zeta = 4001, 4
+    for n, d in ((512, 128), (1024, 256), (256, 64)):
+        A = wl.integer_valued(m, n, 15)
+        seed = sketch_seed(600 + n)
+        want = oracle.f64_sketch(seed, d, zeta, A)
+        sk = ss.Sketch(m, d, zeta, seed)
+        Ap = torch.full((m, n + 4), float("nan"), device="cuda")
+        Ap[:, :n] = dev(A)
+        for view in (Ap[:, :n], dev(A)):
+            got = apply16(ss, sk, view, "tmem")
+            assert np.array_equal(oracle.half_bits_to_f64(bits(got)), want), (n, view.stride(0))
 
 
 def test_odd_n_and_poor_alignment_take_the_generic_path(ss):
