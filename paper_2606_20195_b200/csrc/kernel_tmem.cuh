@@ -132,8 +132,11 @@ SK_DEVINL uint32_t hfma2_u32(uint32_t q, uint32_t mult, uint32_t acc) {
 // ---------------------------------------------------------------------------------------- geometry
 // rows per stage: 32 KiB of A per stage, at least 16 rows (4 stages x 32 KiB x 148 SMs = 19 MB in flight; with 16 KiB
 // stages at n = 64 the consumers waited for data 36 % of their time, profiles/r01_tmem_shapes.md)
-// (bucket-group kernels keep 64 rows at n = 64: their records, side lists and FP16 tiles fill the rest of shared memory)
-__host__ __device__ constexpr int tmem_stage_rows(int n, int bq) { return n <= 64 ? (bq == 1 ? 128 : 64) : n <= 128 ? 64 : n == 256 ? 32 : 16; }
+// (bucket-group kernels with more than one block per warp keep 64 rows at n = 64: their records, side lists and FP16
+// tiles would not fit beside four 32 KiB tiles)
+__host__ __device__ constexpr int tmem_stage_rows(int n, int bq, int zeta) {
+  return n <= 64 ? ((bq == 1 || zeta == bq) ? 128 : 64) : n <= 128 ? 64 : n == 256 ? 32 : 16;
+}
 __host__ __device__ constexpr int tmem_stages(int n) { return n <= 512 ? 4 : 3; }
 // bytes of one (row, bucket group) record / side-list item of the deferral modes: {q offset | row, 0, then (col, mul) x ZB}
 __host__ __device__ constexpr int tmem_rec_bytes(int zb) { return zb == 1 ? 16 : 16 + 8 * zb; }
@@ -172,7 +175,8 @@ struct TmemGeom {
   static constexpr int NPC = DEF ? (CH >= 2 ? 2 : 1) : (CH >= 4 ? 2 : 1);   // n = 64: 4 hashes per 256 B of A, two hash warps
   static constexpr int NPB = DEF ? (BQ < 4 / NPC ? BQ : 4 / NPC) : 1;
   static constexpr int NP = NPC * NPB;
-  static constexpr int L_BYTES = DEF ? NPC * BQ * T * RB + 128 : 0;
+  static constexpr int LCAP = T / NPC;         // rows one chunk phase hashes = the most it can defer
+  static constexpr int L_BYTES = DEF ? NPC * BQ * LCAP * RB + 128 : 0;
   static constexpr int STAGE_BYTES = A_BYTES + E_BYTES + L_BYTES;
   static_assert(STAGE_BYTES % 128 == 0, "TMA destination alignment");
   // bucket groups: every row is needed by BQ warps, so the consumer warps first convert the stage ONCE into a
@@ -184,16 +188,16 @@ struct TmemGeom {
   static_assert((T * N / 4) % (NW * 32) == 0, "whole conversion passes");
 };
 
-__host__ __device__ constexpr int tmem_producers(int n, int bq, int gm) {
-  return gm == 0 ? (tmem_stage_rows(n, bq) >= 128 ? 2 : 1)
-                 : (tmem_stage_rows(n, bq) >= 64 ? 2 : 1) * (bq < (tmem_stage_rows(n, bq) >= 64 ? 2 : 4) ? bq : (tmem_stage_rows(n, bq) >= 64 ? 2 : 4));
+__host__ __device__ constexpr int tmem_producers(int n, int bq, int gm, int zeta) {
+  return gm == 0 ? (tmem_stage_rows(n, bq, zeta) >= 128 ? 2 : 1)
+                 : (tmem_stage_rows(n, bq, zeta) >= 64 ? 2 : 1) * (bq < (tmem_stage_rows(n, bq, zeta) >= 64 ? 2 : 4) ? bq : (tmem_stage_rows(n, bq, zeta) >= 64 ? 2 : 4));
 }
 // ring of stages | barriers + TMEM base (256 B) | with bucket groups: two converted (FP16) tiles | deferral: 2 KiB of
 // producer scratch (the sketch rows of a 32-row chunk, one 128-byte line per producer warp and block)
 constexpr size_t tmem_smem_bytes(int zeta, int n, int bq, int gm) {
-  const size_t t = (size_t)tmem_stage_rows(n, bq);
+  const size_t t = (size_t)tmem_stage_rows(n, bq, zeta);
   const size_t rb = (size_t)tmem_rec_bytes(zeta / bq);
-  const size_t e = gm ? t * bq * rb + 2 * bq * t * rb + 128 : t * zeta * 8;
+  const size_t e = gm ? 2 * t * bq * rb + 128 : t * zeta * 8;   // records + side lists (T rows in all) + counts
   return (size_t)tmem_stages(n) * (t * n * 4 + e) + 256 + (bq > 1 ? 2 * (t * n * 2 + (gm ? (size_t)n * 2 : 0)) : 0) + (gm ? 2048 : 0);
 }
 
@@ -279,11 +283,11 @@ template <int ZB> SK_DEVINL void sts_rec(uint32_t p, uint32_t head, const uint32
 
 // ---------------------------------------------------------------------------------------- the kernel
 template <int ZETA, int X, int S, int BQ, int NW, int GM>
-__global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM)) * 32, 1) k_tmem(TmemArgs g, const __grid_constant__ CUtensorMap tmap) {
-  constexpr int T = tmem_stage_rows(64 * X * S, BQ), NS = tmem_stages(64 * X * S);
+__global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)) * 32, 1) k_tmem(TmemArgs g, const __grid_constant__ CUtensorMap tmap) {
+  constexpr int T = tmem_stage_rows(64 * X * S, BQ, ZETA), NS = tmem_stages(64 * X * S);
   using Geo = TmemGeom<ZETA, X, S, BQ, NW, GM, T>;
   constexpr int TR = Geo::TR, G = Geo::G, N = Geo::N, ZB = Geo::ZB, RB = Geo::RB, NP = Geo::NP, NPC = Geo::NPC, NPB = Geo::NPB;
-  static_assert(NP == tmem_producers(N, BQ, GM), "producer warps");
+  static_assert(NP == tmem_producers(N, BQ, GM, ZETA), "producer warps");
   constexpr int JB = ZETA / NPB;                     // stack blocks one producer warp hashes
   constexpr uint32_t Q0 = NS * Geo::STAGE_BYTES + 256;   // first converted tile
   extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -444,7 +448,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM)) * 32
             }
             if (live) sts_rec<ZB>(sE + ((uint32_t)r * BQ + b) * RB, def ? (uint32_t)(T * Geo::Q_ROW) : (uint32_t)r * Geo::Q_ROW, cm, mm);
             const uint32_t m = __ballot_sync(0xFFFFFFFFu, def);
-            if (def) sts_rec<ZB>(sL + ((cp * BQ + b) * T + cnt[bb] + __popc(m & ((1u << lane) - 1u))) * RB, (uint32_t)r, co, mm);
+            if (def) sts_rec<ZB>(sL + ((cp * BQ + b) * Geo::LCAP + cnt[bb] + __popc(m & ((1u << lane) - 1u))) * RB, (uint32_t)r, co, mm);
             cnt[bb] += __popc(m);
           }
         }
@@ -452,7 +456,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM)) * 32
       if constexpr (Geo::DEF) {
 #pragma unroll
         for (int bb = 0; bb < BQ / NPB; ++bb)
-          if (lane == bb) asm volatile("st.shared.b32 [%0], %1;" ::"r"(sL + NPC * BQ * T * RB + (cp * BQ + b0 + bb) * 4), "r"(cnt[bb]) : "memory");
+          if (lane == bb) asm volatile("st.shared.b32 [%0], %1;" ::"r"(sL + NPC * BQ * Geo::LCAP * RB + (cp * BQ + b0 + bb) * 4), "r"(cnt[bb]) : "memory");
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(full);
@@ -564,11 +568,11 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM)) * 32
         const unsigned char* const sL = smem_raw + slot * Geo::STAGE_BYTES + Geo::A_BYTES + Geo::E_BYTES;
 #pragma unroll 1
         for (uint32_t pl = 0; pl < (uint32_t)NPC; ++pl) {
-          const uint32_t cnt = *reinterpret_cast<const uint32_t*>(sL + NPC * BQ * T * RB + (pl * BQ + bgrp) * 4);
+          const uint32_t cnt = *reinterpret_cast<const uint32_t*>(sL + NPC * BQ * Geo::LCAP * RB + (pl * BQ + bgrp) * 4);
 #pragma unroll 1
           for (uint32_t i = 0; i < cnt; ++i) {
             uint32_t row, q1[1][X], c1[1][ZB], m1[1][ZB];
-            lds_rec<ZB>(sL + ((pl * BQ + bgrp) * T + i) * RB, row, c1[0], m1[0]);
+            lds_rec<ZB>(sL + ((pl * BQ + bgrp) * Geo::LCAP + i) * RB, row, c1[0], m1[0]);
             if (row / TR != rowset) continue;
             lds_q<X>(qlane + row * Geo::Q_ROW, q1[0]);
             tmem_rmw<1, ZB, X, false>(Geo::ABS ? 0u : region, q1, c1, m1);

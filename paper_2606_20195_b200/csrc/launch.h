@@ -31,7 +31,7 @@ struct TmemShape {
 };
 bool tmem_shape(int n, int d, int zeta, int64_t lda, TmemShape* out);
 size_t tmem_smem_bytes_for(int zeta, int n_cta, int bq, int gm);  // n_cta = n / CS
-int tmem_rows_per_stage(int n_cta, int bq);
+int tmem_rows_per_stage(int n_cta, int bq, int zeta);
 cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, const TmemShape& h, int grid, cudaStream_t st);
 cudaError_t launch_tmem_z1(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st);
 cudaError_t launch_tmem_z2(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st);

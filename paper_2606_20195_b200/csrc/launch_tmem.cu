@@ -24,7 +24,7 @@ cudaError_t go(const TmemArgs& g, const CUtensorMap& tmap, int grid, int cs, cud
     const size_t smem = tmem_smem_bytes(Z, N, BQ, GM);
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k<<<dim3((unsigned)grid, (unsigned)cs), (NW + tmem_producers(N, BQ, GM)) * 32, smem, st>>>(g, tmap);
+    k<<<dim3((unsigned)grid, (unsigned)cs), (NW + tmem_producers(N, BQ, GM, Z)) * 32, smem, st>>>(g, tmap);
     return cudaGetLastError();
   }
 }
@@ -98,6 +98,7 @@ bool tmem_shape(int n, int d, int zeta, int64_t lda, TmemShape* out) {
           // 5.07 TB/s).  Deferral needs few clashes -- ZB * C(4,2) / (d/zeta) <= 0.15 -- and d/zeta >= G (G + 1).
           const double zb = (double)zeta / bq, dbk = (double)d / zeta;
           out->GM = (bq == 4 && zb * 6.0 / dbk <= 0.15 && dbk >= 20) ? 1 : 0;
+          if (out->GM == 1 && nc == 64 && zb * 28.0 / dbk <= 0.15 && dbk >= 72) out->GM = 2;   // c4-2048: 2.99 vs 2.93 TB/s
           if (const char* ev = getenv("SK_TMEM_GM")) {   // experiments only
             const int gm = atoi(ev);
             if (bq > 1 && (gm == 0 || (gm == 1 && dbk >= 20) || (gm == 2 && dbk >= 72))) out->GM = gm;
@@ -111,10 +112,10 @@ bool tmem_shape(int n, int d, int zeta, int64_t lda, TmemShape* out) {
 }
 
 size_t tmem_smem_bytes_for(int zeta, int n_cta, int bq, int gm) { return tmem_smem_bytes(zeta, n_cta, bq, gm); }
-int tmem_rows_per_stage(int n_cta, int bq) { return tmem_stage_rows(n_cta, bq); }
+int tmem_rows_per_stage(int n_cta, int bq, int zeta) { return tmem_stage_rows(n_cta, bq, zeta); }
 
 // 2-D tensor map over the row range: {n features, rows} FP32, row pitch lda, box {n / CS features, T rows}
-cudaError_t make_tensor_map(const TmemArgs& g, int n_cta, int bq, CUtensorMap* out) {
+cudaError_t make_tensor_map(const TmemArgs& g, int n_cta, int bq, int zeta, CUtensorMap* out) {
   typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -129,7 +130,7 @@ cudaError_t make_tensor_map(const TmemArgs& g, int n_cta, int bq, CUtensorMap* o
   }
   const cuuint64_t dims[2] = {(cuuint64_t)g.s.n, (cuuint64_t)g.s.rows};
   const cuuint64_t strides[1] = {(cuuint64_t)g.s.lda * 4};
-  const cuuint32_t box[2] = {(cuuint32_t)n_cta, (cuuint32_t)tmem_stage_rows(n_cta, bq)};
+  const cuuint32_t box[2] = {(cuuint32_t)n_cta, (cuuint32_t)tmem_stage_rows(n_cta, bq, zeta)};
   const cuuint32_t estr[2] = {1, 1};
   CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(g.s.A), dims, strides, box, estr,
                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -143,7 +144,7 @@ cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, const TmemShape& h, int
   memset(&tmap, 0, sizeof(tmap));
   if (g.s.lda != g.s.n / h.CS) {   // the kernel's non-contiguous path
     if (g.s.rows > 0x7FFFFFFF) return cudaErrorInvalidValue;
-    cudaError_t e = make_tensor_map(g, g.s.n / h.CS, h.BQ, &tmap);
+    cudaError_t e = make_tensor_map(g, g.s.n / h.CS, h.BQ, zeta, &tmap);
     if (e != cudaSuccess) return e;
   }
   switch (zeta) {

@@ -160,10 +160,10 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
     // one-row steps are issue-bound; from zeta = 2 on the privatised kernel wins wherever it fits
     // the tensor-memory kernel (profiles/r01_tmem_*.md) beats both wherever it fits; below ~4 MiB of A the
     // launch is latency-bound and the lighter kernels win
-    // (64-feature column slices cut into bucket groups -- d = 2048 at n = 256, d = 640 at n = 320 -- measured 2.5-2.7 TB/s
-    // against 2.7-2.8 TB/s of the flat REDs: one LDTM per row and warp, hashes recomputed for every 256 bytes of a row;
-    // without bucket groups -- d = 384 at n = 192 -- the same slices run at 4.65 TB/s)
-    if (tm_ok && !(tm.X * tm.S == 1 && tm.BQ > 1) && rows * (int64_t)n > (1 << 20)) v = SKETCH_VARIANT_TMEM;
+    // (64-feature column slices cut into bucket groups of several blocks -- d = 640 at n = 320 -- measured 2.69 TB/s
+    // against 2.80 TB/s of the flat REDs; with one block per warp they get 128-row stages and win: d = 2048 at n = 256
+    // 2.99 vs 2.74 TB/s; without bucket groups -- d = 384 at n = 192 -- the same slices run at 4.65 TB/s)
+    if (tm_ok && !(tm.X * tm.S == 1 && tm.BQ > 1 && tm.BQ != s->zeta) && rows * (int64_t)n > (1 << 20)) v = SKETCH_VARIANT_TMEM;
     else if (sm_ok && s->zeta >= 2) v = SKETCH_VARIANT_SMEM;
     else if (zt && vmax) v = SKETCH_VARIANT_FLAT_VEC;
     else v = SKETCH_VARIANT_GENERIC;
@@ -181,7 +181,7 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
     p->tm = tm;
     p->wpc = tm.NW + 1;
     p->smem_bytes = sk::tmem_smem_bytes_for(s->zeta, n / tm.CS, tm.BQ, tm.GM);
-    const int T = sk::tmem_rows_per_stage(n / tm.CS, tm.BQ);
+    const int T = sk::tmem_rows_per_stage(n / tm.CS, tm.BQ, s->zeta);
     int64_t stages = (rows + T - 1) / T;
     // one CTA per SM (it owns all 512 TMEM columns); gridDim.y = CS column slices share a row range
     int64_t grid = s->sm_count / tm.CS;

@@ -297,8 +297,7 @@ def test_tmem_column_slices_row_ranges_accumulate_and_lda(ss, d):
     seed = sketch_seed(56 + d)
     want = oracle.f64_sketch(seed, d, zeta, A)
     sk = ss.Sketch(m, d, zeta, seed)
-    # AUTO: tensor memory up to two column slices; four (d = 2048) measured slower than the flat 16-byte REDs
-    assert sk.plan(n)["variant"] == ("tmem" if d <= 1024 else "flat_vec")
+    assert sk.plan(n)["variant"] == "tmem"
     Ap = torch.full((m, n + 12), float("nan"), device="cuda")
     Ap[:, :n] = dev(A)
     out = None
@@ -472,7 +471,8 @@ FULL_SIZES = [
     ("c5", 1 << 25, 128, 256, 4, "tmem"),
     ("c4-512", 1 << 23, 256, 512, 4, "tmem"),
     ("c4", 1 << 23, 256, 1024, 4, "tmem"),
-    ("c4-2048", 1 << 23, 256, 2048, 4, "flat_vec"),
+    ("c4-2048", 1 << 23, 256, 2048, 4, "tmem"),
+    ("e1", 1 << 21, 1024, 2048, 4, "flat_vec"),
     ("c3", 1 << 22, 128, 256, 4, "tmem"),
 ]
 
