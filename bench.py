@@ -48,6 +48,7 @@ WORKLOADS = {
     "n1024-d512": (1 << 21, 1024, 512, 4, 6),
     "n1024-d1024": (1 << 21, 1024, 1024, 4, 6),
     "w320": (1 << 22, 320, 640, 4, 6),
+    "e1-d4096": (1 << 21, 1024, 4096, 4, 5),    # d/n = 4 of the paper's grid: 8 MiB sketch, beyond tensor memory
 }
 PAPER_GBPS = {"e1": (1 << 21) * 1024 * 4 / 7.11e-3 / 1e9}   # PAPER.md:322, H200 NVL (another machine: context)
 L2_RED_PAYLOAD_GBPS = 6000.0   # measured with sketch_red_probe on this pool's B200 (profiles/r01_red_probe.md)

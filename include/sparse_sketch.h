@@ -60,7 +60,7 @@ typedef struct sketch sketch_t; /* opaque, library-owned */
 #define SKETCH_VARIANT_GENERIC 4   /* any n / any alignment scalar fallback (one lane per element) */
 #define SKETCH_VARIANT_TMEM 5      /* tensor-memory-privatised partial sketch per warp (tcgen05.ld / tcgen05.st read-
                                       modify-write), A staged by TMA, hashes computed on the fly by a producer
-                                      warp; FP16-RN, zeta in {1,2,4,8}, n = 64*X*S*CS with X, S in {1,2,4}, CS in 1..8,
+                                      warp; FP16-RN, zeta in {1,2,4,8}, n = 64*X*S*CS with X, S in {1,2,4}, CS in 1..16,
                                       BQ in {1,2,4} bucket groups dividing zeta, S*BQ <= 4 and (d/BQ)*X <= 512
                                       (e.g. n = 256: d <= 2048), lda % 4 == 0, A and B 16-byte
                                       aligned, rows < 2^31 when lda != n / CS (2-D tensor-map coordinates) */

@@ -73,7 +73,7 @@ cudaError_t launch_tmem_z4(const TmemArgs& g, const TmemShape& h, const CUtensor
 bool tmem_shape(int n, int d, int zeta, int64_t lda, TmemShape* out) {
   if (n <= 0 || d <= 0 || zeta <= 0 || n % 64 != 0 || d % zeta != 0) return false;
   const int NW = 4;
-  for (int cs = 1; cs <= 8; ++cs) {   // odd slice counts serve the widths that are not 64 * 2^k (192, 320, 384, ...)
+  for (int cs = 1; cs <= 16; ++cs) {   // odd slice counts serve the widths that are not 64 * 2^k (192, 320, 384, ...)
     if (n % (64 * cs) != 0) continue;
     const int nc = n / cs;
     if (lda != nc && nc > 256) continue;   // strided tiles come through a tensor-map box of at most 256 elements a side

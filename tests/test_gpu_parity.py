@@ -472,7 +472,8 @@ FULL_SIZES = [
     ("c4-512", 1 << 23, 256, 512, 4, "tmem"),
     ("c4", 1 << 23, 256, 1024, 4, "tmem"),
     ("c4-2048", 1 << 23, 256, 2048, 4, "tmem"),
-    ("e1", 1 << 21, 1024, 2048, 4, "flat_vec"),
+    ("e1", 1 << 21, 1024, 2048, 4, "tmem"),
+    ("e1-d4096", 1 << 21, 1024, 4096, 4, "flat_vec"),
     ("c3", 1 << 22, 128, 256, 4, "tmem"),
 ]
 
