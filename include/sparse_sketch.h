@@ -64,6 +64,9 @@ typedef struct sketch sketch_t; /* opaque, library-owned */
                                       BQ in {1,2,4} bucket groups dividing zeta, S*BQ <= 4 and (d/BQ)*X <= 512
                                       (e.g. n = 256: d <= 2048), lda % 4 == 0, A and B 16-byte
                                       aligned, rows < 2^31 when lda != n / CS (2-D tensor-map coordinates) */
+#define SKETCH_VARIANT_SMALL 6     /* per-warp shared-memory partial sketches for small inputs and narrow matrices:
+                                      FP16-RN, zeta in {1,2,4,8}, n and lda even, A 8-byte aligned,
+                                      8*d*n*2 bytes of shared memory (AUTO picks it for launch-bound inputs) */
 
 typedef struct sketch_opts {
   int32_t variant;    /* SKETCH_VARIANT_* */

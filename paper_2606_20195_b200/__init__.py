@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     VARIANT_GENERIC,
     VARIANT_SMEM,
     VARIANT_TMEM,
+    VARIANT_SMALL,
     VARIANT_NAMES,
     Sketch,
     SketchError,

@@ -14,7 +14,7 @@ CSRC = HERE / "csrc"
 OBJ = HERE / "_obj"
 LIB = HERE / "libsparse_sketch.so"
 SOURCES = [CSRC / n for n in ("sparse_sketch.cu", "launch_flat_f16.cu", "launch_flat_f32.cu", "launch_smem.cu", "launch_tmem.cu")]
-HEADERS = [CSRC / n for n in ("args.h", "launch.h", "device_util.cuh", "kernel_flat.cuh", "kernel_misc.cuh", "kernel_smem.cuh", "kernel_tmem.cuh")]
+HEADERS = [CSRC / n for n in ("args.h", "launch.h", "device_util.cuh", "kernel_flat.cuh", "kernel_misc.cuh", "kernel_smem.cuh", "kernel_small.cuh", "kernel_tmem.cuh")]
 # (source, object stem, extra flags): launch_tmem.cu is compiled once per zeta family
 UNITS = [(src, src.stem, []) for src in SOURCES if src.name != "launch_tmem.cu"]
 UNITS += [(CSRC / "launch_tmem.cu", "launch_tmem_z%d" % z, ["-DSK_TMEM_ZETA=%d" % z]) for z in (1, 2, 4, 8)]

@@ -12,8 +12,8 @@ from pathlib import Path
 from . import _build
 
 RN, SR = 0, 1
-VARIANT_AUTO, VARIANT_FLAT_PAIR, VARIANT_FLAT_VEC, VARIANT_SMEM, VARIANT_GENERIC, VARIANT_TMEM = 0, 1, 2, 3, 4, 5
-VARIANT_NAMES = {0: "auto", 1: "flat_pair", 2: "flat_vec", 3: "smem", 4: "generic", 5: "tmem"}
+VARIANT_AUTO, VARIANT_FLAT_PAIR, VARIANT_FLAT_VEC, VARIANT_SMEM, VARIANT_GENERIC, VARIANT_TMEM, VARIANT_SMALL = 0, 1, 2, 3, 4, 5, 6
+VARIANT_NAMES = {0: "auto", 1: "flat_pair", 2: "flat_vec", 3: "smem", 4: "generic", 5: "tmem", 6: "small"}
 
 
 class SketchOpts(C.Structure):

@@ -31,6 +31,12 @@ struct SmemArgs {
   uint32_t zero;  // always 0; the kernel uses it to build a scheduling dependency ptxas cannot fold away
 };
 
+struct SmallArgs {
+  ScatterArgs s;          // packed unused (hashes on the fly); n even, lda even, A 8-byte aligned, B 4-byte aligned
+  int64_t rows_per_warp;  // multiple of 16
+  int32_t d;
+};
+
 struct TmemArgs {
   ScatterArgs s;  // packed unused (the producer warp hashes on the fly); lda % 4 == 0, A and B 16-byte aligned
   int32_t d;

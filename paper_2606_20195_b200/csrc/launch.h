@@ -22,6 +22,9 @@ int smem_step_rows(int zeta);           // R: rows per step; row ranges given to
 cudaError_t launch_hash_pack_rot(uint64_t seed, int zeta, int64_t rows, uint32_t db, uint16_t* out, int grid,
                                  cudaStream_t st);
 int smem_max_bucket();
+// per-warp shared-memory partials for small inputs / narrow matrices (kernel_small.cuh); smem = warps * d * n * 2 bytes
+cudaError_t launch_small_f16(const SmallArgs& g, int zeta, int grid, size_t smem_bytes, cudaStream_t st);
+int small_warps();
 
 // tensor-memory-privatised FP16-RN scatter (kernel_tmem.cuh).  Geometry: n = 64 * X * S * CS; lane holds X half2
 // words, S feature slices and BQ bucket groups per CTA, CS column slices across CTAs (gridDim.y), NW consumer warps.

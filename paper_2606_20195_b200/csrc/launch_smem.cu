@@ -1,4 +1,5 @@
 // launch_smem.cu -- instantiations of the shared-memory-privatised scatter and its hash-pack kernel.
+#include "kernel_small.cuh"
 #include "kernel_smem.cuh"
 #include "launch.h"
 
@@ -33,6 +34,30 @@ cudaError_t launch_smem_f16(const SmemArgs& g, int zeta, int wpc, int grid, size
   }
   return cudaErrorInvalidValue;
 }
+
+namespace {
+template <int ZETA>
+cudaError_t go_small(const SmallArgs& g, int grid, size_t smem_bytes, cudaStream_t st) {
+  auto k = k_small<ZETA>;
+  if (smem_bytes > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    if (e != cudaSuccess) return e;
+  }
+  k<<<grid, kSmallWarps * 32, smem_bytes, st>>>(g);
+  return cudaGetLastError();
+}
+}  // namespace
+
+cudaError_t launch_small_f16(const SmallArgs& g, int zeta, int grid, size_t smem_bytes, cudaStream_t st) {
+  switch (zeta) {
+    case 1: return go_small<1>(g, grid, smem_bytes, st);
+    case 2: return go_small<2>(g, grid, smem_bytes, st);
+    case 4: return go_small<4>(g, grid, smem_bytes, st);
+    case 8: return go_small<8>(g, grid, smem_bytes, st);
+  }
+  return cudaErrorInvalidValue;
+}
+int small_warps() { return kSmallWarps; }
 
 int smem_ring_rows(int zeta, int wpc) { return smem_rows_per_step(zeta) * smem_batch_steps(zeta, wpc <= 4); }
 int smem_step_rows(int zeta) { return smem_rows_per_step(zeta); }

@@ -138,7 +138,7 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
   if (rc) return rc;
   memset(p, 0, sizeof(*p));
   int want = o ? o->variant : SKETCH_VARIANT_AUTO;
-  if (want < 0 || want > SKETCH_VARIANT_TMEM) return SKETCH_ERR_INVALID;
+  if (want < 0 || want > SKETCH_VARIANT_SMALL) return SKETCH_ERR_INVALID;
   p->hash_mode = (o && o->hash_mode) ? o->hash_mode : 1;
   if (p->hash_mode != 1 && p->hash_mode != 2) return SKETCH_ERR_INVALID;
   size_t sm_bytes = 0;
@@ -149,6 +149,10 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
                (rb0 % sk::smem_step_rows(s->zeta) == 0);
   sk::TmemShape tm = {0, 0, 0, 0, 0, 0};
   bool tm_ok = f16 && rounding == SKETCH_RN && tmem_feasible(s, n, lda, A, B, &tm);
+  // per-warp shared-memory partials (kernel_small.cuh)
+  const size_t small_bytes = (size_t)sk::small_warps() * s->d * n * 2;
+  bool small_ok = f16 && rounding == SKETCH_RN && zeta_templated(s->zeta) && n % 2 == 0 && lda % 2 == 0 && aligned(A, 8) &&
+                  small_bytes <= (size_t)s->smem_optin;
   int vmax = flat_vec_for(f16, n, lda, A, B, 8);
   int vpair = flat_vec_for(f16, n, lda, A, B, f16 ? 2 : 1);
   bool zt = zeta_templated(s->zeta);
@@ -165,11 +169,15 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
     // 2.99 vs 2.74 TB/s; without bucket groups -- d = 384 at n = 192 -- the same slices run at 4.65 TB/s)
     if (tm_ok && !(tm.X * tm.S == 1 && tm.BQ > 1 && tm.BQ != s->zeta) && rows * (int64_t)n > (1 << 20)) v = SKETCH_VARIANT_TMEM;
     else if (sm_ok && s->zeta >= 2) v = SKETCH_VARIANT_SMEM;
+    // launch-bound inputs into a sketch of a few KiB: the flat REDs queue ~1000 deep on each L2 sector (c1: 10 us);
+    // per-warp shared-memory partials need no such queue
+    else if (small_ok && small_bytes <= 64 * 1024 && rows * (int64_t)n <= (1 << 20)) v = SKETCH_VARIANT_SMALL;
     else if (zt && vmax) v = SKETCH_VARIANT_FLAT_VEC;
     else v = SKETCH_VARIANT_GENERIC;
   }
   if (v == SKETCH_VARIANT_SMEM && !sm_ok) return SKETCH_ERR_UNSUPPORTED;
   if (v == SKETCH_VARIANT_TMEM && !tm_ok) return SKETCH_ERR_UNSUPPORTED;
+  if (v == SKETCH_VARIANT_SMALL && !small_ok) return SKETCH_ERR_UNSUPPORTED;
   if (v == SKETCH_VARIANT_FLAT_VEC && !(zt && vmax)) return SKETCH_ERR_UNSUPPORTED;
   if (v == SKETCH_VARIANT_FLAT_PAIR && !(zt && vpair)) return SKETCH_ERR_UNSUPPORTED;
   p->variant = v;
@@ -189,6 +197,30 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
     if (grid > stages) grid = stages;
     if (grid < 1) grid = 1;
     p->grid = (int)grid;
+    return SKETCH_OK;
+  }
+
+  if (v == SKETCH_VARIANT_SMALL) {
+    p->hash_mode = 1;
+    p->replicas = 1;
+    p->wpc = sk::small_warps();
+    p->smem_bytes = small_bytes;
+    const int64_t rb = 16;   // rows per step of k_small (two batches of 8; 2 x 4 at zeta = 8)
+    // one step per warp while that keeps the grid at <= 32 CTAs: every CTA ends with d*n/2 REDs into the same few
+    // L2 sectors, which is the queue this kernel exists to avoid
+    int64_t rpw = (rows + 32 * (int64_t)p->wpc - 1) / (32 * (int64_t)p->wpc);
+    rpw = (rpw + rb - 1) / rb * rb;
+    if (rpw < rb) rpw = rb;
+    int64_t grid = (rows + rpw * p->wpc - 1) / (rpw * p->wpc);
+    if (o && o->grid_ctas > 0) {
+      grid = o->grid_ctas;
+      rpw = (rows + grid * p->wpc - 1) / (grid * p->wpc);
+      rpw = (rpw + rb - 1) / rb * rb;
+      if (rpw < rb) rpw = rb;
+    }
+    if (grid < 1) grid = 1;
+    p->grid = (int)grid;
+    p->rows_per_cta = rpw;   // rows per WARP for this variant
     return SKETCH_OK;
   }
 
@@ -347,6 +379,19 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
       g.s = make_args(s, A, n, lda, B, row_begin, rows, sr_seed, 1);
       g.d = s->d;
       rc = launched(sk::launch_tmem_f16(g, s->zeta, p.tm, p.grid, st), "k_tmem");
+      if (rc) return rc;
+    }
+    return SKETCH_OK;
+  }
+
+  if (p.variant == SKETCH_VARIANT_SMALL) {
+    if (!accumulate) CU_TRY(cudaMemsetAsync(B, 0, out_bytes, st));  // a0
+    if (rows > 0) {
+      sk::SmallArgs g;
+      g.s = make_args(s, A, n, lda, B, row_begin, rows, sr_seed, 2);
+      g.rows_per_warp = p.rows_per_cta;
+      g.d = s->d;
+      rc = launched(sk::launch_small_f16(g, s->zeta, p.grid, p.smem_bytes, st), "k_small");
       if (rc) return rc;
     }
     return SKETCH_OK;

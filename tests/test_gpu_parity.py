@@ -37,9 +37,9 @@ def bits(t):
     return b
 
 
-F16_VARIANTS = ["auto", "flat_pair", "flat_vec", "smem", "tmem", "generic"]
+F16_VARIANTS = ["auto", "flat_pair", "flat_vec", "smem", "tmem", "small", "generic"]
 F32_VARIANTS = ["auto", "flat_pair", "flat_vec", "generic"]
-VID = {"auto": 0, "flat_pair": 1, "flat_vec": 2, "smem": 3, "generic": 4, "tmem": 5}
+VID = {"auto": 0, "flat_pair": 1, "flat_vec": 2, "smem": 3, "generic": 4, "tmem": 5, "small": 6}
 
 
 def apply16(ss, sk, A, variant="auto", **kw):
@@ -284,7 +284,7 @@ def test_row_ranges_accumulate_and_lda(ss, variant):
     out32 = None
     for k, (r0, r1) in enumerate(((0, 37), (37, 12001), (12001, m))):
         out32 = sk.apply_f32acc(Ap[r0:r1, :n], out=out32, row_begin=r0, accumulate=k > 0,
-                                variant=VID[variant] if variant not in ("smem", "tmem") else 0)
+                                variant=VID[variant] if variant not in ("smem", "tmem", "small") else 0)
     assert np.array_equal(out32.cpu().numpy().astype(np.float64), want)
 
 
@@ -434,7 +434,7 @@ def test_subnormal_scale_is_exact_in_any_order(ss):
     assert np.abs(mag).max() < 2048 and np.count_nonzero(want) > 0.9 * want.size
     sk = ss.Sketch(m, d, zeta, seed)
     want[want == 0x8000] = 0
-    for variant in ("tmem", "smem", "flat_vec", "flat_pair"):
+    for variant in ("tmem", "smem", "small", "flat_vec", "flat_pair"):
         assert np.array_equal(bits(sk.apply_f16acc(dev(A), variant=VID[variant])), want), variant
 
 
