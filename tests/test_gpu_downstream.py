@@ -151,3 +151,26 @@ def test_paper_shaped_least_squares_fp16_costs_under_one_percent(ss, family):
     assert abs(r32 - r64) <= 0.01 * r64, (r32, r64)
     # one seed, not the paper's median over seeds: +0.14 % (low-coherence) and +1.5 % (coherent, residual 6e-4) measured
     assert r16 <= (1.01 if family == "low_coherence" else 1.03) * r32, (r16, r32)
+
+
+def test_coordinate_subspace_rank_countsketch_vs_sparsestack(ss):
+    # PAPER.md:72-77 (Eq. 3) and :352: on the coordinate subspace U = [I_n; 0] a CountSketch (zeta = 1) of d = 2n rows is
+    # full rank only with probability prod_{j<n}(1 - j/d) (~1e-40 at n = 256: two unit rows share a bucket), while
+    # SparseStack with zeta = 4 keeps full rank at d = 2n.  Entries are 0 / 1 and every bucket sum is a small multiple of
+    # 1/2, so the FP16 GPU sketch is exact and its rank is the rank of S U itself.
+    m, n = 1 << 16, 256
+    d = 2 * n
+    A = np.zeros((m, n), dtype=np.float32)
+    A[np.arange(n), np.arange(n)] = 1.0
+    Ad = dev(A)
+    for zeta, full in ((1, False), (4, True)):
+        seed = sketch_seed(80 + zeta)
+        sk = ss.Sketch(m, d, zeta, seed)
+        SA = f16_to_f64(sk.apply_f16acc(Ad))
+        assert np.array_equal(SA, oracle.f64_sketch(seed, d, zeta, A, threads=THREADS))
+        rank = int(np.linalg.matrix_rank(SA))
+        b, _ = oracle.hashes(seed, d, zeta, n)
+        distinct = len(set(b[:, 0].tolist()))
+        if zeta == 1:
+            assert rank == distinct < n          # rank of a CountSketch on unit rows = number of distinct buckets hit
+        assert (rank == n) == full, (zeta, rank)
