@@ -11,30 +11,31 @@
 // per FP16 half), and the SM's L1/shared data pipe -- 81 % busy in the shared-memory kernel
 // (profiles/r01_smem_c5.md) -- only carries A itself.
 //
-// CTA = NW consumer warps + 1 producer warp, one CTA per SM (it allocates all 512 TMEM columns).
-//   producer  : per stage of T rows: cp.async.bulk (TMA, L2 evict-first) of the A tile into a ring of NS
-//               shared-memory slots, completion on an mbarrier; meanwhile its 32 lanes compute the stage's
-//               hashes ON THE FLY (a1: splitmix64 counter hash, one lane per row) and store per (row, block)
-//               an 8-byte entry {TMEM column offset = bucket*X, HFMA2 multiplier = +-1.0 in both halves}.
+// CTA = NW = 4 consumer warps + 1 producer warp (2 at n = 64, up to 4 in the deferral modes), one CTA per SM (it
+// allocates all 512 TMEM columns), persistent over stages of T rows (32 KiB of A, a ring of NS shared-memory slots).
+//   producers : one TMA copy per stage -- cp.async.bulk for a contiguous tile, a 2-D tensor-map box
+//               {N features x T rows} (cp.async.bulk.tensor.2d; rows past the end zero-filled) for strided rows and
+//               column slices -- L2 evict-first, completion on an mbarrier; meanwhile their lanes compute the stage's
+//               hashes ON THE FLY (a1: splitmix64 counter hash, one lane per row) and store per (row, block) an entry
+//               {TMEM address or column offset of the sketch row, HFMA2 multiplier = +-1.0 in both halves}.
 //               No separate hash pass, no packed hash array in HBM.
-//   consumers : warp w owns TMEM lanes [32*(w%4), +32) (the hardware's lane quadrant of that warp) and
-//               columns [(w/4)*d*X, +d*X): a private d x 64X partial sketch.  n = 64*X*S: a row is cut in S
-//               column slices; warp w takes slice w%S of the rows of row-set w/S of every stage.
-//               Rows are processed in groups of G: all LDTMs of a group are issued, then one
-//               tcgen05.wait::ld, then the HFMA2s and STTMs.  Two rows of a group that hit the same
-//               bucket are chained in registers (the later row adds onto the earlier row's result and both
-//               store the chain's final value) -- the bucket is warp-uniform, so this is a select, not
-//               divergence.  tcgen05.wait::st orders a group's LDTMs behind the previous group's STTMs.
+//   consumers : warp w owns TMEM lanes [32*(w%4), +32) (the hardware's lane quadrant of that warp): a private
+//               (d/BQ) x 64X partial sketch.  The CTA's N = 64*X*S features are cut in S slices; warp w takes slice
+//               w % S and bucket group (w / S) % BQ of the rows of row-set w / (S*BQ) of every stage.
+//               Rows are processed in groups of G: all LDTMs of a group are issued, then one tcgen05.wait::ld, then
+//               the HFMA2s and STTMs; tcgen05.wait::st orders a group's LDTMs behind the previous group's STTMs.
+//               Two rows of a group that hit the same sketch row are either chained in registers or kept apart by the
+//               producers (deferral) -- see TmemGeom.
 //   flush     : LDTM.x8 -> result-discarding vector REDs into B.
 //
 // Sketches larger than one warp's 512 TMEM columns (d * X > 512) are split two ways:
 //   BQ bucket groups : the zeta stack blocks are cut into BQ groups of ZB = zeta / BQ consecutive blocks
 //               (disjoint sketch-row ranges); a warp of group b holds only the d / BQ sketch
-//               rows of its blocks and adds only those contributions.  Every row is then converted by BQ
-//               warps, which costs shared-memory reads and F2FPs but no tensor-memory capacity.
-//   CS column slices : gridDim.y CTAs share a row range, CTA y takes the features [y * N, (y + 1) * N) of every
-//               row (N = 64 * X * S); its A tile is fetched row by row (N * 4 bytes each), the hashes are
-//               recomputed per slice.  d = 1024, n = 256: X = 2, BQ = 4, CS = 2;  d = 2048: X = 1, BQ = 4, CS = 4.
+//               rows of its blocks and adds only those contributions.  Every row is then needed by BQ warps, so
+//               the consumers first convert the stage ONCE into a shared FP16 tile (a3, a4) and scatter from that.
+//   CS column slices : gridDim.y CTAs (1..16) share a row range, CTA y takes the features [y * N, (y + 1) * N) of
+//               every row; the hashes are recomputed per slice.  n = 256: d = 1024 -> X = 2, BQ = 4, CS = 2;
+//               d = 2048 -> X = 1, BQ = 4, CS = 4; the paper's n = 1024, d = 2048 -> X = 1, BQ = 4, CS = 16.
 // Accumulation is FP16 RN throughout; the hierarchy is (warp-private partial) -> RED into B.
 #pragma once
 

@@ -99,7 +99,8 @@ bool tmem_shape(int n, int d, int zeta, int64_t lda, TmemShape* out) {
           const double zb = (double)zeta / bq, dbk = (double)d / zeta;
           out->GM = (bq == 4 && zb * 6.0 / dbk <= 0.15 && dbk >= 20) ? 1 : 0;
           if (out->GM == 1 && nc == 64 && zb * 28.0 / dbk <= 0.15 && dbk >= 72) out->GM = 2;   // c4-2048: 2.99 vs 2.93 TB/s
-          if (const char* ev = getenv("SK_TMEM_GM")) {   // experiments only
+          static const char* const ev = getenv("SK_TMEM_GM");   // experiments only (read once)
+          if (ev) {
             const int gm = atoi(ev);
             if (bq > 1 && (gm == 0 || (gm == 1 && dbk >= 20) || (gm == 2 && dbk >= 72))) out->GM = gm;
           }
