@@ -218,6 +218,10 @@ def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    for _ in range(5):                 # a driver still tearing down a previous large process can fail one init
+        if torch.cuda.is_available():
+            break
+        time.sleep(2.0)
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
     torch.cuda.set_device(local)
