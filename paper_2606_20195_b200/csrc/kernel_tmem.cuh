@@ -484,7 +484,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
         // a3, a4 once per element: the whole stage -> FP16 tile `it & 1` (row pitch N * 2 bytes)
         const float4* const tile = reinterpret_cast<const float4*>(smem_raw + slot * Geo::STAGE_BYTES);
         unsigned char* const qb = smem_raw + Q0 + (it & 1u) * Geo::Q_BYTES;
-        constexpr int CI = (T * N / 4) / (NW * 32), CB = CI < 8 ? CI : 8;   // loads in batches of CB (the stores may alias for all the compiler knows)
+        constexpr int CI = (T * N / 4) / (NW * 32), CB = (BQ >= 4 && CI >= 16) ? 16 : (CI < 8 ? CI : 8);   // loads in batches of CB (the stores may alias for all the compiler knows; 16 measured +1-2 % with four bucket groups, -5 % with two)
 #pragma unroll
         for (int i0 = 0; i0 < CI; i0 += CB) {
           float4 t[CB];
