@@ -184,6 +184,9 @@ struct TmemGeom {
   // shared FP16 tile (a3, a4), meet at a named barrier, and then each scatters its own blocks from that tile.
   // Two tiles (stage parity); the deferral modes append one all-zero row to each.
   static constexpr bool SHQ = BQ > 1;
+  // deferral modes: the PRODUCER warps convert the stage, in place (the FP16 tile takes the first half of the FP32
+  // tile's bytes), once its TMA copy has landed; the consumers only scatter.  TMA runs NS - 1 stages ahead.
+  static constexpr bool PCONV = DEF;
   static constexpr int Q_ROW = N * 2;
   static constexpr int Q_BYTES = T * Q_ROW + (DEF ? Q_ROW : 0);
   static_assert((T * N / 4) % (NW * 32) == 0, "whole conversion passes");
@@ -193,13 +196,13 @@ __host__ __device__ constexpr int tmem_producers(int n, int bq, int gm, int zeta
   return gm == 0 ? (tmem_stage_rows(n, bq, zeta) >= 128 ? 2 : 1)
                  : (tmem_stage_rows(n, bq, zeta) >= 64 ? 2 : 1) * (bq < (tmem_stage_rows(n, bq, zeta) >= 64 ? 2 : 4) ? bq : (tmem_stage_rows(n, bq, zeta) >= 64 ? 2 : 4));
 }
-// ring of stages | barriers + TMEM base (256 B) | with bucket groups: two converted (FP16) tiles | deferral: 2 KiB of
-// producer scratch (the sketch rows of a 32-row chunk, one 128-byte line per producer warp and block)
+// ring of stages | barriers + TMEM base (256 B) | chained bucket-group kernels: two converted (FP16) tiles | deferral:
+// one all-zero FP16 row + 2 KiB of producer scratch (the sketch rows of a 32-row chunk, a 128-byte line per warp and block)
 constexpr size_t tmem_smem_bytes(int zeta, int n, int bq, int gm) {
   const size_t t = (size_t)tmem_stage_rows(n, bq, zeta);
   const size_t rb = (size_t)tmem_rec_bytes(zeta / bq);
   const size_t e = gm ? 2 * t * bq * rb + 128 : t * zeta * 8;   // records + side lists (T rows in all) + counts
-  return (size_t)tmem_stages(n) * (t * n * 4 + e) + 256 + (bq > 1 ? 2 * (t * n * 2 + (gm ? (size_t)n * 2 : 0)) : 0) + (gm ? 2048 : 0);
+  return (size_t)tmem_stages(n) * (t * n * 4 + e) + 256 + (gm ? (size_t)n * 2 + 2048 : bq > 1 ? 2 * t * n * 2 : 0);
 }
 
 // a5 for R rows x ZB stack blocks of one warp: LDTM, one RN16 add per half (fma.rn.f16x2 by +-1), STTM.
@@ -290,7 +293,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
   constexpr int TR = Geo::TR, G = Geo::G, N = Geo::N, ZB = Geo::ZB, RB = Geo::RB, NP = Geo::NP, NPC = Geo::NPC, NPB = Geo::NPB;
   static_assert(NP == tmem_producers(N, BQ, GM, ZETA), "producer warps");
   constexpr int JB = ZETA / NPB;                     // stack blocks one producer warp hashes
-  constexpr uint32_t Q0 = NS * Geo::STAGE_BYTES + 256;   // first converted tile
+  constexpr uint32_t Q0 = NS * Geo::STAGE_BYTES + 256;   // first converted tile (chained modes) / the zero row (deferral)
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const ScatterArgs& a = g.s;
   const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -298,7 +301,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
   // shared-memory carve-up: [NS][A tile | entries or records | side lists] then the barriers, then the FP16 tiles
   const uint32_t smem0 = smem_u32(smem_raw);
   const uint32_t bars = smem0 + NS * Geo::STAGE_BYTES;     // full[NS], empty[NS], 8 B each
-  uint32_t* const tbase_p = reinterpret_cast<uint32_t*>(smem_raw + NS * Geo::STAGE_BYTES + 16 * NS);
+  uint32_t* const tbase_p = reinterpret_cast<uint32_t*>(smem_raw + NS * Geo::STAGE_BYTES + 24 * NS);   // after full, empty, tma
 
   if (warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tbase_p)) : "memory");
@@ -308,15 +311,13 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
     for (int k = 0; k < NS; ++k) {
       mbar_init(bars + 8 * k, NP);             // full: one arrive per producer warp (+ the TMA transaction bytes)
       mbar_init(bars + 8 * (NS + k), NW);      // empty: one arrive per consumer warp
+      mbar_init(bars + 8 * (2 * NS + k), 1);   // tma (producer-side conversion only): the issuing lane's arrive + the transaction bytes
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async;" ::: "memory");
   }
-  if constexpr (Geo::DEF) {                    // the all-zero row behind each converted tile
-    for (uint32_t i = tid * 4; i < 2u * Geo::Q_ROW; i += (NW + NP) * 32 * 4) {
-      const uint32_t tile = i / Geo::Q_ROW, off = i % Geo::Q_ROW;
-      *reinterpret_cast<uint32_t*>(smem_raw + Q0 + tile * Geo::Q_BYTES + T * Geo::Q_ROW + off) = 0u;
-    }
+  if constexpr (Geo::DEF) {                    // the all-zero FP16 row the deferred rows' records point at
+    for (uint32_t i = tid * 4; i < (uint32_t)Geo::Q_ROW; i += (NW + NP) * 32 * 4) *reinterpret_cast<uint32_t*>(smem_raw + Q0 + i) = 0u;
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
@@ -331,31 +332,56 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
     // ================================================================ producers: TMA + hash stage (a1, a2)
     const uint32_t pw = warp - NW;                 // producer warp pw: 32-row chunks cp, cp + NPC, ...; stack blocks [j0, j0 + JB)
     const uint32_t cp = pw % NPC, j0 = (pw / NPC) * JB, b0 = j0 / ZB;
-    unsigned char* const scr = smem_raw + Q0 + 2 * Geo::Q_BYTES + pw * (JB * 128);   // deferral: [JB][32] sketch rows
+    unsigned char* const scr = smem_raw + Q0 + Geo::Q_ROW + pw * (JB * 128);   // deferral: [JB][32] sketch rows
     static_assert(!Geo::DEF || NP * JB * 128 <= 2048, "producer scratch");
     const uint64_t policy = l2_evict_first_policy();
     const bool contiguous = (a.lda == N);          // implies a single column slice
+    // a2: TMA copy of this CTA's k-th stage (producer warp 0).  Waits until the consumers have released the slot;
+    // completion (bytes) on `full` (consumer-side conversion) or on `tma` (producer-side conversion)
+    auto issue = [&](uint32_t k) {
+      const int64_t st = blockIdx.x + (int64_t)k * gridDim.x;
+      if (st >= nstages) return;
+      const uint32_t slot = k % NS, ph = (k / NS) & 1;
+      const uint32_t sA = smem0 + slot * Geo::STAGE_BYTES;
+      const uint32_t bar = bars + 8 * ((Geo::PCONV ? 2 * NS : 0) + slot);
+      mbar_wait(bars + 8 * (NS + slot), ph ^ 1);   // passes at once the first time round the ring
+      if constexpr (Geo::PCONV) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the slot held generic-proxy writes (FP16 tile)
+      const int64_t row0 = st * T;
+      const int32_t nrows = (int32_t)min((int64_t)T, a.rows - row0);
+      if (contiguous) {
+        if (lane == 0) {
+          mbar_expect_tx(bar, (uint32_t)nrows * N * 4);
+          bulk_g2s(sA, a.A + row0 * a.lda, (uint32_t)nrows * N * 4, bar, policy);
+        }
+        if (nrows < T) {                         // last stage of the matrix: rows past the end contribute +0
+          const uint32_t z0 = sA + nrows * N * 4, z1 = sA + Geo::A_BYTES;
+          for (uint32_t p = z0 + lane * 16; p < z1; p += 32 * 16) asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(p), "r"(0u) : "memory");
+        }
+      } else if (lane == 0) {                    // strided rows / column slice: one tiled TMA copy per stage
+        mbar_expect_tx(bar, (uint32_t)T * N * 4);
+        tensor_g2s(sA, &tmap, (int32_t)col0, (int32_t)row0, bar, policy);
+      }
+      if constexpr (Geo::PCONV) {
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar);
+      }
+    };
+    constexpr uint32_t AHEAD = NS - 1;
+    if constexpr (Geo::PCONV) {
+      if (pw == 0)
+        for (uint32_t k = 0; k < AHEAD; ++k) issue(k);
+    }
     uint32_t it = 0;
     for (int64_t st = blockIdx.x; st < nstages; st += gridDim.x, ++it) {
       const uint32_t slot = it % NS, ph = (it / NS) & 1;
       const uint32_t sA = smem0 + slot * Geo::STAGE_BYTES, sE = sA + Geo::A_BYTES, sL = sE + Geo::E_BYTES;
       const uint32_t full = bars + 8 * slot, empty = bars + 8 * (NS + slot);
-      mbar_wait(empty, ph ^ 1);                // passes at once the first time round the ring
       const int64_t row0 = st * T;
-      const int32_t nrows = (int32_t)min((int64_t)T, a.rows - row0);
-      if (pw != 0) {
-      } else if (contiguous) {
-        if (lane == 0) {
-          mbar_expect_tx(full, (uint32_t)nrows * N * 4);
-          bulk_g2s(sA, a.A + row0 * a.lda, (uint32_t)nrows * N * 4, full, policy);
-        }
-      } else if (lane == 0) {                  // strided rows / column slice: one tiled TMA copy per stage
-        mbar_expect_tx(full, (uint32_t)T * N * 4);
-        tensor_g2s(sA, &tmap, (int32_t)col0, (int32_t)row0, full, policy);
-      }
-      if (pw == 0 && contiguous && nrows < T) {           // last stage of the matrix: rows past the end contribute +0
-        const uint32_t z0 = sA + nrows * N * 4, z1 = sA + Geo::A_BYTES;
-        for (uint32_t p = z0 + lane * 16; p < z1; p += 32 * 16) asm volatile("st.shared.v4.b32 [%0], {%1,%1,%1,%1};" ::"r"(p), "r"(0u) : "memory");
+      if constexpr (Geo::PCONV) {
+        if (pw != 0) mbar_wait(empty, ph ^ 1);   // warp 0 waited before it issued this stage's copy
+      } else {
+        if (pw == 0) issue(it);
+        else mbar_wait(empty, ph ^ 1);
       }
       // a1: rows lane, lane + 32, ... of the stage
       uint32_t cnt[BQ];                        // deferral: side-list lengths (warp-uniform)
@@ -447,7 +473,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
               co[jj] = abase(b) + (bk[bb * ZB + jj] - b * dloc) * X;
               mm[jj] = mulw[bb * ZB + jj];
             }
-            if (live) sts_rec<ZB>(sE + ((uint32_t)r * BQ + b) * RB, def ? (uint32_t)(T * Geo::Q_ROW) : (uint32_t)r * Geo::Q_ROW, cm, mm);
+            if (live) sts_rec<ZB>(sE + ((uint32_t)r * BQ + b) * RB, def ? Q0 - slot * (uint32_t)Geo::STAGE_BYTES : (uint32_t)r * Geo::Q_ROW, cm, mm);
             const uint32_t m = __ballot_sync(0xFFFFFFFFu, def);
             if (def) sts_rec<ZB>(sL + ((cp * BQ + b) * Geo::LCAP + cnt[bb] + __popc(m & ((1u << lane) - 1u))) * RB, (uint32_t)r, co, mm);
             cnt[bb] += __popc(m);
@@ -459,8 +485,34 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
         for (int bb = 0; bb < BQ / NPB; ++bb)
           if (lane == bb) asm volatile("st.shared.b32 [%0], %1;" ::"r"(sL + NPC * BQ * Geo::LCAP * RB + (cp * BQ + b0 + bb) * 4), "r"(cnt[bb]) : "memory");
       }
+      if constexpr (Geo::PCONV) {
+        // a3, a4 once per element, in place: FP16 word pair k of the tile lands on bytes [8k, 8k + 8), i.e. on FP32 data
+        // that an earlier pass (or, in the first pass, this pass before the barrier) has already read
+        mbar_wait(bars + 8 * (2 * NS + slot), ph);
+        constexpr uint32_t P = NP * 32;
+        constexpr int CI = (T * N / 4) / P, CB = CI < 16 ? CI : 16;
+        static_assert((T * N / 4) % P == 0 && CI % CB == 0, "whole conversion passes");
+        const uint32_t ptid = pw * 32 + lane;
+        const float4* const tile = reinterpret_cast<const float4*>(smem_raw + slot * Geo::STAGE_BYTES);
+        uint2* const qt = reinterpret_cast<uint2*>(smem_raw + slot * Geo::STAGE_BYTES);
+        const float scale = a.scale;
+#pragma unroll 1
+        for (int i0 = 0; i0 < CI; i0 += CB) {
+          float4 t[CB];
+#pragma unroll
+          for (int i = 0; i < CB; ++i) t[i] = tile[(uint32_t)(i0 + i) * P + ptid];
+          if constexpr (NP > 1) asm volatile("bar.sync 2, %0;" ::"n"(P) : "memory");
+          else __syncwarp();
+#pragma unroll
+          for (int i = 0; i < CB; ++i)
+            qt[(uint32_t)(i0 + i) * P + ptid] = make_uint2(pack_rn(t[i].x * scale, t[i].y * scale), pack_rn(t[i].z * scale, t[i].w * scale));
+        }
+      }
       __syncwarp();
       if (lane == 0) mbar_arrive(full);
+      if constexpr (Geo::PCONV) {
+        if (pw == 0) issue(it + AHEAD);
+      }
     }
   } else {
     // ================================================================ consumers: a3, a4, a5 in tensor memory
@@ -480,7 +532,9 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
       const unsigned char* const sE = smem_raw + slot * Geo::STAGE_BYTES + Geo::A_BYTES + e_off;
       mbar_wait(bars + 8 * slot, ph);
       const unsigned char* qlane = nullptr;    // this lane's words of row 0 of the converted tile
-      if constexpr (Geo::SHQ) {
+      if constexpr (Geo::PCONV) {
+        qlane = smem_raw + slot * Geo::STAGE_BYTES + (slice * 64 * X + lane * 2 * X) * 2;   // converted in place by the producers
+      } else if constexpr (Geo::SHQ) {
         // a3, a4 once per element: the whole stage -> FP16 tile `it & 1` (row pitch N * 2 bytes)
         const float4* const tile = reinterpret_cast<const float4*>(smem_raw + slot * Geo::STAGE_BYTES);
         unsigned char* const qb = smem_raw + Q0 + (it & 1u) * Geo::Q_BYTES;
