@@ -98,7 +98,6 @@ bool tmem_shape(int n, int d, int zeta, int64_t lda, TmemShape* out) {
           // 5.07 TB/s).  Deferral needs few clashes -- ZB * C(4,2) / (d/zeta) <= 0.15 -- and d/zeta >= G (G + 1).
           const double zb = (double)zeta / bq, dbk = (double)d / zeta;
           out->GM = (bq == 4 && zb * 6.0 / dbk <= 0.15 && dbk >= 20) ? 1 : 0;
-          if (out->GM == 1 && nc == 64 && zb * 28.0 / dbk <= 0.15 && dbk >= 72) out->GM = 2;   // c4-2048: 2.99 vs 2.93 TB/s
           static const char* const ev = getenv("SK_TMEM_GM");   // experiments only (read once)
           if (ev) {
             const int gm = atoi(ev);
