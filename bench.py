@@ -58,8 +58,8 @@ VARIANTS = {"auto": 0, "flat_pair": 1, "flat_vec": 2, "smem": 3, "generic": 4, "
 # `ncu --set full` captures (profiles/*.md name the commands); None where not captured.
 NCU_TRAFFIC_BYTES = {
     ("c5", "smem"): 17448452000 + 4160000,   # profiles/r01_smem_c5.md: 17.448 GB read (A 17.180 + packed hashes 0.268) + 4 MB written
-    ("e1", "tmem"): 8594198000 + 4182784,    # profiles/r01_tmem_shapes.md
-    ("c4", "tmem"): 8590917000 + 4116480,
+    ("e1", "tmem"): 8594182000 + 3782912,    # profiles/r01_tmem_shapes.md
+    ("c4", "tmem"): 8590524000 + 3837184,
     ("c5", "tmem"): 17180124000 + 3726080,   # profiles/r01_tmem_c5.md: 17.180 GB read (A only) + 3.7 MB written
 }
 
