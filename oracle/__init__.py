@@ -19,13 +19,13 @@ from pathlib import Path
 import numpy as np
 
 _HERE = Path(__file__).resolve().parent
-_SRC = [_HERE / "sketch_oracle.cpp", _HERE / "f16c_crosscheck.cpp"]
+_SRC = [_HERE / "sketch_oracle.cpp", _HERE / "f16c_crosscheck.cpp", _HERE / "bf16_crosscheck.cpp"]
 _LIB = _HERE / "_build" / "liboracle.so"
 _lock = threading.Lock()
 _lib = None
 
 IDEAL, BQ, BC = 0, 1, 2  # modes of f64_sketch (Eq. 7)
-RN, SR = 0, 1
+RN, SR, DITHER = 0, 1, 2   # conversion rules of PAPER.md:193-207 (Sec. III-D)
 
 
 def _host_has_f16c() -> bool:
@@ -47,6 +47,9 @@ def build(force: bool = False) -> Path:
         o0 = _LIB.parent / "sketch_oracle.o"
         subprocess.check_call(common + ["-c", str(_SRC[0]), "-o", str(o0)])
         objs.append(str(o0))
+        o2 = _LIB.parent / "bf16_crosscheck.o"
+        subprocess.check_call(common + ["-c", str(_SRC[2]), "-o", str(o2)])
+        objs.append(str(o2))
         if _host_has_f16c():
             o1 = _LIB.parent / "f16c_crosscheck.o"
             subprocess.check_call(common + ["-mf16c", "-c", str(_SRC[1]), "-o", str(o1)])
@@ -97,6 +100,30 @@ def lib() -> C.CDLL:
         L.orc_seq32_accumulate.argtypes = [u64, i32, i32, vp, i64, i64, i32, i64, vp]
         L.orc_range_counts.restype = C.c_int
         L.orc_range_counts.argtypes = [i32, vp, i64, i32, i64, vp]
+        L.orc_bf16_rn.restype = u16
+        L.orc_bf16_rn.argtypes = [C.c_float]
+        L.orc_bf16_to_double.restype = C.c_double
+        L.orc_bf16_to_double.argtypes = [u16]
+        L.orc_bf16_add.restype = u16
+        L.orc_bf16_add.argtypes = [u16, u16]
+        L.orc_xorshift64.restype = u64
+        L.orc_xorshift64.argtypes = [u64]
+        L.orc_dither_c.restype = C.c_float
+        L.orc_dither_c.argtypes = []
+        L.orc_bf16_rn_array.restype = None
+        L.orc_bf16_rn_array.argtypes = [vp, i64, vp]
+        L.orc_bf16_add_array.restype = None
+        L.orc_bf16_add_array.argtypes = [vp, vp, i64, vp]
+        L.orc_bf16_to_double_array.restype = None
+        L.orc_bf16_to_double_array.argtypes = [vp, i64, vp]
+        L.orc_dither16_array.restype = None
+        L.orc_dither16_array.argtypes = [vp, vp, C.c_float, i64, vp]
+        L.orc_seqbf16_accumulate.restype = C.c_int
+        L.orc_seqbf16_accumulate.argtypes = [u64, i32, i32, vp, i64, i64, i32, i64, vp]
+        L.orc_x_bf16_vs_bits.restype = i64
+        L.orc_x_bf16_vs_bits.argtypes = [u32, u64, u32, i32, vp]
+        L.orc_x_bf16_add_vs_float.restype = i64
+        L.orc_x_bf16_add_vs_float.argtypes = [u32, u32, i32, vp]
         if hasattr(L, "orc_x_rn16_vs_f16c"):
             L.orc_x_rn16_vs_f16c.restype = i64
             L.orc_x_rn16_vs_f16c.argtypes = [u32, u64, u32, i32, vp]
@@ -154,6 +181,50 @@ def sr16(p, r24) -> np.ndarray:
     assert p.shape == r24.shape
     out = np.empty(p.shape, dtype=np.uint16)
     lib().orc_sr16_array(_ptr(p), _ptr(r24), p.size, _ptr(out))
+    return out
+
+
+def bf16_rn(p) -> np.ndarray:
+    """RN to bfloat16 of float32 values -> uint16 bit patterns."""
+    p = np.ascontiguousarray(p, dtype=np.float32)
+    out = np.empty(p.shape, dtype=np.uint16)
+    lib().orc_bf16_rn_array(_ptr(p), p.size, _ptr(out))
+    return out
+
+
+def bf16_add(z, v) -> np.ndarray:
+    """RN_bf16(z + v) on uint16 bit patterns."""
+    z = np.ascontiguousarray(z, dtype=np.uint16)
+    v = np.ascontiguousarray(v, dtype=np.uint16)
+    assert z.shape == v.shape
+    out = np.empty(z.shape, dtype=np.uint16)
+    lib().orc_bf16_add_array(_ptr(z), _ptr(v), z.size, _ptr(out))
+    return out
+
+
+def bf16_bits_to_f64(b) -> np.ndarray:
+    b = np.ascontiguousarray(b, dtype=np.uint16)
+    out = np.empty(b.shape, dtype=np.float64)
+    lib().orc_bf16_to_double_array(_ptr(b), b.size, _ptr(out))
+    return out
+
+
+def xorshift64(x: int) -> int:
+    return int(lib().orc_xorshift64(x & (2**64 - 1)))
+
+
+def dither_c() -> np.float32:
+    """The FP32 coefficient c of Eq. (6)."""
+    return np.float32(lib().orc_dither_c())
+
+
+def dither16(p, r24, c=None) -> np.ndarray:
+    """Q_dith(p) = RN16(p + (u0 - 1/2) c p), u0 = r24 * 2^-24 (Eq. 6) -> uint16 bit patterns."""
+    p = np.ascontiguousarray(p, dtype=np.float32)
+    r24 = np.ascontiguousarray(r24, dtype=np.uint32)
+    assert p.shape == r24.shape
+    out = np.empty(p.shape, dtype=np.uint16)
+    lib().orc_dither16_array(_ptr(p), _ptr(r24), float(dither_c() if c is None else c), p.size, _ptr(out))
     return out
 
 
@@ -216,6 +287,15 @@ def seq16_sketch(seed: int, d: int, zeta: int, A: np.ndarray, rounding: int = RN
     return D
 
 
+def seqbf16_sketch(seed: int, d: int, zeta: int, A: np.ndarray, row_begin: int = 0) -> np.ndarray:
+    """Sequential bfloat16 accumulation in ascending (i, j) order -> uint16 bit patterns [d, n]."""
+    A = _check_A(A)
+    D = np.zeros((d, A.shape[1]), dtype=np.uint16)
+    _ok(lib().orc_seqbf16_accumulate(seed, d, zeta, _ptr(A), row_begin, A.shape[0], A.shape[1],
+                                     A.strides[0] // 4, _ptr(D)))
+    return D
+
+
 def seq32_sketch(seed: int, d: int, zeta: int, A: np.ndarray, row_begin: int = 0) -> np.ndarray:
     A = _check_A(A)
     B = np.zeros((d, A.shape[1]), dtype=np.float32)
@@ -245,4 +325,16 @@ def rn16_vs_f16c(first: int, count: int, stride: int, threads: int):
 def add16_vs_f16c(v0: int, v_stride: int, threads: int):
     bad = C.c_uint32(0)
     n = lib().orc_x_add16_vs_f16c(v0, v_stride, threads, C.addressof(bad))
+    return int(n), int(bad.value)
+
+
+def bf16_vs_bits(first: int, count: int, stride: int, threads: int):
+    bad = C.c_uint32(0)
+    n = lib().orc_x_bf16_vs_bits(first, count, stride, threads, C.addressof(bad))
+    return int(n), int(bad.value)
+
+
+def bf16_add_vs_float(v0: int, v_stride: int, threads: int):
+    bad = C.c_uint32(0)
+    n = lib().orc_x_bf16_add_vs_float(v0, v_stride, threads, C.addressof(bad))
     return int(n), int(bad.value)

@@ -20,6 +20,11 @@
 //   SEQ16 mode ........ integer-valued input == F64 bit-exact; serial bound PAPER.md:261
 //   BQ / BC modes ..... Proposition 1 (Eq. 8, 9)
 //   SR ................ unbiasedness over all 2^24 draws; Cor. 3 Eq. (12) variance
+//   bf16 rn / add ..... exhaustive (all 2^32 floats) vs the integer add-and-truncate rule, torch.bfloat16,
+//                       worked example at u = 2^-8, serial bound; SEQ-BF16: integer-valued input == F64
+//   xorshift64 ........ Marsaglia's published vector (tests/golden/xorshift64_vector.txt)
+//   dither ............ c = 0 and u0 = 1/2 reduce to RN16; oddness; monotone in u0; closed-form
+//                       jump probabilities over all 2^24 draws (Eq. 6)
 // "parity unpinned" (bit-wise) for SEQ16 on generic inputs: the GPU order is
 // arbitrary, so SEQ16 is one legal result, compared statistically.
 //
@@ -155,9 +160,67 @@ inline uint16_t float_to_half_sr(float p, uint32_t r24) {
   return (uint16_t)(sign | bits);
 }
 
-// s = fp32(1/sqrt(zeta)), correctly rounded from FP64 (reading R5; PAPER.md:161
-// "signed FP32 scale eps/sqrt(zeta)").
-inline float scale_f32(int32_t zeta) { return (float)(1.0 / std::sqrt((double)zeta)); }
+
+// ---------------------------------------------------------------------------
+// bfloat16 control (PAPER.md:382 Fig. 7 "BF16 is a wider-range reference", :396 "BF16 remains
+// finite throughout ... residual is about 20% larger").  Format: 1 sign, 8 exponent (bias 127,
+// the FP32 range), 7 fraction bits; u = 2^-8; subnormal spacing 2^-133.  Written from the
+// format definition like the binary16 routines above; subnormals kept, overflow -> +-inf.
+// ---------------------------------------------------------------------------
+inline double bf16_to_double(uint16_t b) {
+  uint32_t sign = b >> 15;
+  uint32_t e = (b >> 7) & 0xFF;
+  uint32_t f = b & 0x7F;
+  double v;
+  if (e == 0) {
+    v = std::ldexp((double)f, -133);                  // subnormal: f * 2^-133
+  } else if (e == 255) {
+    v = f ? std::nan("") : INFINITY;
+  } else {
+    v = std::ldexp((double)(128 + f), (int)e - 134);  // (1+f/128)*2^(e-127)
+  }
+  return sign ? -v : v;
+}
+
+// Round a double to bfloat16: nearest, ties to even, gradual underflow, one rounding on the
+// exact value; |x| >= 2^128 (1 - 2^-9) -> inf.
+inline uint16_t double_to_bf16_rn(double x) {
+  uint16_t sign = std::signbit(x) ? 0x8000 : 0;
+  if (std::isnan(x)) return (uint16_t)(sign | 0x7FC0);
+  double a = std::fabs(x);
+  if (std::isinf(a)) return (uint16_t)(sign | 0x7F80);
+  if (a == 0.0) return sign;
+  int ex;
+  (void)std::frexp(a, &ex);
+  int e = ex - 1;                                    // a in [2^e, 2^(e+1))
+  int qexp = (e < -126) ? -133 : (e - 7);            // spacing of the bf16 grid around a
+  double scaled = std::ldexp(a, -qexp);              // exact, < 256
+  double fl = std::floor(scaled);
+  double rem = scaled - fl;
+  uint64_t n = (uint64_t)fl;
+  if (rem > 0.5 || (rem == 0.5 && (n & 1ULL))) n += 1;
+  uint32_t bits;
+  if (qexp == -133) {
+    bits = (uint32_t)n;                              // n in [0,128]; 128 == smallest normal 0x0080
+  } else {
+    int be = e + 127;
+    if (n == 256) { n = 128; be += 1; }
+    if (be >= 255) return (uint16_t)(sign | 0x7F80);
+    bits = ((uint32_t)be << 7) | (uint32_t)(n - 128);
+  }
+  return (uint16_t)(sign | bits);
+}
+
+inline uint16_t float_to_bf16_rn(float p) { return double_to_bf16_rn((double)p); }
+
+// z <- RN_bf16(z + v).  The sum is formed in double and rounded once to bf16.  When the exponents
+// are at most 44 apart the double sum is exact (8 + 44 + 1 <= 53 bits).  Otherwise |v| < 2^-43 |z|,
+// the exact sum lies strictly inside the rounding interval of z (half a bf16 spacing is >= 2^-10 |z|
+// away), and so does its double rounding: both round to z.  Either way this is the correctly
+// rounded bf16 sum (PAPER.md:253's recursion with u = 2^-8).
+inline uint16_t bf16_add_rn(uint16_t z, uint16_t v) {
+  return double_to_bf16_rn(bf16_to_double(z) + bf16_to_double(v));
+}
 
 // One FP32 multiply, single rounding (PAPER.md:127 `s * a0`).  volatile keeps
 // the compiler from contracting or widening it.
@@ -165,6 +228,51 @@ inline float mul_f32(float s, float a) {
   volatile float r = s * a;
   return r;
 }
+// One FP32 add, single rounding.
+inline float add_f32(float a, float b) {
+  volatile float r = a + b;
+  return r;
+}
+
+// ---------------------------------------------------------------------------
+// Dither conversion, Eq. (6):  Q_dith(q) = RN16(q + (u0 - 1/2) c q),
+// "a 24-bit variate u0 in [0,1) from an xorshift generator and the FP32 coefficient c written as
+// 0.00097656f ...; the perturbation is evaluated in FP32".  Reading R20: every
+// operation is one FP32 operation rounded to nearest, in the order the formula is written, no
+// fused multiply-add:  t = u0 - 1/2 (exact: a 24-bit integer times 2^-24),  w = fl(t * c),
+// e = fl(w * q),  q' = fl(q + e),  result RN16(q').
+// ---------------------------------------------------------------------------
+inline uint16_t float_to_half_dither(float q, uint32_t r24, float c) {
+  float u0 = (float)(r24 & 0xFFFFFFu) * 5.9604644775390625e-08f;  // r24 * 2^-24, exact
+  float t = u0 - 0.5f;                                            // exact
+  float w = mul_f32(t, c);
+  float e = mul_f32(w, q);
+  float qp = add_f32(q, e);
+  return float_to_half_rn(qp);
+}
+
+// One step of Marsaglia's xorshift64 generator (shifts 13, 7, 17; "Xorshift RNGs", 2003).
+inline uint64_t xorshift64(uint64_t x) {
+  x ^= x << 13;
+  x ^= x >> 7;
+  x ^= x << 17;
+  return x;
+}
+// The 64 dither bits of one column pair, reading R21: a xorshift64 generator seeded per
+// contribution pair from the counter hash (state 0, which xorshift cannot leave, is replaced by
+// the SplitMix64 increment), first output.  Bits 63..40 -> column 2*pair, bits 39..16 -> 2*pair+1
+// (the layout of reading R14).
+inline uint64_t dither_bits(uint64_t sr_seed, uint64_t ctr) {
+  uint64_t x = splitmix64(sr_seed ^ ctr);
+  if (x == 0) x = 0x9E3779B97F4A7C15ULL;
+  return xorshift64(x);
+}
+constexpr float kDitherC = 0.00097656f;  // PAPER.md:201, "approximately 2^-10"
+
+// s = fp32(1/sqrt(zeta)), correctly rounded from FP64 (reading R5; PAPER.md:161
+// "signed FP32 scale eps/sqrt(zeta)").
+inline float scale_f32(int32_t zeta) { return (float)(1.0 / std::sqrt((double)zeta)); }
+
 
 }  // namespace
 
@@ -178,6 +286,25 @@ double orc_half_to_double(uint16_t h) { return half_to_double(h); }
 uint16_t orc_add16(uint16_t z, uint16_t v) { return half_add_rn(z, v); }
 uint16_t orc_sr16(float p, uint32_t r24) { return float_to_half_sr(p, r24); }
 float orc_scale_f32(int32_t zeta) { return scale_f32(zeta); }
+
+uint16_t orc_bf16_rn(float p) { return float_to_bf16_rn(p); }
+double orc_bf16_to_double(uint16_t b) { return bf16_to_double(b); }
+uint16_t orc_bf16_add(uint16_t z, uint16_t v) { return bf16_add_rn(z, v); }
+uint64_t orc_xorshift64(uint64_t x) { return xorshift64(x); }
+float orc_dither_c(void) { return kDitherC; }
+void orc_bf16_rn_array(const float* p, int64_t count, uint16_t* out) {
+  for (int64_t k = 0; k < count; ++k) out[k] = float_to_bf16_rn(p[k]);
+}
+void orc_bf16_add_array(const uint16_t* z, const uint16_t* v, int64_t count, uint16_t* out) {
+  for (int64_t k = 0; k < count; ++k) out[k] = bf16_add_rn(z[k], v[k]);
+}
+void orc_bf16_to_double_array(const uint16_t* b, int64_t count, double* out) {
+  for (int64_t k = 0; k < count; ++k) out[k] = bf16_to_double(b[k]);
+}
+// Eq. (6) with an explicit coefficient, so the pins can set c = 0
+void orc_dither16_array(const float* p, const uint32_t* r24, float c, int64_t count, uint16_t* out) {
+  for (int64_t k = 0; k < count; ++k) out[k] = float_to_half_dither(p[k], r24[k], c);
+}
 
 void orc_rn16_array(const float* p, int64_t count, uint16_t* out) {
   for (int64_t k = 0; k < count; ++k) out[k] = float_to_half_rn(p[k]);
@@ -291,7 +418,8 @@ void orc_f64_finalize(int32_t zeta, int64_t count, double* B) {
 
 // --- SEQ16: one legal FP16 result (Listing 2 + PAPER.md:253) -----
 // rows ascending, blocks ascending (reading R8), every column:
-//   p = fp32(eps*s * a);  v = RN16(p) [or SR16(p, bits) if rounding==1];  D = RN16(D + v).
+//   p = fp32(eps*s * a);  v = RN16(p) [or SR16(p, bits) if rounding==1, or Q_dith(p) of Eq. (6) if
+//   rounding==2: same counter, bits through one xorshift64 step, reading R21];  D = RN16(D + v).
 // D is d x n row-major binary16 bit patterns, caller-initialised (+0 for a fresh sketch),
 // so rows can be streamed in chunks.  SR bits (reading R14):
 //   R = splitmix64(sr_seed ^ ((i*zeta+j)*ceil(n/2) + pair)); bits 63..40 -> column 2*pair,
@@ -317,6 +445,11 @@ int orc_seq16_accumulate(uint64_t seed, int32_t d, int32_t zeta, const float* A,
         uint16_t v;
         if (rounding == 0) {
           v = float_to_half_rn(p);
+        } else if (rounding == 2) {
+          uint64_t ctr = ((uint64_t)i * (uint64_t)zeta + (uint64_t)j) * npairs + (uint64_t)(c >> 1);
+          uint64_t R = dither_bits(sr_seed, ctr);
+          uint32_t r24 = (c & 1) ? (uint32_t)((R >> 16) & 0xFFFFFFu) : (uint32_t)(R >> 40);
+          v = float_to_half_dither(p, r24, kDitherC);
         } else {
           uint64_t ctr = ((uint64_t)i * (uint64_t)zeta + (uint64_t)j) * npairs + (uint64_t)(c >> 1);
           uint64_t R = splitmix64(sr_seed ^ ctr);
@@ -325,6 +458,28 @@ int orc_seq16_accumulate(uint64_t seed, int32_t d, int32_t zeta, const float* A,
         }
         drow[c] = half_add_rn(drow[c], v);
       }
+    }
+  }
+  return 0;
+}
+
+// --- SEQ-BF16: the same sequential loop with bfloat16 conversion and accumulation (the BF16
+// control of PAPER.md:382, :396): p = fp32(eps*s*a); v = RN_bf16(p); D = RN_bf16(D + v).
+// D is d x n row-major bfloat16 bit patterns, caller-initialised.
+int orc_seqbf16_accumulate(uint64_t seed, int32_t d, int32_t zeta, const float* A, int64_t row_begin,
+                           int64_t rows, int32_t n, int64_t lda, uint16_t* D) {
+  if (d <= 0 || zeta < 1 || d % zeta != 0 || n <= 0 || lda < n) return -1;
+  int32_t db = d / zeta;
+  float s = scale_f32(zeta);
+  for (int64_t r = 0; r < rows; ++r) {
+    const float* arow = A + r * lda;
+    for (int32_t j = 0; j < zeta; ++j) {
+      int32_t b;
+      uint32_t sb;
+      hash_ij(seed, row_begin + r, j, zeta, db, &b, &sb);
+      float es = sb ? -s : s;
+      uint16_t* drow = D + (int64_t)b * n;
+      for (int32_t c = 0; c < n; ++c) drow[c] = bf16_add_rn(drow[c], float_to_bf16_rn(mul_f32(es, arow[c])));
     }
   }
   return 0;
