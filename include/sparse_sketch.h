@@ -79,7 +79,8 @@ typedef struct sketch_opts {
   int64_t row_begin;  /* global index of the first row stored at A (rows are hashed by global index) */
   int64_t rows;       /* number of rows at A; 0 = m - row_begin */
   int32_t grid_ctas;  /* 0 = auto; tuning / tests only */
-  int32_t reserved;   /* must be 0 */
+  int32_t tmem_group_mode; /* 0 = auto; tuning / tests only, TMEM variant with bucket groups: 1 = chained groups,
+                              2 / 3 = deferral with groups of 4 / 8 rows (ignored where the geometry has no such mode) */
 } sketch_opts_t;
 
 /* ---- handle ------------------------------------------------------------------------------- */

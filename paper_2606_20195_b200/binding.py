@@ -25,7 +25,7 @@ class SketchOpts(C.Structure):
         ("row_begin", C.c_int64),
         ("rows", C.c_int64),
         ("grid_ctas", C.c_int32),
-        ("reserved", C.c_int32),
+        ("tmem_group_mode", C.c_int32),
     ]
 
 
@@ -98,9 +98,9 @@ def _stream_ptr(stream=None) -> int:
     return int(st.cuda_stream)
 
 
-def _opts(variant=0, replicas=0, hash_mode=0, accumulate=False, row_begin=0, rows=0, grid_ctas=0):
+def _opts(variant=0, replicas=0, hash_mode=0, accumulate=False, row_begin=0, rows=0, grid_ctas=0, tmem_group_mode=0):
     return SketchOpts(int(variant), int(replicas), int(hash_mode), int(bool(accumulate)), int(row_begin), int(rows),
-                      int(grid_ctas), 0)
+                      int(grid_ctas), int(tmem_group_mode))
 
 
 def _check_cuda(t, dtype, what):
@@ -160,6 +160,17 @@ class Sketch:
             raise ValueError("A must be 2-D row-major (unit column stride)")
         return A.data_ptr(), int(A.shape[1]), int(A.stride(0)) if A.shape[0] > 1 else max(int(A.stride(0)), int(A.shape[1]))
 
+    def _range_opts(self, A, opts):
+        """rows defaults to the rows of A.  The ABI reads rows = 0 as "through row m - 1", so an EMPTY A is passed as the
+        empty range that starts at m (nothing is read; B is zeroed unless accumulate is set)."""
+        opts = dict(opts)
+        opts.setdefault("rows", int(A.shape[0]))
+        if int(opts["rows"]) == 0:
+            if int(A.shape[0]) != 0:
+                raise ValueError("rows=0 is ambiguous: pass the number of rows of A")
+            opts["row_begin"] = self.m
+        return opts
+
     def apply_f32acc(self, A, out=None, stream=None, **opts):
         import torch
 
@@ -169,8 +180,7 @@ class Sketch:
         _check_cuda(out, torch.float32, "out")
         assert out.is_contiguous() and tuple(out.shape) == (self.d, n)
         if opts:
-            opts.setdefault("rows", A.shape[0])
-            o = _opts(**opts)
+            o = _opts(**self._range_opts(A, opts))
             rc = lib().sketch_apply_f32acc_ex(self._h, ap, n, lda, out.data_ptr(), C.byref(o), _stream_ptr(stream))
         else:
             if A.shape[0] != self.m:
@@ -189,8 +199,7 @@ class Sketch:
         _check_cuda(out, torch.float16, "out")
         assert out.is_contiguous() and tuple(out.shape) == (self.d, n)
         if opts:
-            opts.setdefault("rows", A.shape[0])
-            o = _opts(**opts)
+            o = _opts(**self._range_opts(A, opts))
             rc = lib().sketch_apply_f16acc_ex(self._h, ap, n, lda, out.data_ptr(), rounding, sr_seed & (2**64 - 1), C.byref(o),
                                               _stream_ptr(stream))
         else:
@@ -210,8 +219,7 @@ class Sketch:
         if out_host is None:
             out_host = torch.empty((self.d, n), dtype=torch.float16, pin_memory=True)
         assert not out_host.is_cuda and out_host.dtype == torch.float16 and out_host.is_contiguous()
-        opts.setdefault("rows", A_host.shape[0])
-        o = _opts(**opts)
+        o = _opts(**self._range_opts(A_host, opts))
         rc = lib().sketch_apply_f16acc_host(self._h, A_host.data_ptr(), n, int(A_host.stride(0)), out_host.data_ptr(), rounding,
                                             sr_seed & (2**64 - 1), C.byref(o))
         if rc:
@@ -226,8 +234,7 @@ class Sketch:
         if out_host is None:
             out_host = torch.empty((self.d, n), dtype=torch.float32, pin_memory=True)
         assert not out_host.is_cuda and out_host.dtype == torch.float32 and out_host.is_contiguous()
-        opts.setdefault("rows", A_host.shape[0])
-        o = _opts(**opts)
+        o = _opts(**self._range_opts(A_host, opts))
         rc = lib().sketch_apply_f32acc_host(self._h, A_host.data_ptr(), n, int(A_host.stride(0)), out_host.data_ptr(), C.byref(o))
         if rc:
             raise SketchError(rc, "sketch_apply_f32acc_host")

@@ -19,7 +19,8 @@ struct ScatterArgs {
   uint64_t sr_seed;
   float scale;          // fp32(1/sqrt(zeta)), correctly rounded on the host (R5)
   uint32_t cpr;         // chunks of VEC columns per row = n / VEC
-  uint32_t cpr_magic;   // ceil(2^32 / cpr): c / cpr == umulhi(c, magic) for c*cpr < 2^32
+  uint32_t cpr_magic;   // ceil(2^32 / cpr): c / cpr == umulhi(c, magic) while c * cpr < 2^32; 0 = cpr is 1; ~0 = use c / cpr
+  int64_t odd_tail;     // k_generic, FP16 straight into B: index of the last element when d*n is odd (added by CAS), else -1
   const void* packed;   // hash_mode 2: packed entries for global rows, index i*zeta + j (ranked u16 or u32); else nullptr
 };
 

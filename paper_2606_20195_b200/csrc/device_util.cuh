@@ -116,6 +116,18 @@ SK_DEVINL void red_h1(__half* p, uint16_t v) {
   red_h2(reinterpret_cast<void*>(a & ~(uintptr_t)3), word);
 }
 
+// The last element of a sketch with an odd number of elements has no partner inside B: its enclosing word would
+// reach two bytes past the buffer.  That one element is added with a 16-bit compare-and-swap loop instead.
+SK_DEVINL void red_h1_cas(__half* p, uint16_t v) {
+  unsigned short* q = reinterpret_cast<unsigned short*>(p);
+  unsigned short old = *reinterpret_cast<volatile unsigned short*>(q), assumed;
+  do {
+    assumed = old;
+    const __half sum = __hadd(__ushort_as_half(assumed), __ushort_as_half(v));
+    old = atomicCAS(q, assumed, __half_as_ushort(sum));
+  } while (old != assumed);
+}
+
 // ------------------------------------------------------------------------------------------------
 // Streaming loads of A: read once, never reused -> bypass L1 allocation; the 256-bit form also takes
 // L2::evict_first (ptxas accepts that modifier only on .v8.b32/.v4.b64 loads).

@@ -99,7 +99,8 @@ __global__ void __launch_bounds__(kFlatThreads) k_flat(ScatterArgs a) {
     }
     // ---- stream the HB x n floats
     for (uint32_t c = lane; c < ((chunks + 31u) & ~31u); c += 32) {
-      uint32_t rr = a.cpr_magic ? __umulhi(c, a.cpr_magic) : c;  // c / cpr (magic 0 <=> cpr == 1)
+      // c / cpr: magic 0 <=> cpr == 1; magic ~0 <=> the multiply-high form is not exact for this width (host: make_args)
+      uint32_t rr = a.cpr_magic == 0u ? c : (a.cpr_magic == 0xFFFFFFFFu ? c / a.cpr : __umulhi(c, a.cpr_magic));
       uint32_t ch = c - rr * a.cpr;
       bool valid = (c < chunks) && (r0 + rr < a.rows);
       rr = valid ? rr : 0u;
@@ -158,7 +159,8 @@ __global__ void __launch_bounds__(kFlatThreads) k_generic(ScatterArgs a) {
           uint32_t r24 = (c & 1) ? ((uint32_t)(R >> 16) & 0xFFFFFFu) : (uint32_t)(R >> 40);
           v = (uint16_t)sr16_bits(ps, r24);
         }
-        red_h1(reinterpret_cast<__half*>(Bbase) + off, v);
+        if (off == a.odd_tail) red_h1_cas(reinterpret_cast<__half*>(Bbase) + off, v);   // last element of an odd-sized B
+        else red_h1(reinterpret_cast<__half*>(Bbase) + off, v);
       } else {
         red_f1(reinterpret_cast<float*>(Bbase) + off, ps);
       }

@@ -1,13 +1,35 @@
 // launch.h -- host-side launchers, one translation unit per kernel family so nvcc compiles them in parallel.
-// Each returns the launch status (cudaGetLastError) or cudaErrorInvalidValue for an unsupported combination.
+// Each returns the launch status (cudaGetLastError), or kNoKernel when no instantiation exists for the combination
+// -- the host-side plan rules those out before anything is launched, so seeing it is an internal error.
 #pragma once
 
 #include <cuda.h>
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 #include "args.h"
 
 namespace sk {
+
+constexpr cudaError_t kNoKernel = cudaErrorInvalidDeviceFunction;
+
+// Raise a kernel's dynamic-shared-memory limit to the device's opt-in maximum, once per (kernel, device): the hot
+// call then does no cudaFuncSetAttribute (SURVEY 8b "never allocates per call"; a captured stream sees launches only).
+template <auto Kernel>
+inline cudaError_t allow_max_dynamic_smem() {
+  static std::atomic<uint64_t> done{0};   // bit per device ordinal
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 64 && ((done.load(std::memory_order_acquire) >> dev) & 1ull)) return cudaSuccess;
+  int optin = 0;
+  e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(Kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+  if (e == cudaSuccess && dev < 64) done.fetch_or(1ull << dev, std::memory_order_release);
+  return e;
+}
 
 cudaError_t launch_flat_f16(const ScatterArgs& a, int zeta, int vec, int rounding, int packed_width, int grid,
                             cudaStream_t st);
@@ -32,10 +54,12 @@ int small_warps();
 struct TmemShape {
   int X, S, BQ, CS, NW, GM;
 };
-bool tmem_shape(int n, int d, int zeta, int64_t lda, TmemShape* out);
+bool tmem_shape(int n, int d, int zeta, int64_t lda, int gm_force /* -1 = auto */, TmemShape* out);
+bool tmem_tensor_map_ok(int64_t lda, int64_t rows, int n_cta);
+cudaError_t tmem_make_tensor_map(const float* A, int n, int64_t lda, int64_t rows, int n_cta, int box_rows, CUtensorMap* out);
 size_t tmem_smem_bytes_for(int zeta, int n_cta, int bq, int gm);  // n_cta = n / CS
 int tmem_rows_per_stage(int n_cta, int bq, int zeta);
-cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, const TmemShape& h, int grid, cudaStream_t st);
+cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, const TmemShape& h, const CUtensorMap* tmap, int grid, cudaStream_t st);
 cudaError_t launch_tmem_z1(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st);
 cudaError_t launch_tmem_z2(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st);
 cudaError_t launch_tmem_z4(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st);

@@ -20,7 +20,7 @@ cudaError_t by_vec(const ScatterArgs& a, int vec, int pw, int grid, cudaStream_t
     case 4: return go<ZETA, 4, RND>(a, pw, grid, st);
     case 2: return go<ZETA, 2, RND>(a, pw, grid, st);
   }
-  return cudaErrorInvalidValue;
+  return kNoKernel;
 }
 
 template <int RND>
@@ -31,7 +31,7 @@ cudaError_t by_zeta(const ScatterArgs& a, int zeta, int vec, int pw, int grid, c
     case 4: return by_vec<4, RND>(a, vec, pw, grid, st);
     case 8: return by_vec<8, RND>(a, vec, pw, grid, st);
   }
-  return cudaErrorInvalidValue;
+  return kNoKernel;
 }
 
 }  // namespace

@@ -20,7 +20,7 @@ cudaError_t by_vec(const ScatterArgs& a, int vec, int pw, int grid, cudaStream_t
     case 2: return go<ZETA, 2>(a, pw, grid, st);
     case 1: return go<ZETA, 1>(a, pw, grid, st);
   }
-  return cudaErrorInvalidValue;
+  return kNoKernel;
 }
 
 }  // namespace
@@ -32,7 +32,7 @@ cudaError_t launch_flat_f32(const ScatterArgs& a, int zeta, int vec, int packed_
     case 4: return by_vec<4>(a, vec, packed_width, grid, st);
     case 8: return by_vec<8>(a, vec, packed_width, grid, st);
   }
-  return cudaErrorInvalidValue;
+  return kNoKernel;
 }
 
 cudaError_t launch_generic(const ScatterArgs& a, bool f16, int rounding, int grid, cudaStream_t st) {

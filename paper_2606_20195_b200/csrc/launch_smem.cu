@@ -10,13 +10,13 @@ template <int ZETA>
 cudaError_t go(const SmemArgs& g, int wpc, int grid, size_t smem_bytes, cudaStream_t st) {
   cudaError_t e;
   if (wpc <= 4) {
-    auto k = k_smem<ZETA, smem_batch_steps(ZETA, true), 4>;
-    e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    constexpr auto k = k_smem<ZETA, smem_batch_steps(ZETA, true), 4>;
+    e = allow_max_dynamic_smem<k>();
     if (e != cudaSuccess) return e;
     k<<<grid, wpc * 32, smem_bytes, st>>>(g);
   } else {
-    auto k = k_smem<ZETA, smem_batch_steps(ZETA, false), 16>;
-    e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    constexpr auto k = k_smem<ZETA, smem_batch_steps(ZETA, false), 16>;
+    e = allow_max_dynamic_smem<k>();
     if (e != cudaSuccess) return e;
     k<<<grid, wpc * 32, smem_bytes, st>>>(g);
   }
@@ -32,15 +32,15 @@ cudaError_t launch_smem_f16(const SmemArgs& g, int zeta, int wpc, int grid, size
     case 4: return go<4>(g, wpc, grid, smem_bytes, st);
     case 8: return go<8>(g, wpc, grid, smem_bytes, st);
   }
-  return cudaErrorInvalidValue;
+  return kNoKernel;
 }
 
 namespace {
 template <int ZETA>
 cudaError_t go_small(const SmallArgs& g, int grid, size_t smem_bytes, cudaStream_t st) {
-  auto k = k_small<ZETA>;
+  constexpr auto k = k_small<ZETA>;
   if (smem_bytes > 48 * 1024) {
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    cudaError_t e = allow_max_dynamic_smem<k>();
     if (e != cudaSuccess) return e;
   }
   k<<<grid, kSmallWarps * 32, smem_bytes, st>>>(g);
@@ -55,7 +55,7 @@ cudaError_t launch_small_f16(const SmallArgs& g, int zeta, int grid, size_t smem
     case 4: return go_small<4>(g, grid, smem_bytes, st);
     case 8: return go_small<8>(g, grid, smem_bytes, st);
   }
-  return cudaErrorInvalidValue;
+  return kNoKernel;
 }
 int small_warps() { return kSmallWarps; }
 
@@ -70,7 +70,7 @@ cudaError_t launch_hash_pack_rot(uint64_t seed, int zeta, int64_t rows, uint32_t
     case 2: k_hash_pack_rot<2><<<grid, 256, 0, st>>>(seed, rows, db, out); break;
     case 4: k_hash_pack_rot<4><<<grid, 256, 0, st>>>(seed, rows, db, out); break;
     case 8: k_hash_pack_rot<8><<<grid, 256, 0, st>>>(seed, rows, db, out); break;
-    default: return cudaErrorInvalidValue;
+    default: return kNoKernel;
   }
   return cudaGetLastError();
 }

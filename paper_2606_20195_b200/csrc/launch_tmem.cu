@@ -1,7 +1,6 @@
 // launch_tmem.cu -- instantiations of the tensor-memory-privatised scatter.  Compiled once per zeta
 // (-DSK_TMEM_ZETA=1|2|4|8) so the four families build in parallel; the zeta = 4 unit also holds the
 // shape logic and the dispatcher.
-#include <cstdlib>
 #include <cstring>
 
 #include "kernel_tmem.cuh"
@@ -18,11 +17,11 @@ template <int X, int S, int BQ, int NW, int GM>
 cudaError_t go(const TmemArgs& g, const CUtensorMap& tmap, int grid, int cs, cudaStream_t st) {
   constexpr int Z = SK_TMEM_ZETA, N = 64 * X * S;
   if constexpr (Z % BQ != 0) {
-    return cudaErrorInvalidValue;
+    return kNoKernel;
   } else {
-    auto k = k_tmem<Z, X, S, BQ, NW, GM>;
+    constexpr auto k = k_tmem<Z, X, S, BQ, NW, GM>;
     const size_t smem = tmem_smem_bytes(Z, N, BQ, GM);
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = allow_max_dynamic_smem<k>();
     if (e != cudaSuccess) return e;
     k<<<dim3((unsigned)grid, (unsigned)cs), (NW + tmem_producers(N, BQ, GM, Z)) * 32, smem, st>>>(g, tmap);
     return cudaGetLastError();
@@ -52,7 +51,7 @@ cudaError_t dispatch(const TmemArgs& g, const TmemShape& h, const CUtensorMap& t
       case 414: return h.GM == 1 ? go<4, 1, 4, 4, 1>(g, tmap, grid, h.CS, st) : h.GM == 2 ? go<4, 1, 4, 4, 2>(g, tmap, grid, h.CS, st) : go<4, 1, 4, 4, 0>(g, tmap, grid, h.CS, st);
     }
   }
-  return cudaErrorInvalidValue;
+  return kNoKernel;
 }
 
 }  // namespace
@@ -68,9 +67,9 @@ cudaError_t launch_tmem_z4(const TmemArgs& g, const TmemShape& h, const CUtensor
 
 // Geometry for an n-feature, d-row, zeta-block sketch: the fewest column slices CS that fit at all, then
 // the (X, S, BQ) with the fewest issued instructions per KiB of A.  Model (from the SASS of the main loop,
-// profiles/r02_tmem_shapes.md): a row slice of 256 X bytes costs 1 + 3 X instructions to load and convert
+// profiles/r01_tmem_shapes.md): a row slice of 256 X bytes costs 1 + 3 X instructions to load and convert
 // (in each of the BQ warps that need it) and 5.25 + 2 X per stack block to read-modify-write.
-bool tmem_shape(int n, int d, int zeta, int64_t lda, TmemShape* out) {
+bool tmem_shape(int n, int d, int zeta, int64_t lda, int gm_force, TmemShape* out) {
   if (n <= 0 || d <= 0 || zeta <= 0 || n % 64 != 0 || d % zeta != 0) return false;
   const int NW = 4;
   for (int cs = 1; cs <= 16; ++cs) {   // odd slice counts serve the widths that are not 64 * 2^k (192, 320, 384, ...)
@@ -98,11 +97,8 @@ bool tmem_shape(int n, int d, int zeta, int64_t lda, TmemShape* out) {
           // 5.07 TB/s).  Deferral needs few clashes -- ZB * C(4,2) / (d/zeta) <= 0.15 -- and d/zeta >= G (G + 1).
           const double zb = (double)zeta / bq, dbk = (double)d / zeta;
           out->GM = (bq == 4 && zb * 6.0 / dbk <= 0.15 && dbk >= 20) ? 1 : 0;
-          static const char* const ev = getenv("SK_TMEM_GM");   // experiments only (read once)
-          if (ev) {
-            const int gm = atoi(ev);
-            if (bq > 1 && (gm == 0 || (gm == 1 && dbk >= 20) || (gm == 2 && dbk >= 72))) out->GM = gm;
-          }
+          // tuning / tests (sketch_opts_t::tmem_group_mode): forced where the mode exists for this geometry
+          if (gm_force >= 0 && bq > 1 && (gm_force == 0 || (gm_force == 1 && dbk >= 20) || (gm_force == 2 && dbk >= 72))) out->GM = gm_force;
         }
       }
     }
@@ -114,8 +110,14 @@ bool tmem_shape(int n, int d, int zeta, int64_t lda, TmemShape* out) {
 size_t tmem_smem_bytes_for(int zeta, int n_cta, int bq, int gm) { return tmem_smem_bytes(zeta, n_cta, bq, gm); }
 int tmem_rows_per_stage(int n_cta, int bq, int zeta) { return tmem_stage_rows(n_cta, bq, zeta); }
 
-// 2-D tensor map over the row range: {n features, rows} FP32, row pitch lda, box {n / CS features, T rows}
-cudaError_t make_tensor_map(const TmemArgs& g, int n_cta, int bq, int zeta, CUtensorMap* out) {
+// 2-D tensor map over the row range: {n features, rows} FP32, row pitch lda, box {n_cta features, box_rows rows}.
+// Limits (checked by tmem_tensor_map_ok, i.e. by the plan): coordinates are int32, the row pitch is a multiple of 16
+// bytes below 2^40, a box side is at most 256 elements.
+bool tmem_tensor_map_ok(int64_t lda, int64_t rows, int n_cta) {
+  return rows <= 0x7FFFFFFFll && lda % 4 == 0 && lda * 4 < (1ll << 40) && n_cta <= 256;
+}
+
+cudaError_t tmem_make_tensor_map(const float* A, int n, int64_t lda, int64_t rows, int n_cta, int box_rows, CUtensorMap* out) {
   typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -128,32 +130,28 @@ cudaError_t make_tensor_map(const TmemArgs& g, int n_cta, int bq, int zeta, CUte
     if (q != cudaDriverEntryPointSuccess || !p) return cudaErrorNotSupported;
     fn = reinterpret_cast<encode_fn>(p);
   }
-  const cuuint64_t dims[2] = {(cuuint64_t)g.s.n, (cuuint64_t)g.s.rows};
-  const cuuint64_t strides[1] = {(cuuint64_t)g.s.lda * 4};
-  const cuuint32_t box[2] = {(cuuint32_t)n_cta, (cuuint32_t)tmem_stage_rows(n_cta, bq, zeta)};
+  const cuuint64_t dims[2] = {(cuuint64_t)n, (cuuint64_t)rows};
+  const cuuint64_t strides[1] = {(cuuint64_t)lda * 4};
+  const cuuint32_t box[2] = {(cuuint32_t)n_cta, (cuuint32_t)box_rows};
   const cuuint32_t estr[2] = {1, 1};
-  CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(g.s.A), dims, strides, box, estr,
+  CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(A), dims, strides, box, estr,
                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, const TmemShape& h, int grid, cudaStream_t st) {
-  if (64 * h.X * h.S * h.CS != g.s.n) return cudaErrorInvalidValue;
-  CUtensorMap tmap;
-  memset(&tmap, 0, sizeof(tmap));
-  if (g.s.lda != g.s.n / h.CS) {   // the kernel's non-contiguous path
-    if (g.s.rows > 0x7FFFFFFF) return cudaErrorInvalidValue;
-    cudaError_t e = make_tensor_map(g, g.s.n / h.CS, h.BQ, zeta, &tmap);
-    if (e != cudaSuccess) return e;
-  }
+// tmap: the tensor map of this (A, n, lda, rows, geometry) when the tile is not contiguous (lda != n / CS), else ignored
+cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, const TmemShape& h, const CUtensorMap* tmap, int grid, cudaStream_t st) {
+  if (64 * h.X * h.S * h.CS != g.s.n) return kNoKernel;
+  static const CUtensorMap kNoMap = {};
+  const CUtensorMap& tm = (g.s.lda != g.s.n / h.CS) ? *tmap : kNoMap;
   switch (zeta) {
-    case 1: return launch_tmem_z1(g, h, tmap, grid, st);
-    case 2: return launch_tmem_z2(g, h, tmap, grid, st);
-    case 4: return launch_tmem_z4(g, h, tmap, grid, st);
-    case 8: return launch_tmem_z8(g, h, tmap, grid, st);
+    case 1: return launch_tmem_z1(g, h, tm, grid, st);
+    case 2: return launch_tmem_z2(g, h, tm, grid, st);
+    case 4: return launch_tmem_z4(g, h, tm, grid, st);
+    case 8: return launch_tmem_z8(g, h, tm, grid, st);
   }
-  return cudaErrorInvalidValue;
+  return kNoKernel;
 }
 #endif
 

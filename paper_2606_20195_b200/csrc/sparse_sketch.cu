@@ -56,6 +56,20 @@ struct sketch {
   cudaStream_t st_copy, st_comp;
   cudaEvent_t ev_copied[2], ev_done[2];
   int host_ready;
+  // stream ordering of the library-owned scratch (rep, packed): the last stream that used it and an event recorded
+  // behind that use; an apply on another stream waits for the event first
+  cudaStream_t scratch_stream;
+  cudaEvent_t ev_scratch;
+  int scratch_busy;   // 0 = never used, 1 = ev_scratch is valid
+  // tensor maps of the strided / column-sliced tensor-memory launches, keyed by what they encode (a handle is applied
+  // to the same few matrices over and over: the hot call then does no encoding)
+  struct TmapSlot {
+    const float* A;
+    int64_t lda, rows;
+    int32_t n, n_cta, box_rows;
+    CUtensorMap map;
+  } tmaps[8];
+  int tmap_count, tmap_next;
 };
 
 namespace {
@@ -111,10 +125,11 @@ bool smem_feasible(const sketch* s, int n, int64_t lda, const void* A, const voi
   return true;
 }
 
-bool tmem_feasible(const sketch* s, int n, int64_t lda, const void* A, const void* B, sk::TmemShape* h) {
+bool tmem_feasible(const sketch* s, int n, int64_t lda, int64_t rows, const void* A, const void* B, int gm_force, sk::TmemShape* h) {
   if (!zeta_templated(s->zeta)) return false;
-  if (!sk::tmem_shape(n, s->d, s->zeta, lda, h)) return false;
+  if (!sk::tmem_shape(n, s->d, s->zeta, lda, gm_force, h)) return false;
   if (lda % 4 != 0 || !aligned(A, 16) || !aligned(B, 16)) return false;  // TMA bulk copies: 16-byte granules
+  if (lda != n / h->CS && !sk::tmem_tensor_map_ok(lda, rows, n / h->CS)) return false;   // the 2-D tensor-map path
   return sk::tmem_smem_bytes_for(s->zeta, n / h->CS, h->BQ, h->GM) <= (size_t)s->smem_optin;
 }
 
@@ -148,14 +163,16 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
   bool sm_ok = f16 && rounding == SKETCH_RN && smem_feasible(s, n, lda, A, B, &sm_bytes) &&
                (rb0 % sk::smem_step_rows(s->zeta) == 0);
   sk::TmemShape tm = {0, 0, 0, 0, 0, 0};
-  bool tm_ok = f16 && rounding == SKETCH_RN && tmem_feasible(s, n, lda, A, B, &tm);
+  const int gm_force = (o ? o->tmem_group_mode : 0) - 1;
+  bool tm_ok = f16 && rounding == SKETCH_RN && tmem_feasible(s, n, lda, rows, A, B, gm_force, &tm);
   // per-warp shared-memory partials (kernel_small.cuh)
   const size_t small_bytes = (size_t)sk::small_warps() * s->d * n * 2;
   bool small_ok = f16 && rounding == SKETCH_RN && zeta_templated(s->zeta) && n % 2 == 0 && lda % 2 == 0 && aligned(A, 8) &&
                   small_bytes <= (size_t)s->smem_optin;
   int vmax = flat_vec_for(f16, n, lda, A, B, 8);
   int vpair = flat_vec_for(f16, n, lda, A, B, f16 ? 2 : 1);
-  bool zt = zeta_templated(s->zeta);
+  // the flat kernels index the chunks of a (32 / zeta)-row macro step with 32 bits
+  bool zt = zeta_templated(s->zeta) && (int64_t)n * (32 / (zeta_templated(s->zeta) ? s->zeta : 1)) < (1ll << 31);
 
   int v = want;
   if (v == SKETCH_VARIANT_AUTO) {
@@ -286,6 +303,10 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
   return SKETCH_OK;
 }
 
+// elements between two partial sketches / result slots: padded to 16 bytes so that every partial keeps the vector-RED
+// alignment of the first (d * n may be odd)
+inline int64_t padded_count(int64_t count) { return (count + 7) / 8 * 8; }
+
 sk::ScatterArgs make_args(const sketch* s, const float* A, int n, int64_t lda, void* B, int64_t row_begin,
                           int64_t rows, uint64_t sr_seed, int vec) {
   sk::ScatterArgs a;
@@ -294,8 +315,9 @@ sk::ScatterArgs make_args(const sketch* s, const float* A, int n, int64_t lda, v
   a.row_begin = row_begin;
   a.rows = rows;
   a.B = B;
-  a.replica_stride = (int64_t)s->d * n;
+  a.replica_stride = padded_count((int64_t)s->d * n);
   a.replicas = 1;
+  a.odd_tail = -1;
   a.n = n;
   a.zeta = s->zeta;
   a.db = s->db;
@@ -303,15 +325,61 @@ sk::ScatterArgs make_args(const sketch* s, const float* A, int n, int64_t lda, v
   a.sr_seed = sr_seed;
   a.scale = s->scale;
   a.cpr = (uint32_t)(n / (vec > 0 ? vec : 1));
-  a.cpr_magic = (a.cpr <= 1) ? 0u : (uint32_t)(((1ull << 32) + a.cpr - 1) / a.cpr);
+  // c / cpr by multiply-high: with magic = ceil(2^32 / cpr), umulhi(c, magic) is exact while c * (magic * cpr - 2^32) <
+  // 2^32; the excess is below cpr and c below (32 / zeta) * cpr, so (32 / zeta) * cpr^2 <= 2^32 suffices.  Wider rows
+  // (n ~ 16k and up) divide.
+  const uint64_t cmax = (uint64_t)(32 / (s->zeta <= 32 ? (s->zeta > 0 ? s->zeta : 1) : 32)) * a.cpr;
+  a.cpr_magic = (a.cpr <= 1) ? 0u : (cmax * a.cpr <= (1ull << 32)) ? (uint32_t)(((1ull << 32) + a.cpr - 1) / a.cpr) : 0xFFFFFFFFu;
   a.packed = nullptr;
   return a;
 }
 
+// Every feasibility condition is decided on the host by make_plan, before anything is enqueued: a failing launch is
+// a CUDA error (SKETCH_ERR_CUDA, text in sketch_last_error), never "unsupported".
 int launched(cudaError_t e, const char* what) {
+  if (e != cudaSuccess) return cuda_fail(e, what);
   g_launches.fetch_add(1, std::memory_order_relaxed);
-  if (e == cudaErrorInvalidValue) return SKETCH_ERR_UNSUPPORTED;
-  return e == cudaSuccess ? SKETCH_OK : cuda_fail(e, what);
+  return SKETCH_OK;
+}
+
+// Order the library-owned scratch behind its previous use when the caller switches streams.  Inside a stream capture
+// nothing is recorded or waited for (events cannot cross a capture): captured applies that share scratch must be
+// ordered by the caller (include/sparse_sketch.h).
+int scratch_acquire(sketch* s, cudaStream_t st, bool* capturing) {
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  CU_TRY(cudaStreamIsCapturing(st, &cs));
+  *capturing = cs != cudaStreamCaptureStatusNone;
+  if (*capturing) return SKETCH_OK;
+  if (s->scratch_busy && s->scratch_stream != st) CU_TRY(cudaStreamWaitEvent(st, s->ev_scratch, 0));
+  return SKETCH_OK;
+}
+int scratch_release(sketch* s, cudaStream_t st, bool capturing) {
+  if (capturing) return SKETCH_OK;
+  if (!s->ev_scratch) CU_TRY(cudaEventCreateWithFlags(&s->ev_scratch, cudaEventDisableTiming));
+  CU_TRY(cudaEventRecord(s->ev_scratch, st));
+  s->scratch_stream = st;
+  s->scratch_busy = 1;
+  return SKETCH_OK;
+}
+
+// tensor map of a strided / column-sliced tensor-memory launch, from the handle's cache
+int tensor_map_for(sketch* s, const float* A, int n, int64_t lda, int64_t rows, int n_cta, int box_rows, const CUtensorMap** out) {
+  for (int k = 0; k < s->tmap_count; ++k) {
+    const sketch::TmapSlot& t = s->tmaps[k];
+    if (t.A == A && t.lda == lda && t.rows == rows && t.n == n && t.n_cta == n_cta && t.box_rows == box_rows) {
+      *out = &t.map;
+      return SKETCH_OK;
+    }
+  }
+  const int slot = s->tmap_next;
+  sketch::TmapSlot& t = s->tmaps[slot];
+  cudaError_t e = sk::tmem_make_tensor_map(A, n, lda, rows, n_cta, box_rows, &t.map);
+  if (e != cudaSuccess) return cuda_fail(e, "cuTensorMapEncodeTiled");
+  t.A = A; t.lda = lda; t.rows = rows; t.n = n; t.n_cta = n_cta; t.box_rows = box_rows;
+  s->tmap_next = (slot + 1) % 8;
+  if (s->tmap_count < 8) ++s->tmap_count;
+  *out = &t.map;
+  return SKETCH_OK;
 }
 
 // a1 in its precomputed form.  16-bit entries in sub-step order (kernel_smem.cuh) when zeta is templated and the
@@ -348,7 +416,7 @@ int validate_apply(const sketch* s, const void* A, int32_t n, int64_t lda, const
   (void)f16;
   int64_t rb = o ? o->row_begin : 0;
   int64_t r = o ? o->rows : 0;
-  if (o && o->reserved != 0) return SKETCH_ERR_INVALID;
+  if (o && (o->tmem_group_mode < 0 || o->tmem_group_mode > 3)) return SKETCH_ERR_INVALID;
   if (rb < 0 || r < 0 || rb > s->m) return SKETCH_ERR_INVALID;
   if (r == 0) r = s->m - rb;
   if (rb + r > s->m) return SKETCH_ERR_INVALID;
@@ -378,7 +446,13 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
       sk::TmemArgs g;
       g.s = make_args(s, A, n, lda, B, row_begin, rows, sr_seed, 1);
       g.d = s->d;
-      rc = launched(sk::launch_tmem_f16(g, s->zeta, p.tm, p.grid, st), "k_tmem");
+      const CUtensorMap* tmap = nullptr;
+      const int n_cta = n / p.tm.CS;
+      if (lda != n_cta) {
+        rc = tensor_map_for(s, A, n, lda, rows, n_cta, sk::tmem_rows_per_stage(n_cta, p.tm.BQ, s->zeta), &tmap);
+        if (rc) return rc;
+      }
+      rc = launched(sk::launch_tmem_f16(g, s->zeta, p.tm, tmap, p.grid, st), "k_tmem");
       if (rc) return rc;
     }
     return SKETCH_OK;
@@ -405,10 +479,15 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
       g.rows_per_cta = p.rows_per_cta;
       g.d = s->d;
       g.zero = 0u;
+      bool capturing = false;
+      rc = scratch_acquire(s, st, &capturing);
+      if (rc) return rc;
       rc = ensure_packed(s, st, false);
       if (rc) return rc;
       g.s.packed = s->packed;
       rc = launched(sk::launch_smem_f16(g, s->zeta, p.wpc, p.grid, p.smem_bytes, st), "k_smem");
+      if (rc) return rc;
+      rc = scratch_release(s, st, capturing);
       if (rc) return rc;
     }
     return SKETCH_OK;
@@ -417,16 +496,25 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
   // flat / generic: RED into B itself (P == 1) or into P partial sketches folded afterwards
   void* target = B;
   int P = p.replicas;
+  const int64_t count = (int64_t)s->d * n;
+  const int64_t pstride = padded_count(count);      // elements between partial sketches
+  const bool packed_hashes = p.hash_mode == 2 && p.variant != SKETCH_VARIANT_GENERIC;
+  const bool uses_scratch = P > 1 || packed_hashes;
+  bool capturing = false;
+  if (uses_scratch) {
+    rc = scratch_acquire(s, st, &capturing);
+    if (rc) return rc;
+  }
   if (P > 1) {
-    rc = ensure_scratch(&s->rep, &s->rep_bytes, out_bytes * P);
+    rc = ensure_scratch(&s->rep, &s->rep_bytes, (size_t)pstride * elem * P);
     if (rc) return rc;
     target = s->rep;
-    CU_TRY(cudaMemsetAsync(target, 0, out_bytes * P, st));
+    CU_TRY(cudaMemsetAsync(target, 0, (size_t)pstride * elem * P, st));
   } else if (!accumulate) {
     CU_TRY(cudaMemsetAsync(B, 0, out_bytes, st));
   }
   int pw = 0;
-  if (p.hash_mode == 2 && p.variant != SKETCH_VARIANT_GENERIC) {
+  if (packed_hashes) {
     rc = ensure_packed(s, st, false);
     if (rc) return rc;
     pw = s->packed_width;
@@ -436,6 +524,7 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
     a.replicas = P;
     a.packed = pw ? s->packed : nullptr;
     if (p.variant == SKETCH_VARIANT_GENERIC) {
+      if (f16 && P == 1 && (count & 1)) a.odd_tail = count - 1;
       rc = launched(sk::launch_generic(a, f16, rounding == SKETCH_SR, p.grid, st), "k_generic");
     } else if (!f16) {
       rc = launched(sk::launch_flat_f32(a, s->zeta, p.vec, pw, p.grid, st), "k_flat<f32>");
@@ -445,12 +534,15 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
     if (rc) return rc;
   }
   if (P > 1) {
-    int64_t count = (int64_t)s->d * n;
     int grid = (int)((count + 255) / 256);
     if (grid > s->sm_count * 8) grid = s->sm_count * 8;
-    if (f16) sk::k_reduce_replicas<true><<<grid, 256, 0, st>>>(target, count, P, B, count, accumulate);
-    else sk::k_reduce_replicas<false><<<grid, 256, 0, st>>>(target, count, P, B, count, accumulate);
+    if (f16) sk::k_reduce_replicas<true><<<grid, 256, 0, st>>>(target, pstride, P, B, count, accumulate);
+    else sk::k_reduce_replicas<false><<<grid, 256, 0, st>>>(target, pstride, P, B, count, accumulate);
     rc = launch_check("k_reduce_replicas");
+    if (rc) return rc;
+  }
+  if (uses_scratch) {
+    rc = scratch_release(s, st, capturing);
     if (rc) return rc;
   }
   return SKETCH_OK;
@@ -468,20 +560,12 @@ int ensure_host_path(sketch* s) {
   return SKETCH_OK;
 }
 
-int apply_host(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void* B, bool f16, int rounding,
-               uint64_t sr_seed, const sketch_opts_t* o) {
-  sketch* s = const_cast<sketch*>(cs);
-  if (!s || !A || !B) return SKETCH_ERR_NULL;
-  if (n <= 0) return SKETCH_ERR_INVALID;
-  if (lda < n) return SKETCH_ERR_LDA;
-  int64_t rb = o ? o->row_begin : 0, rows = o ? o->rows : 0;
-  if (rb < 0 || rows < 0 || rb > s->m) return SKETCH_ERR_INVALID;
-  if (rows == 0) rows = s->m - rb;
-  if (rb + rows > s->m) return SKETCH_ERR_INVALID;
-  int rc = ensure_host_path(s);
-  if (rc) return rc;
+int apply_host_impl(sketch* s, const float* A, int32_t n, int64_t lda, void* B, bool f16, int rounding, uint64_t sr_seed,
+                    const sketch_opts_t* o, int64_t rb, int64_t rows) {
+  int rc;
   const size_t elem = f16 ? 2 : 4;
   const size_t out_bytes = (size_t)s->d * n * elem;
+  const size_t slot_bytes = (size_t)padded_count((int64_t)s->d * n) * elem;   // 16-byte aligned slots (d * n may be odd)
   // staging: two buffers of ~256 MiB, whole rows, row count a multiple of 32
   const size_t row_bytes = (size_t)n * 4;
   int64_t chunk_rows = (int64_t)((256u << 20) / row_bytes);
@@ -502,10 +586,10 @@ int apply_host(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void*
   // on a single running sum (measured at c5: relF 2.5e-2 instead of 7e-3).
   const int64_t nchunks = rows > 0 ? (rows + chunk_rows - 1) / chunk_rows : 0;
   const int64_t kSlots = nchunks < 64 ? (nchunks > 0 ? nchunks : 1) : 64;
-  rc = ensure_scratch(&s->bdev, &s->bdev_bytes, out_bytes * (size_t)(kSlots + 1));
+  rc = ensure_scratch(&s->bdev, &s->bdev_bytes, slot_bytes * (size_t)(kSlots + 1));
   if (rc) return rc;
-  char* const slots = static_cast<char*>(s->bdev);            // [kSlots][d][n]
-  char* const result = slots + out_bytes * (size_t)kSlots;     // [d][n]
+  char* const slots = static_cast<char*>(s->bdev);            // [kSlots][padded d*n]
+  char* const result = slots + slot_bytes * (size_t)kSlots;    // [d][n]
   sketch_opts_t oo;
   memset(&oo, 0, sizeof(oo));
   if (o) oo = *o;
@@ -525,7 +609,7 @@ int apply_host(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void*
     oo.row_begin = rb + r0;
     oo.rows = nr;
     oo.accumulate = k >= kSlots ? 1 : 0;
-    rc = apply_device(s, (const float*)s->stage[b], n, n, slots + out_bytes * (size_t)(k % kSlots), f16, rounding, sr_seed, &oo,
+    rc = apply_device(s, (const float*)s->stage[b], n, n, slots + slot_bytes * (size_t)(k % kSlots), f16, rounding, sr_seed, &oo,
                       s->st_comp);
     if (rc) return rc;
     CU_TRY(cudaEventRecord(s->ev_done[b], s->st_comp));
@@ -534,14 +618,37 @@ int apply_host(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void*
     const int64_t count = (int64_t)s->d * n;
     int grid = (int)((count + 255) / 256);
     if (grid > s->sm_count * 8) grid = s->sm_count * 8;
-    if (f16) sk::k_reduce_replicas<true><<<grid, 256, 0, s->st_comp>>>(slots, count, (int)kSlots, result, count, user_acc);
-    else sk::k_reduce_replicas<false><<<grid, 256, 0, s->st_comp>>>(slots, count, (int)kSlots, result, count, user_acc);
+    if (f16) sk::k_reduce_replicas<true><<<grid, 256, 0, s->st_comp>>>(slots, padded_count(count), (int)kSlots, result, count, user_acc);
+    else sk::k_reduce_replicas<false><<<grid, 256, 0, s->st_comp>>>(slots, padded_count(count), (int)kSlots, result, count, user_acc);
     rc = launch_check("k_reduce_replicas (chunks)");
     if (rc) return rc;
   }
   CU_TRY(cudaMemcpyAsync(B, result, out_bytes, cudaMemcpyDeviceToHost, s->st_comp));
   CU_TRY(cudaStreamSynchronize(s->st_comp));
   return SKETCH_OK;
+}
+
+int apply_host(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void* B, bool f16, int rounding,
+               uint64_t sr_seed, const sketch_opts_t* o) {
+  sketch* s = const_cast<sketch*>(cs);
+  if (!s || !A || !B) return SKETCH_ERR_NULL;
+  if (n <= 0) return SKETCH_ERR_INVALID;
+  if (lda < n) return SKETCH_ERR_LDA;
+  int64_t rb = o ? o->row_begin : 0, rows = o ? o->rows : 0;
+  if (rb < 0 || rows < 0 || rb > s->m) return SKETCH_ERR_INVALID;
+  if (rows == 0) rows = s->m - rb;
+  if (rb + rows > s->m) return SKETCH_ERR_INVALID;
+  int rc = ensure_device(s);
+  if (rc) return rc;
+  rc = ensure_host_path(s);
+  if (rc) return rc;
+  rc = apply_host_impl(s, A, n, lda, B, f16, rounding, sr_seed, o, rb, rows);
+  if (rc) {
+    // no copy from the caller's A (or into its B) may still be in flight when the call returns
+    cudaStreamSynchronize(s->st_copy);
+    cudaStreamSynchronize(s->st_comp);
+  }
+  return rc;
 }
 
 }  // namespace
@@ -575,6 +682,7 @@ int sketch_destroy(sketch_t* s) {
   for (int k = 0; k < 2; ++k)
     if (s->stage[k]) cudaFree(s->stage[k]);
   if (s->bdev) cudaFree(s->bdev);
+  if (s->ev_scratch) cudaEventDestroy(s->ev_scratch);
   if (s->host_ready) {
     cudaStreamDestroy(s->st_copy);
     cudaStreamDestroy(s->st_comp);
@@ -603,7 +711,13 @@ int sketch_hashes_dump(const sketch_t* cs, int32_t* bucket_dev, uint8_t* signbit
 
 int sketch_precompute_hashes(sketch_t* s, void* stream) {
   if (!s) return SKETCH_ERR_NULL;
-  return ensure_packed(s, reinterpret_cast<cudaStream_t>(stream), true);
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  bool capturing = false;
+  int rc = scratch_acquire(s, st, &capturing);
+  if (rc) return rc;
+  rc = ensure_packed(s, st, true);
+  if (rc) return rc;
+  return scratch_release(s, st, capturing);
 }
 
 int sketch_apply_f32acc(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, float* B_dev, void* stream) {
