@@ -50,6 +50,8 @@ typedef struct sketch sketch_t; /* opaque, library-owned */
 /* conversion rule of the FP16 path (Sec. III-D) */
 #define SKETCH_RN 0 /* round-to-nearest-even, __float2half semantics */
 #define SKETCH_SR 1 /* stochastic conversion with counter-based bits (readings R13, R14) */
+#define SKETCH_DITHER 2 /* dither conversion, Eq. (6): RN16(q + (u0 - 1/2) c q), c = 0.00097656f, u0 a 24-bit variate,
+                           every operation one FP32 rounding (readings R20, R21) */
 
 /* kernel variants (all compute the same sums; they differ in where partial sums live) */
 #define SKETCH_VARIANT_AUTO 0      /* chosen per shape from measurement */
@@ -60,10 +62,18 @@ typedef struct sketch sketch_t; /* opaque, library-owned */
 #define SKETCH_VARIANT_GENERIC 4   /* any n / any alignment scalar fallback (one lane per element) */
 #define SKETCH_VARIANT_TMEM 5      /* tensor-memory-privatised partial sketch per warp (tcgen05.ld / tcgen05.st read-
                                       modify-write), A staged by TMA, hashes computed on the fly by a producer
-                                      warp; FP16-RN, zeta in {1,2,4,8}, n = 64*X*S*CS with X, S in {1,2,4}, CS in 1..16,
-                                      BQ in {1,2,4} bucket groups dividing zeta, S*BQ <= 4 and (d/BQ)*X <= 512
-                                      (e.g. n = 256: d <= 2048), lda % 4 == 0, A and B 16-byte
-                                      aligned, rows < 2^31 when lda != n / CS (2-D tensor-map coordinates) */
+                                      warp; every accumulation mode (FP16 RN / SR / dither, bfloat16, FP32);
+                                      zeta in {1,2,4,8}, n = 32*FW*X*S*CS with FW = 2 features per 32-bit word for
+                                      the 16-bit sketches and 1 for FP32, X, S in {1,2,4}, CS in 1..16,
+                                      BQ in {1,2,4} bucket groups dividing zeta (SR / dither: BQ = 1), S*BQ <= 4 and
+                                      (d/BQ)*X <= 512 (e.g. FP16 n = 256: d <= 2048), lda % 4 == 0,
+                                      A and B 16-byte aligned, rows < 2^31 when lda != n / CS (2-D tensor-map
+                                      coordinates).
+                                      Overflow signature: partial sums live per warp and meet at the flush, so a
+                                      sketch entry whose partials overflowed to +inf in one warp and -inf in
+                                      another comes back NaN, where one running sum (FLAT with replicas = 1, or
+                                      the sequential order) sticks at +-inf.  Both are legal orders (reading R9);
+                                      count non-finite entries, not infinities, when comparing with PAPER.md:394 */
 #define SKETCH_VARIANT_SMALL 6     /* per-warp shared-memory partial sketches for small inputs and narrow matrices:
                                       FP16-RN, zeta in {1,2,4,8}, n and lda even, A 8-byte aligned,
                                       8*d*n*2 bytes of shared memory (AUTO picks it for launch-bound inputs) */
@@ -118,10 +128,15 @@ int sketch_apply_f32acc(const sketch_t* s, const float* A_dev, int32_t n, int64_
  * p = fp32(+-s * a), v = RN16(p) (or SR16), B16[bucket, c] = RN16(B16[bucket, c] + v), each FP16 component
  * independently, subnormals kept (.noftz), overflow -> +-inf.  The order of the additions is unspecified
  * ("Parallel atomic updates may also realize different orders").
- * B_dev: d x n IEEE binary16 row-major, overwritten.  rounding: SKETCH_RN / SKETCH_SR; sr_seed is used
- * only for SR.  Any n >= 1 is accepted (odd n runs the scalar GENERIC variant). */
+ * B_dev: d x n IEEE binary16 row-major, overwritten.  rounding: SKETCH_RN / SKETCH_SR / SKETCH_DITHER; sr_seed is
+ * used by SR and dither only.  Any n >= 1 is accepted (odd n runs the scalar GENERIC variant). */
 int sketch_apply_f16acc(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev,
                         int rounding, uint64_t sr_seed, void* stream);
+
+/* bfloat16-accumulate control (PAPER.md:382 Fig. 7, :396 "BF16 ... wider range"): the FP16 path with bfloat16 in
+ * place of binary16 -- p = fp32(+-s * a), v = RN_bf16(p), B[bucket, c] = RN_bf16(B[bucket, c] + v), subnormals kept.
+ * B_dev: d x n bfloat16 row-major, overwritten.  RN conversion only. */
+int sketch_apply_bf16acc(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev, void* stream);
 
 /* Same, with explicit options (variant override, row range, accumulate-into-B).  opts == NULL means
  * all-zero options, i.e. exactly the calls above. */
@@ -129,6 +144,26 @@ int sketch_apply_f32acc_ex(const sketch_t* s, const float* A_dev, int32_t n, int
                            const sketch_opts_t* opts, void* stream);
 int sketch_apply_f16acc_ex(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev,
                            int rounding, uint64_t sr_seed, const sketch_opts_t* opts, void* stream);
+
+int sketch_apply_bf16acc_ex(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev,
+                            const sketch_opts_t* opts, void* stream);
+
+/* ---- least-squares front end (PAPER.md:356 Sec. V-D; :312) ---------------------------------- */
+
+/* One pass over the rows for [A | b]: "We sketch A in the chosen precision and b in FP32 with the same map"
+ * (PAPER.md:356).  A as sketch_apply_f16acc (RN) / sketch_apply_f32acc; b_dev: FP32 vector, element k = the right-hand
+ * side of row (row_begin + k); Sb32_dev: d FP32 values, overwritten with S*b (or added to, with opts->accumulate):
+ * Sb[bucket(i, j)] += fp32(+-s * b_i), FP32 products and sums in unspecified order, same map as A.
+ * Where the tensor-memory variant runs, the lanes that hash a row also add its b contributions (no second pass,
+ * no second hash); other variants run a one-column FP32 scatter behind the first.  opts may be NULL. */
+int sketch_apply_f16acc_with_rhs(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, const float* b_dev,
+                                 void* B16_dev, float* Sb32_dev, const sketch_opts_t* opts, void* stream);
+int sketch_apply_f32acc_with_rhs(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, const float* b_dev,
+                                 float* B32_dev, float* Sb32_dev, const sketch_opts_t* opts, void* stream);
+
+/* "widen FP16 SA exactly" ("layout/promotion"): out_dev[k] = fp32(B16_dev[k]) for k < count, exact for
+ * every binary16 (is_bf16 = 0) or bfloat16 (is_bf16 = 1) value.  Device pointers; asynchronous on `stream`. */
+int sketch_widen(const void* B16_dev, int64_t count, int is_bf16, float* out_dev, void* stream);
 
 /* End-to-end entry points with HOST buffers: A_host (m x n, lda) is streamed to the device in row chunks
  * through two library-owned staging buffers (copy of chunk k+1 overlaps the kernels of chunk k), sketched
@@ -151,7 +186,7 @@ int sketch_red_probe(void* sketch_dev, int32_t d, int32_t n, int32_t kind, int32
                      int32_t grid_ctas, int32_t iters, uint64_t* red_ops_out, void* stream);
 
 /* Which variant / replica count / hash mode AUTO resolves to for this shape; host-only, no launch.
- * is_f16: 1 = f16acc, 0 = f32acc.  Any out pointer may be NULL. */
+ * is_f16: 0 = f32acc, 1 = f16acc, 2 = bf16acc.  Any out pointer may be NULL. */
 int sketch_plan(const sketch_t* s, int32_t n, int64_t lda, int is_f16, int rounding, const sketch_opts_t* opts,
                 int32_t* variant_out, int32_t* replicas_out, int32_t* hash_mode_out, int32_t* grid_out);
 

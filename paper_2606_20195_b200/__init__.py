@@ -5,6 +5,7 @@ CUDA kernels of ``csrc/``; this package only marshals arguments (``binding.py``)
 fallback: importing the binding raises if ``libsparse_sketch.so`` cannot be built or loaded.
 """
 from .binding import (  # noqa: F401
+    DITHER,
     RN,
     SR,
     VARIANT_AUTO,
@@ -23,5 +24,6 @@ from .binding import (  # noqa: F401
     sketch_launch_count,
     sketch_red_probe,
     sketch_strerror,
+    sketch_widen,
     sketch_version,
 )

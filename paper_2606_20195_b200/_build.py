@@ -13,11 +13,14 @@ HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 OBJ = HERE / "_obj"
 LIB = HERE / "libsparse_sketch.so"
-SOURCES = [CSRC / n for n in ("sparse_sketch.cu", "launch_flat_f16.cu", "launch_flat_f32.cu", "launch_smem.cu", "launch_tmem.cu")]
+SOURCES = [CSRC / n for n in ("sparse_sketch.cu", "tmem_host.cu", "launch_flat_f16.cu", "launch_flat_bf16.cu", "launch_flat_f32.cu", "launch_smem.cu",
+                              "launch_tmem.cu")]
 HEADERS = [CSRC / n for n in ("args.h", "launch.h", "device_util.cuh", "kernel_flat.cuh", "kernel_misc.cuh", "kernel_smem.cuh", "kernel_small.cuh", "kernel_tmem.cuh")]
-# (source, object stem, extra flags): launch_tmem.cu is compiled once per zeta family
-UNITS = [(src, src.stem, []) for src in SOURCES if src.name != "launch_tmem.cu"]
-UNITS += [(CSRC / "launch_tmem.cu", "launch_tmem_z%d" % z, ["-DSK_TMEM_ZETA=%d" % z]) for z in (1, 2, 4, 8)]
+# (source, object stem, extra flags): launch_tmem.cu is compiled once per (zeta, accumulation mode) family; the largest
+# units (FP16-RN with its deferral kernels) go first so the pool finishes together
+UNITS = [(CSRC / "launch_tmem.cu", "launch_tmem_z%d_m%d" % (z, mo), ["-DSK_TMEM_ZETA=%d" % z, "-DSK_TMEM_MODE=%d" % mo])
+         for mo in (0, 1, 4, 2, 3) for z in (8, 4, 2, 1)]
+UNITS += [(src, src.stem, []) for src in SOURCES if src.name != "launch_tmem.cu"]
 HEADERS.append(HERE.parent / "include" / "sparse_sketch.h")
 
 NVCC_FLAGS = [
@@ -55,7 +58,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     OBJ.mkdir(exist_ok=True)
     if not force and not _stale(LIB, SOURCES + HEADERS):
         return LIB
-    with ThreadPoolExecutor(max_workers=len(UNITS)) as ex:
+    with ThreadPoolExecutor(max_workers=min(len(UNITS), os.cpu_count() or 4)) as ex:
         objs = list(ex.map(lambda u: _compile(u, force), UNITS))
     tmp = LIB.with_suffix(".so.tmp%d" % os.getpid())
     res = subprocess.run([_nvcc(), "-shared", "-o", str(tmp)] + [str(o) for o in objs], capture_output=True, text=True)

@@ -11,7 +11,7 @@ from pathlib import Path
 
 from . import _build
 
-RN, SR = 0, 1
+RN, SR, DITHER = 0, 1, 2
 VARIANT_AUTO, VARIANT_FLAT_PAIR, VARIANT_FLAT_VEC, VARIANT_SMEM, VARIANT_GENERIC, VARIANT_TMEM, VARIANT_SMALL = 0, 1, 2, 3, 4, 5, 6
 VARIANT_NAMES = {0: "auto", 1: "flat_pair", 2: "flat_vec", 3: "smem", 4: "generic", 5: "tmem", 6: "small"}
 
@@ -48,6 +48,11 @@ SYMBOLS = {
     "sketch_precompute_hashes": (_int, [_vp, _vp]),
     "sketch_apply_f32acc": (_int, [_vp, _vp, _i32, _i64, _vp, _vp]),
     "sketch_apply_f16acc": (_int, [_vp, _vp, _i32, _i64, _vp, _int, _u64, _vp]),
+    "sketch_apply_bf16acc": (_int, [_vp, _vp, _i32, _i64, _vp, _vp]),
+    "sketch_apply_bf16acc_ex": (_int, [_vp, _vp, _i32, _i64, _vp, _OP, _vp]),
+    "sketch_apply_f16acc_with_rhs": (_int, [_vp, _vp, _i32, _i64, _vp, _vp, _vp, _OP, _vp]),
+    "sketch_apply_f32acc_with_rhs": (_int, [_vp, _vp, _i32, _i64, _vp, _vp, _vp, _OP, _vp]),
+    "sketch_widen": (_int, [_vp, _i64, _int, _vp, _vp]),
     "sketch_apply_f32acc_ex": (_int, [_vp, _vp, _i32, _i64, _vp, _OP, _vp]),
     "sketch_apply_f16acc_ex": (_int, [_vp, _vp, _i32, _i64, _vp, _int, _u64, _OP, _vp]),
     "sketch_apply_f32acc_host": (_int, [_vp, _vp, _i32, _i64, _vp, _OP]),
@@ -115,6 +120,22 @@ def sketch_red_probe(scratch, d: int, n: int, kind: int, replicas: int, grid_cta
     if rc:
         raise SketchError(rc, "sketch_red_probe")
     return int(ops.value)
+
+
+def sketch_widen(B16, out=None, stream=None):
+    """Exact FP32 copy of a binary16 / bfloat16 sketch (sketch_widen)."""
+    import torch
+
+    if not B16.is_cuda or B16.dtype not in (torch.float16, torch.bfloat16) or not B16.is_contiguous():
+        raise TypeError("B16 must be a contiguous CUDA tensor of dtype float16 or bfloat16")
+    if out is None:
+        out = torch.empty(B16.shape, dtype=torch.float32, device=B16.device)
+    _check_cuda(out, torch.float32, "out")
+    assert out.is_contiguous() and out.numel() == B16.numel()
+    rc = lib().sketch_widen(B16.data_ptr(), B16.numel(), int(B16.dtype == torch.bfloat16), out.data_ptr(), _stream_ptr(stream))
+    if rc:
+        raise SketchError(rc, "sketch_widen")
+    return out
 
 
 class Sketch:
@@ -210,6 +231,56 @@ class Sketch:
             raise SketchError(rc, "sketch_apply_f16acc")
         return out
 
+    def apply_bf16acc(self, A, out=None, stream=None, **opts):
+        import torch
+
+        ap, n, lda = self._A_args(A)
+        if out is None:
+            out = torch.empty((self.d, n), dtype=torch.bfloat16, device=A.device)
+        _check_cuda(out, torch.bfloat16, "out")
+        assert out.is_contiguous() and tuple(out.shape) == (self.d, n)
+        if opts:
+            o = _opts(**self._range_opts(A, opts))
+            rc = lib().sketch_apply_bf16acc_ex(self._h, ap, n, lda, out.data_ptr(), C.byref(o), _stream_ptr(stream))
+        else:
+            if A.shape[0] != self.m:
+                raise ValueError("A has %d rows, sketch was created for m=%d (pass row_begin=/rows= for a slice)" % (A.shape[0], self.m))
+            rc = lib().sketch_apply_bf16acc(self._h, ap, n, lda, out.data_ptr(), _stream_ptr(stream))
+        if rc:
+            raise SketchError(rc, "sketch_apply_bf16acc")
+        return out
+
+    # ---- least-squares front end: [A | b] in one pass, exact widening
+    def _with_rhs(self, name, dtype, A, b, out, Sb, stream, opts):
+        import torch
+
+        ap, n, lda = self._A_args(A)
+        _check_cuda(b, torch.float32, "b")
+        if b.dim() != 1 or not b.is_contiguous() or b.shape[0] != A.shape[0]:
+            raise ValueError("b must be a contiguous vector with one entry per row of A")
+        if out is None:
+            out = torch.empty((self.d, n), dtype=dtype, device=A.device)
+        if Sb is None:
+            Sb = torch.empty((self.d,), dtype=torch.float32, device=A.device)
+        _check_cuda(out, dtype, "out")
+        _check_cuda(Sb, torch.float32, "Sb")
+        assert out.is_contiguous() and tuple(out.shape) == (self.d, n) and Sb.is_contiguous() and tuple(Sb.shape) == (self.d,)
+        o = _opts(**self._range_opts(A, opts))
+        rc = getattr(lib(), name)(self._h, ap, n, lda, b.data_ptr(), out.data_ptr(), Sb.data_ptr(), C.byref(o), _stream_ptr(stream))
+        if rc:
+            raise SketchError(rc, name)
+        return out, Sb
+
+    def apply_f16acc_with_rhs(self, A, b, out=None, Sb=None, stream=None, **opts):
+        import torch
+
+        return self._with_rhs("sketch_apply_f16acc_with_rhs", torch.float16, A, b, out, Sb, stream, opts)
+
+    def apply_f32acc_with_rhs(self, A, b, out=None, Sb=None, stream=None, **opts):
+        import torch
+
+        return self._with_rhs("sketch_apply_f32acc_with_rhs", torch.float32, A, b, out, Sb, stream, opts)
+
     # ---- host-buffer applies (end-to-end: H2D streaming + kernels + D2H inside the call)
     def apply_f16acc_host(self, A_host, out_host=None, rounding: int = RN, sr_seed: int = 0, **opts):
         import torch
@@ -241,7 +312,8 @@ class Sketch:
         return out_host
 
     # ---- planning (host only)
-    def plan(self, n: int, lda: int | None = None, f16: bool = True, rounding: int = RN, **opts):
+    def plan(self, n: int, lda: int | None = None, f16=True, rounding: int = RN, **opts):
+        """f16: False / 0 = f32acc, True / 1 = f16acc, 2 = bf16acc."""
         v, p, h, g = _i32(0), _i32(0), _i32(0), _i32(0)
         o = _opts(**opts)
         rc = lib().sketch_plan(self._h, n, lda or n, int(f16), rounding, C.byref(o), C.byref(v), C.byref(p), C.byref(h), C.byref(g))

@@ -3,8 +3,11 @@
 // result-discarding reductions (a5, a6).
 #pragma once
 
+#include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include <stdint.h>
+
+#include "args.h"
 
 #define SK_DEVINL __device__ __forceinline__
 
@@ -40,6 +43,13 @@ SK_DEVINL uint32_t entry_signmask_f32(uint32_t e) { return e & 0x80000000u; }
 SK_DEVINL uint32_t pack_rn(float x0, float x1) {
   __half2 h = __floats2half2_rn(x0, x1);
   return *reinterpret_cast<uint32_t*>(&h);
+}
+
+// bfloat16 control: cvt.rn.bf16x2.f32, round-to-nearest-even, subnormals kept, overflow -> inf
+SK_DEVINL uint32_t pack_bf16_rn(float x0, float x1) {
+  uint32_t d;
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(x1), "f"(x0));   // first source -> upper half
+  return d;
 }
 
 // SR (R13): magnitude rounded toward zero to l, moved one grid step away
@@ -80,6 +90,37 @@ SK_DEVINL uint32_t pack_sr(float x0, float x1, uint64_t sr_seed, uint64_t ctr) {
   return lo | (hi << 16);
 }
 
+// Dither, Eq. (6) (R20): RN16(q + (u0 - 1/2) c q), every operation one FP32 operation
+// rounded to nearest in the written order (no contraction into an FMA).  u0 - 1/2 = (r24 - 2^23) 2^-24 exactly, and
+// fl(((r24 - 2^23) 2^-24) c) = fl((r24 - 2^23) c) 2^-24: a power-of-two factor commutes with the rounding (no underflow:
+// the product is 0 or at least 2^-34), so the two roundings of t and w collapse into one multiply by c 2^-24.
+SK_DEVINL float dither_f32(float q, uint32_t r24) {
+  const float ti = (float)((int32_t)r24 - (1 << 23));               // exact: |.| <= 2^23
+  const float w = __fmul_rn(ti, 0.00097656f * 5.9604644775390625e-08f);   // c 2^-24: the literal's bits, exponent - 24
+  const float e = __fmul_rn(w, q);
+  return __fadd_rn(q, e);
+}
+// one xorshift64 step (13, 7, 17) on the counter hash (state 0 replaced), R21; bit layout as R14
+SK_DEVINL uint64_t dither_bits(uint64_t sr_seed, uint64_t ctr) {
+  uint64_t x = splitmix64(sr_seed ^ ctr);
+  x = x ? x : 0x9E3779B97F4A7C15ull;
+  x ^= x << 13;
+  x ^= x >> 7;
+  x ^= x << 17;
+  return x;
+}
+SK_DEVINL uint32_t pack_dither(float x0, float x1, uint64_t sr_seed, uint64_t ctr) {
+  const uint64_t R = dither_bits(sr_seed, ctr);
+  return pack_rn(dither_f32(x0, (uint32_t)(R >> 40)), dither_f32(x1, (uint32_t)(R >> 16) & 0xFFFFFFu));
+}
+// conversion of one signed column pair under rule RND (FP16 path)
+template <int RND>
+SK_DEVINL uint32_t pack_f16(float x0, float x1, uint64_t sr_seed, uint64_t ctr) {
+  if constexpr (RND == RND_SR) return pack_sr(x0, x1, sr_seed, ctr);
+  else if constexpr (RND == RND_DITHER) return pack_dither(x0, x1, sr_seed, ctr);
+  else return pack_rn(x0, x1);
+}
+
 // ------------------------------------------------------------------------------------------------
 // Result-discarding reductions to global memory (L2).  PAPER.md:177-183: atom.global.add with the
 // result unused -> SASS REDG (no return path).  sm_90+/sm_100a also take 8- and 16-byte vector forms
@@ -96,6 +137,22 @@ SK_DEVINL void red_h8(void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
   asm volatile("red.global.add.noftz.v4.f16x2 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(a), "r"(b), "r"(c), "r"(d)
                : "memory");
 }
+SK_DEVINL void red_b2(void* p, uint32_t a) {
+  asm volatile("red.global.add.noftz.bf16x2 [%0], %1;" ::"l"(p), "r"(a) : "memory");
+}
+SK_DEVINL void red_b4(void* p, uint32_t a, uint32_t b) {
+  asm volatile("red.global.add.noftz.v2.bf16x2 [%0], {%1,%2};" ::"l"(p), "r"(a), "r"(b) : "memory");
+}
+SK_DEVINL void red_b8(void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("red.global.add.noftz.v4.bf16x2 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(a), "r"(b), "r"(c), "r"(d)
+               : "memory");
+}
+// packed 16-bit REDs by element type
+template <int OUT> SK_DEVINL void red_p2(void* p, uint32_t a) { if constexpr (OUT == OUT_BF16) red_b2(p, a); else red_h2(p, a); }
+template <int OUT> SK_DEVINL void red_p4(void* p, uint32_t a, uint32_t b) { if constexpr (OUT == OUT_BF16) red_b4(p, a, b); else red_h4(p, a, b); }
+template <int OUT> SK_DEVINL void red_p8(void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  if constexpr (OUT == OUT_BF16) red_b8(p, a, b, c, d); else red_h8(p, a, b, c, d);
+}
 SK_DEVINL void red_f1(void* p, float a) {
   asm volatile("red.global.add.f32 [%0], %1;" ::"l"(p), "f"(a) : "memory");
 }
@@ -110,21 +167,25 @@ SK_DEVINL void red_f4(void* p, float a, float b, float c, float d) {
 // scalar FP16 add for odd n: there is no native scalar f16 RED on sm_100a (red.global.add.noftz.f16
 // assembles to a CAS loop), so add {v, +0} or {+0, v} with the packed RED on the enclosing aligned
 // 4-byte word: x + (+0) = x for every x except -0 -> +0, which the path never produces (R10).
-SK_DEVINL void red_h1(__half* p, uint16_t v) {
+template <int OUT = OUT_F16>
+SK_DEVINL void red_h1(void* p, uint16_t v) {
   uintptr_t a = reinterpret_cast<uintptr_t>(p);
   uint32_t word = (a & 2) ? ((uint32_t)v << 16) : (uint32_t)v;
-  red_h2(reinterpret_cast<void*>(a & ~(uintptr_t)3), word);
+  red_p2<OUT>(reinterpret_cast<void*>(a & ~(uintptr_t)3), word);
 }
 
 // The last element of a sketch with an odd number of elements has no partner inside B: its enclosing word would
 // reach two bytes past the buffer.  That one element is added with a 16-bit compare-and-swap loop instead.
-SK_DEVINL void red_h1_cas(__half* p, uint16_t v) {
+template <int OUT = OUT_F16>
+SK_DEVINL void red_h1_cas(void* p, uint16_t v) {
   unsigned short* q = reinterpret_cast<unsigned short*>(p);
   unsigned short old = *reinterpret_cast<volatile unsigned short*>(q), assumed;
   do {
     assumed = old;
-    const __half sum = __hadd(__ushort_as_half(assumed), __ushort_as_half(v));
-    old = atomicCAS(q, assumed, __half_as_ushort(sum));
+    unsigned short sum;
+    if constexpr (OUT == OUT_BF16) sum = __bfloat16_as_ushort(__hadd(__ushort_as_bfloat16(assumed), __ushort_as_bfloat16(v)));
+    else sum = __half_as_ushort(__hadd(__ushort_as_half(assumed), __ushort_as_half(v)));
+    old = atomicCAS(q, assumed, sum);
   } while (old != assumed);
 }
 

@@ -28,26 +28,26 @@ SK_DEVINL uint32_t unpack_entry(PackT p) {
 // Replicas: CTA b adds into partial sketch b % P, which cuts same-address serialisation in L2 and the
 // depth of every running sum by P; k_reduce_replicas folds them.
 // ------------------------------------------------------------------------------------------------
-template <int VEC, bool F16, int ROUNDING>
+template <int VEC, int OUT, int ROUNDING>
 SK_DEVINL void emit_contribution(void* Bbase, int64_t off, const float (&p)[VEC], const uint32_t (&q)[VEC / 2 > 0 ? VEC / 2 : 1],
                                  uint32_t e, uint64_t sr_seed, uint64_t sr_ctr) {
-  if constexpr (F16) {
-    __half* dst = reinterpret_cast<__half*>(Bbase) + off;
+  if constexpr (OUT != OUT_F32) {
+    uint16_t* dst = reinterpret_cast<uint16_t*>(Bbase) + off;
     uint32_t w[VEC / 2];
-    if constexpr (ROUNDING == 0) {
-      uint32_t sm = entry_signmask_h2(e);
+    if constexpr (ROUNDING == RND_RN) {
+      uint32_t sm = entry_signmask_h2(e);   // binary16 and bfloat16 keep the sign in bit 15 of each half
 #pragma unroll
       for (int k = 0; k < VEC / 2; ++k) w[k] = q[k] ^ sm;
     } else {
-      uint32_t sf = entry_signmask_f32(e);
+      uint32_t sf = entry_signmask_f32(e);  // SR / dither convert the SIGNED product, per contribution
 #pragma unroll
       for (int k = 0; k < VEC / 2; ++k)
-        w[k] = pack_sr(__uint_as_float(__float_as_uint(p[2 * k]) ^ sf), __uint_as_float(__float_as_uint(p[2 * k + 1]) ^ sf),
-                       sr_seed, sr_ctr + k);
+        w[k] = pack_f16<ROUNDING>(__uint_as_float(__float_as_uint(p[2 * k]) ^ sf), __uint_as_float(__float_as_uint(p[2 * k + 1]) ^ sf),
+                                  sr_seed, sr_ctr + k);
     }
-    if constexpr (VEC == 8) red_h8(dst, w[0], w[1], w[2], w[3]);
-    else if constexpr (VEC == 4) red_h4(dst, w[0], w[1]);
-    else red_h2(dst, w[0]);
+    if constexpr (VEC == 8) red_p8<OUT>(dst, w[0], w[1], w[2], w[3]);
+    else if constexpr (VEC == 4) red_p4<OUT>(dst, w[0], w[1]);
+    else red_p2<OUT>(dst, w[0]);
   } else {
     float* dst = reinterpret_cast<float*>(Bbase) + off;
     uint32_t sf = entry_signmask_f32(e);
@@ -63,8 +63,9 @@ SK_DEVINL void emit_contribution(void* Bbase, int64_t off, const float (&p)[VEC]
   }
 }
 
-template <int ZETA, int VEC, bool F16, int ROUNDING, typename PackT>
+template <int ZETA, int VEC, int OUT, int ROUNDING, typename PackT>
 __global__ void __launch_bounds__(kFlatThreads) k_flat(ScatterArgs a) {
+  constexpr bool F16 = OUT != OUT_F32;   // a 16-bit sketch (binary16 or bfloat16)
   static_assert(32 % ZETA == 0, "ZETA must divide 32");
   constexpr int HB = 32 / ZETA;            // rows per macro step
   constexpr bool PRE = sizeof(PackT) > 1;  // PackT = uint8_t means "hash on the fly"
@@ -114,9 +115,9 @@ __global__ void __launch_bounds__(kFlatThreads) k_flat(ScatterArgs a) {
 #pragma unroll
         for (int k = 0; k < VEC; ++k) p[k] = 0.f;
       }
-      if constexpr (F16 && ROUNDING == 0) {
+      if constexpr (F16 && ROUNDING == RND_RN) {
 #pragma unroll
-        for (int k = 0; k < VEC / 2; ++k) q[k] = pack_rn(p[2 * k], p[2 * k + 1]);
+        for (int k = 0; k < VEC / 2; ++k) q[k] = OUT == OUT_BF16 ? pack_bf16_rn(p[2 * k], p[2 * k + 1]) : pack_rn(p[2 * k], p[2 * k + 1]);
       }
 #pragma unroll
       for (int j = 0; j < ZETA; ++j) {
@@ -124,7 +125,7 @@ __global__ void __launch_bounds__(kFlatThreads) k_flat(ScatterArgs a) {
         if (valid) {
           int64_t off = (int64_t)entry_bucket(ej) * a.n + (int64_t)ch * VEC;
           uint64_t sr_ctr = ((uint64_t)(a.row_begin + r0 + rr) * ZETA + j) * npairs + (uint64_t)ch * (VEC / 2);
-          emit_contribution<VEC, F16, ROUNDING>(Bbase, off, p, q, ej, a.sr_seed, sr_ctr);
+          emit_contribution<VEC, OUT, ROUNDING>(Bbase, off, p, q, ej, a.sr_seed, sr_ctr);
         }
       }
     }
@@ -134,8 +135,9 @@ __global__ void __launch_bounds__(kFlatThreads) k_flat(ScatterArgs a) {
 // ------------------------------------------------------------------------------------------------
 // Generic fallback: one lane per (row, column) element, runtime zeta, scalar RED; any n, lda, alignment.
 // ------------------------------------------------------------------------------------------------
-template <bool F16, int ROUNDING>
+template <int OUT, int ROUNDING>
 __global__ void __launch_bounds__(kFlatThreads) k_generic(ScatterArgs a) {
+  constexpr bool F16 = OUT != OUT_F32;
   const int64_t total = a.rows * (int64_t)a.n;
   const int64_t stride = (int64_t)gridDim.x * blockDim.x;
   const uint32_t npairs = ((uint32_t)a.n + 1u) >> 1;
@@ -152,15 +154,19 @@ __global__ void __launch_bounds__(kFlatThreads) k_generic(ScatterArgs a) {
       float ps = __uint_as_float(__float_as_uint(p) ^ entry_signmask_f32(e));
       if constexpr (F16) {
         uint16_t v;
-        if constexpr (ROUNDING == 0) {
+        if constexpr (OUT == OUT_BF16) {
+          v = __bfloat16_as_ushort(__float2bfloat16_rn(ps));
+        } else if constexpr (ROUNDING == RND_RN) {
           v = __half_as_ushort(__float2half_rn(ps));
         } else {
-          uint64_t R = splitmix64(a.sr_seed ^ (ctr * npairs + (uint64_t)(c >> 1)));
+          const uint64_t pc = ctr * npairs + (uint64_t)(c >> 1);
+          uint64_t R = ROUNDING == RND_SR ? splitmix64(a.sr_seed ^ pc) : dither_bits(a.sr_seed, pc);
           uint32_t r24 = (c & 1) ? ((uint32_t)(R >> 16) & 0xFFFFFFu) : (uint32_t)(R >> 40);
-          v = (uint16_t)sr16_bits(ps, r24);
+          v = ROUNDING == RND_SR ? (uint16_t)sr16_bits(ps, r24) : __half_as_ushort(__float2half_rn(dither_f32(ps, r24)));
         }
-        if (off == a.odd_tail) red_h1_cas(reinterpret_cast<__half*>(Bbase) + off, v);   // last element of an odd-sized B
-        else red_h1(reinterpret_cast<__half*>(Bbase) + off, v);
+        uint16_t* dst = reinterpret_cast<uint16_t*>(Bbase) + off;
+        if (off == a.odd_tail) red_h1_cas<OUT>(dst, v);   // last element of an odd-sized B
+        else red_h1<OUT>(dst, v);
       } else {
         red_f1(reinterpret_cast<float*>(Bbase) + off, ps);
       }

@@ -35,15 +35,21 @@ __global__ void k_hash_pack32(uint64_t seed, int64_t total, uint32_t zeta, uint3
 // FP16 path stays an FP16 RN add, "All policies subsequently use RN atomic addition");
 // FP32: float adds.  accumulate != 0 adds the fold into the existing out.
 // ------------------------------------------------------------------------------------------------
-template <bool F16>
+template <int OUT>
 __global__ void k_reduce_replicas(const void* __restrict__ rep, int64_t replica_stride, int32_t replicas, void* __restrict__ out,
                                   int64_t count, int accumulate) {
   int64_t stride = (int64_t)gridDim.x * blockDim.x;
   for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < count; k += stride) {
-    if constexpr (F16) {
+    if constexpr (OUT == OUT_F16) {
       const __half* r = reinterpret_cast<const __half*>(rep);
       __half* o = reinterpret_cast<__half*>(out);
       __half acc = accumulate ? o[k] : __ushort_as_half(0);
+      for (int p = 0; p < replicas; ++p) acc = __hadd(acc, r[(int64_t)p * replica_stride + k]);
+      o[k] = acc;
+    } else if constexpr (OUT == OUT_BF16) {
+      const __nv_bfloat16* r = reinterpret_cast<const __nv_bfloat16*>(rep);
+      __nv_bfloat16* o = reinterpret_cast<__nv_bfloat16*>(out);
+      __nv_bfloat16 acc = accumulate ? o[k] : __ushort_as_bfloat16(0);
       for (int p = 0; p < replicas; ++p) acc = __hadd(acc, r[(int64_t)p * replica_stride + k]);
       o[k] = acc;
     } else {
@@ -54,6 +60,14 @@ __global__ void k_reduce_replicas(const void* __restrict__ rep, int64_t replica_
       o[k] = acc;
     }
   }
+}
+
+// exact widening of a 16-bit sketch to FP32 (PAPER.md:356 "widen FP16 SA exactly"; :312 "layout/promotion")
+template <int OUT>
+__global__ void k_widen(const uint16_t* __restrict__ in, int64_t count, float* __restrict__ out) {
+  int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < count; k += stride)
+    out[k] = OUT == OUT_BF16 ? __bfloat162float(__ushort_as_bfloat16(in[k])) : __half2float(__ushort_as_half(in[k]));
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -124,10 +124,18 @@ SK_DEVINL void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;"); 
 // empty volatile asm that "modifies" the register gives the compiler that dependency at no cost.
 SK_DEVINL void tmem_tie(uint32_t& v) { asm volatile("" : "+r"(v)); }
 
-SK_DEVINL uint32_t hfma2_u32(uint32_t q, uint32_t mult, uint32_t acc) {
+// acc + q * (+-1): one correctly rounded add per component, subnormals kept
+template <int MODE> SK_DEVINL uint32_t tm_fma(uint32_t q, uint32_t mult, uint32_t acc) {
   uint32_t d;
-  asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(d) : "r"(q), "r"(mult), "r"(acc));
+  if constexpr (MODE == TM_F32) asm("fma.rn.f32 %0, %1, %2, %3;" : "=r"(d) : "r"(q), "r"(mult), "r"(acc));
+  else if constexpr (MODE == TM_BF16) asm("fma.rn.bf16x2 %0, %1, %2, %3;" : "=r"(d) : "r"(q), "r"(mult), "r"(acc));
+  else asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(d) : "r"(q), "r"(mult), "r"(acc));
   return d;
+}
+// a3, a4 for an RN mode: two adjacent features -> one 16-bit pair
+template <int MODE> SK_DEVINL uint32_t tm_pack(float x0, float x1) {
+  if constexpr (MODE == TM_BF16) return pack_bf16_rn(x0, x1);
+  else return pack_rn(x0, x1);
 }
 
 // ---------------------------------------------------------------------------------------- geometry
@@ -151,8 +159,11 @@ __host__ __device__ constexpr int tmem_rec_bytes(int zb) { return zb == 1 ? 16 :
 //          group touches (adding +0 there changes nothing), and appends the row to a per-stage side list that the
 //          consumers apply one row at a time after the main loop.  The main loop then has pairwise distinct TMEM
 //          addresses within a group by construction: no compares, no selects, 8 read-modify-writes in flight.
-template <int ZETA, int X, int S, int BQ, int NW, int GM, int T>
+template <int ZETA, int X, int S, int BQ, int NW, int GM, int T, int MODE = TM_F16>
 struct TmemGeom {
+  static constexpr int FW = tm_fw(MODE);
+  static_assert(GM == 0 || MODE == TM_F16, "deferral modes exist for the FP16-RN path only");
+  static_assert(!tm_perj(MODE) || BQ == 1, "per-contribution conversion: one bucket group");
   static_assert(NW % 4 == 0 && NW % (S * BQ) == 0, "consumer warps: whole lane quadrants, whole slice x bucket-group sets");
   static_assert(ZETA % BQ == 0, "bucket groups are whole stack blocks");
   static_assert(GM == 0 || BQ > 1, "deferral needs the shared FP16 tile of the bucket-group kernels");
@@ -163,7 +174,7 @@ struct TmemGeom {
   static constexpr bool ABS = S == 1;             // entries hold absolute tensor-memory addresses (see the producer)
   static constexpr int G = GM == 1 ? 4 : GM == 2 ? 8 : (ZB >= 4 || (BQ > 1 && ZB >= 2)) ? 2 : 4;  // rows per group (LDTMs in flight = G * ZB)
   static_assert(TR % G == 0 && 32 % G == 0, "whole groups");
-  static constexpr int N = 64 * X * S;         // features of the CTA's column slice
+  static constexpr int N = 32 * FW * X * S;    // features of the CTA's column slice
   static constexpr int WC = kTmemCols / (NW / 4);  // tensor-memory columns of one warp's private region
   static constexpr int A_BYTES = T * N * 4;
   // chained modes: entries [row][zeta] {col, mul}.  Deferral: records [row][BQ] of RB bytes, then per (chunk phase,
@@ -183,7 +194,7 @@ struct TmemGeom {
   // bucket groups: every row is needed by BQ warps, so the consumer warps first convert the stage ONCE into a
   // shared FP16 tile (a3, a4), meet at a named barrier, and then each scatters its own blocks from that tile.
   // Two tiles (stage parity); the deferral modes append one all-zero row to each.
-  static constexpr bool SHQ = BQ > 1;
+  static constexpr bool SHQ = BQ > 1 && (MODE == TM_F16 || MODE == TM_BF16);   // FP32 words are read from the A tile itself
   // deferral modes: the PRODUCER warps convert the stage, in place (the FP16 tile takes the first half of the FP32
   // tile's bytes), once its TMA copy has landed; the consumers only scatter.  TMA runs NS - 1 stages ahead.
   static constexpr bool PCONV = DEF;
@@ -198,19 +209,21 @@ __host__ __device__ constexpr int tmem_producers(int n, int bq, int gm, int zeta
 }
 // ring of stages | barriers + TMEM base (256 B) | chained bucket-group kernels: two converted (FP16) tiles | deferral:
 // one all-zero FP16 row + 2 KiB of producer scratch (the sketch rows of a 32-row chunk, a 128-byte line per warp and block)
-constexpr size_t tmem_smem_bytes(int zeta, int n, int bq, int gm) {
+constexpr size_t tmem_smem_bytes(int zeta, int n, int bq, int gm, int mode = TM_F16) {
   const size_t t = (size_t)tmem_stage_rows(n, bq, zeta);
   const size_t rb = (size_t)tmem_rec_bytes(zeta / bq);
   const size_t e = gm ? 2 * t * bq * rb + 128 : t * zeta * 8;   // records + side lists (T rows in all) + counts
-  return (size_t)tmem_stages(n) * (t * n * 4 + e) + 256 + (gm ? (size_t)n * 2 + 2048 : bq > 1 ? 2 * t * n * 2 : 0);
+  const bool shq = bq > 1 && (mode == TM_F16 || mode == TM_BF16);
+  return (size_t)tmem_stages(n) * (t * n * 4 + e) + 256 + (gm ? (size_t)n * 2 + 2048 : shq ? 2 * t * n * 2 : 0);
 }
 
 // a5 for R rows x ZB stack blocks of one warp: LDTM, one RN16 add per half (fma.rn.f16x2 by +-1), STTM.
 // CHAIN: two rows of the call that hit the same sketch row are chained in registers (the later row adds onto
 // the earlier row's result and both store the chain's final value; the bucket is warp-uniform, so this is a
 // select, not divergence).  Without CHAIN the caller guarantees distinct sketch rows within a block.
-template <int R, int ZB, int X, bool CHAIN>
-SK_DEVINL void tmem_rmw(uint32_t region, const uint32_t (*q)[X], const uint32_t (*col)[ZB], const uint32_t (*mul)[ZB]) {
+template <int R, int ZB, int X, bool CHAIN, int MODE = TM_F16>
+SK_DEVINL void tmem_rmw(uint32_t region, const uint32_t (*q)[tm_perj(MODE) ? ZB : 1][X], const uint32_t (*col)[ZB], const uint32_t (*mul)[ZB]) {
+  constexpr bool PERJ = tm_perj(MODE);         // q differs per stack block (the sign went in before the conversion)
   uint32_t acc[R][ZB][X];
   tmem_wait_st();                              // the previous stores are in TMEM
 #pragma unroll
@@ -237,7 +250,7 @@ SK_DEVINL void tmem_rmw(uint32_t region, const uint32_t (*q)[X], const uint32_t 
         }
       }
 #pragma unroll
-      for (int k = 0; k < X; ++k) acc[r][j][k] = hfma2_u32(q[r][k], mul[r][j], acc[r][j][k]);
+      for (int k = 0; k < X; ++k) acc[r][j][k] = tm_fma<MODE>(q[r][PERJ ? j : 0][k], PERJ ? tm_one(MODE) : mul[r][j], acc[r][j][k]);
     }
     if constexpr (CHAIN) {
 #pragma unroll
@@ -286,10 +299,11 @@ template <int ZB> SK_DEVINL void sts_rec(uint32_t p, uint32_t head, const uint32
 }
 
 // ---------------------------------------------------------------------------------------- the kernel
-template <int ZETA, int X, int S, int BQ, int NW, int GM>
-__global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)) * 32, 1) k_tmem(TmemArgs g, const __grid_constant__ CUtensorMap tmap) {
-  constexpr int T = tmem_stage_rows(64 * X * S, BQ, ZETA), NS = tmem_stages(64 * X * S);
-  using Geo = TmemGeom<ZETA, X, S, BQ, NW, GM, T>;
+template <int ZETA, int X, int S, int BQ, int NW, int GM, int MODE>
+__global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S, BQ, GM, ZETA)) * 32, 1) k_tmem(TmemArgs g, const __grid_constant__ CUtensorMap tmap) {
+  constexpr int FW = tm_fw(MODE);
+  constexpr int T = tmem_stage_rows(32 * FW * X * S, BQ, ZETA), NS = tmem_stages(32 * FW * X * S);
+  using Geo = TmemGeom<ZETA, X, S, BQ, NW, GM, T, MODE>;
   constexpr int TR = Geo::TR, G = Geo::G, N = Geo::N, ZB = Geo::ZB, RB = Geo::RB, NP = Geo::NP, NPC = Geo::NPC, NPB = Geo::NPB;
   static_assert(NP == tmem_producers(N, BQ, GM, ZETA), "producer warps");
   constexpr int JB = ZETA / NPB;                     // stack blocks one producer warp hashes
@@ -397,7 +411,15 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
         for (int j = 0; j < JB; ++j) {
           const uint32_t e = hash_entry(a.seed, ctr0 + j0 + j, j0 + j, a.db);
           bk[j] = entry_bucket(e);
-          mulw[j] = 0x3C003C00u ^ entry_signmask_h2(e);
+          mulw[j] = tm_one(MODE) ^ (MODE == TM_F32 ? entry_signmask_f32(e) : entry_signmask_h2(e));
+        }
+        // fused right-hand side ("b in FP32 with the same map"): the lane that hashed row r adds +-s b_r to
+        // the FP32 sketch of b, one result-discarding RED per stack block; the first column slice only
+        if (g.rhs != nullptr && blockIdx.y == 0 && live && row0 + r < a.rows) {
+          const float bv = __fmul_rn(a.scale, g.rhs[row0 + r]);
+          float* const sb = g.Sb + (size_t)(blockIdx.x % (uint32_t)g.sb_replicas) * (size_t)g.sb_stride;
+#pragma unroll
+          for (int j = 0; j < JB; ++j) red_f1(sb + bk[j], __uint_as_float(__float_as_uint(bv) ^ ((mulw[j] & (MODE == TM_F32 ? 0x80000000u : 0x8000u)) ? 0x80000000u : 0u)));
         }
         // region of the consumer warp that owns (this row, bucket group b) when there is one feature slice
         auto abase = [&](uint32_t b) -> uint32_t {
@@ -523,7 +545,10 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
     tmem_wait_st();
 
     const float scale = a.scale;
-    const uint32_t a_off = (rowset * TR) * (N * 4) + (slice * 64 * X + lane * 2 * X) * 4;
+    const uint32_t a_off = (rowset * TR) * (N * 4) + (slice * 32 * FW * X + lane * FW * X) * 4;
+    // per-contribution conversion (SR / dither): counter of this lane's first column pair (R14: (row zeta + j) ceil(n/2) + pair)
+    [[maybe_unused]] const uint64_t npairs = ((uint64_t)a.n + 1u) >> 1;
+    [[maybe_unused]] const uint64_t pair0 = ((uint64_t)col0 + slice * 64 * X + lane * 2 * X) >> 1;
     const uint32_t e_off = Geo::DEF ? ((rowset * TR) * BQ + bgrp) * RB : (rowset * TR) * (ZETA * 8) + bgrp * (ZB * 8);
     uint32_t it = 0;
     for (int64_t st = blockIdx.x; st < nstages; st += gridDim.x, ++it) {
@@ -547,7 +572,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
 #pragma unroll
           for (int i = 0; i < CB; ++i)
             reinterpret_cast<uint2*>(qb)[(uint32_t)(i0 + i) * (NW * 32) + tid] =
-                make_uint2(pack_rn(t[i].x * scale, t[i].y * scale), pack_rn(t[i].z * scale, t[i].w * scale));
+                make_uint2(tm_pack<MODE>(t[i].x * scale, t[i].y * scale), tm_pack<MODE>(t[i].z * scale, t[i].w * scale));
         }
         // all consumer warps: tile `it & 1` is complete, and every warp is done scattering tile `(it - 1) & 1`
         asm volatile("bar.sync 1, %0;" ::"n"(NW * 32) : "memory");
@@ -557,7 +582,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
         // software pipeline over the groups of the stage: records two groups ahead, FP16 words one group ahead of the
         // read-modify-write that uses them (their shared-memory latency hides under the tensor-memory round trip)
         constexpr int NG = TR / G;
-        uint32_t qo[2][G], col[3][G][ZB], mul[3][G][ZB], q[2][G][X];
+        uint32_t qo[2][G], col[3][G][ZB], mul[3][G][ZB], q[2][G][1][X];
 #pragma unroll
         for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + r * (BQ * RB), qo[0][r], col[0][r], mul[0][r]);
         if constexpr (NG > 1) {
@@ -565,12 +590,12 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
           for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + (G + r) * (BQ * RB), qo[1][r], col[1][r], mul[1][r]);
         }
 #pragma unroll
-        for (int r = 0; r < G; ++r) lds_q<X>(qlane + qo[0][r], q[0][r]);
+        for (int r = 0; r < G; ++r) lds_q<X>(qlane + qo[0][r], q[0][r][0]);
 #pragma unroll
         for (int gi = 0; gi < NG; ++gi) {
           if (gi + 1 < NG) {
 #pragma unroll
-            for (int r = 0; r < G; ++r) lds_q<X>(qlane + qo[(gi + 1) & 1][r], q[(gi + 1) & 1][r]);
+            for (int r = 0; r < G; ++r) lds_q<X>(qlane + qo[(gi + 1) & 1][r], q[(gi + 1) & 1][r][0]);
           }
           if (gi + 2 < NG) {
 #pragma unroll
@@ -582,26 +607,36 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
       } else {
 #pragma unroll
       for (int g0 = 0; g0 < TR; g0 += G) {
-        uint32_t q[G][X], col[G][ZB], mul[G][ZB];
+        constexpr bool PERJ = tm_perj(MODE);
+        uint32_t q[G][PERJ ? ZB : 1][X], col[G][ZB], mul[G][ZB];
+        [[maybe_unused]] float v[G][FW * X];     // PERJ: the scaled products, converted per stack block below
 #pragma unroll
         for (int r = 0; r < G; ++r) {
           {
             if constexpr (Geo::SHQ) {
-              lds_q<X>(qlane + (rowset * TR + g0 + r) * Geo::Q_ROW, q[r]);
+              lds_q<X>(qlane + (rowset * TR + g0 + r) * Geo::Q_ROW, q[r][0]);
             } else {
-              // a2 (from the staged tile), a3, a4: q = RN16(s * a), two features per word
-              float v[2 * X];
+              // a2 (from the staged tile), a3: p = s * a for this lane's FW * X features
               const unsigned char* pa = sA + (g0 + r) * (N * 4);
-              if constexpr (X == 1) { const float2 t = *reinterpret_cast<const float2*>(pa); v[0] = t.x; v[1] = t.y; }
+              if constexpr (FW * X == 1) { v[r][0] = *reinterpret_cast<const float*>(pa); }
+              else if constexpr (FW * X == 2) { const float2 t = *reinterpret_cast<const float2*>(pa); v[r][0] = t.x; v[r][1] = t.y; }
               else {
 #pragma unroll
-                for (int k = 0; k < X / 2; ++k) {
+                for (int k = 0; k < FW * X / 4; ++k) {
                   const float4 t = *reinterpret_cast<const float4*>(pa + 16 * k);
-                  v[4 * k] = t.x; v[4 * k + 1] = t.y; v[4 * k + 2] = t.z; v[4 * k + 3] = t.w;
+                  v[r][4 * k] = t.x; v[r][4 * k + 1] = t.y; v[r][4 * k + 2] = t.z; v[r][4 * k + 3] = t.w;
                 }
               }
 #pragma unroll
-              for (int k = 0; k < X; ++k) q[r][k] = pack_rn(v[2 * k] * scale, v[2 * k + 1] * scale);
+              for (int k = 0; k < FW * X; ++k) v[r][k] *= scale;
+              // a4 for the convert-once modes: RN16 / RN-bf16 of two features per word, or the FP32 product itself
+              if constexpr (MODE == TM_F32) {
+#pragma unroll
+                for (int k = 0; k < X; ++k) q[r][0][k] = __float_as_uint(v[r][k]);
+              } else if constexpr (!PERJ) {
+#pragma unroll
+                for (int k = 0; k < X; ++k) q[r][0][k] = tm_pack<MODE>(v[r][2 * k], v[r][2 * k + 1]);
+              }
             }
             const unsigned char* pe = sE + (g0 + r) * (ZETA * 8);
             if constexpr (ZB == 1) { const uint2 t = *reinterpret_cast<const uint2*>(pe); col[r][0] = t.x; mul[r][0] = t.y; }
@@ -612,10 +647,23 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
                 col[r][2 * k] = t.x; mul[r][2 * k] = t.y; col[r][2 * k + 1] = t.z; mul[r][2 * k + 1] = t.w;
               }
             }
+            if constexpr (PERJ) {
+              // a4 per contribution: convert the SIGNED product of (row, block j) with that contribution's own random bits
+              const uint64_t grow = (uint64_t)(a.row_begin + st * T + rowset * TR + g0 + r);
+#pragma unroll
+              for (int j = 0; j < ZB; ++j) {
+                const uint32_t sf = (mul[r][j] & 0x8000u) << 16;
+                const uint64_t ctr = (grow * ZETA + (bgrp * ZB + j)) * npairs + pair0;
+#pragma unroll
+                for (int k = 0; k < X; ++k)
+                  q[r][j][k] = pack_f16<MODE == TM_F16_SR ? RND_SR : RND_DITHER>(__uint_as_float(__float_as_uint(v[r][2 * k]) ^ sf),
+                                                                                 __uint_as_float(__float_as_uint(v[r][2 * k + 1]) ^ sf), a.sr_seed, ctr + k);
+              }
+            }
           }
         }
         // a5: read-modify-write of G x ZB sketch rows in tensor memory; same-bucket rows chained in registers
-        tmem_rmw<G, ZB, X, true>(Geo::ABS ? 0u : region, q, col, mul);
+        tmem_rmw<G, ZB, X, true, MODE>(Geo::ABS ? 0u : region, q, col, mul);
       }
       }
       if constexpr (Geo::DEF) {
@@ -626,10 +674,10 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
           const uint32_t cnt = *reinterpret_cast<const uint32_t*>(sL + NPC * BQ * Geo::LCAP * RB + (pl * BQ + bgrp) * 4);
 #pragma unroll 1
           for (uint32_t i = 0; i < cnt; ++i) {
-            uint32_t row, q1[1][X], c1[1][ZB], m1[1][ZB];
+            uint32_t row, q1[1][1][X], c1[1][ZB], m1[1][ZB];
             lds_rec<ZB>(sL + ((pl * BQ + bgrp) * Geo::LCAP + i) * RB, row, c1[0], m1[0]);
             if (row / TR != rowset) continue;
-            lds_q<X>(qlane + row * Geo::Q_ROW, q1[0]);
+            lds_q<X>(qlane + row * Geo::Q_ROW, q1[0][0]);
             tmem_rmw<1, ZB, X, false>(Geo::ABS ? 0u : region, q1, c1, m1);
           }
         }
@@ -640,7 +688,8 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
 
     // ---- flush: private partial sketch -> B with result-discarding vector REDs (a5's last level)
     tmem_wait_st();
-    __half* const Bw = reinterpret_cast<__half*>(a.B) + (size_t)(bgrp * dloc) * a.n + col0 + slice * 64 * X + lane * 2 * X;
+    constexpr int OUT = tm_out(MODE);
+    const size_t b_off = (size_t)(bgrp * dloc) * a.n + col0 + slice * 32 * FW * X + lane * FW * X;   // elements
     for (uint32_t c = 0; c < ncols; c += 8) {
       uint32_t v[8];
       tmem_ld8(region + c, v);
@@ -649,10 +698,18 @@ __global__ void __launch_bounds__((NW + tmem_producers(64 * X * S, BQ, GM, ZETA)
       for (int k = 0; k < 8; ++k) tmem_tie(v[k]);
 #pragma unroll
       for (int b = 0; b < 8 / X; ++b) {
-        __half* dst = Bw + (size_t)(c / X + b) * a.n;
-        if constexpr (X == 1) { if (v[b] != 0u) red_h2(dst, v[b]); }
-        else if constexpr (X == 2) { if ((v[2 * b] | v[2 * b + 1]) != 0u) red_h4(dst, v[2 * b], v[2 * b + 1]); }
-        else { if ((v[4 * b] | v[4 * b + 1] | v[4 * b + 2] | v[4 * b + 3]) != 0u) red_h8(dst, v[4 * b], v[4 * b + 1], v[4 * b + 2], v[4 * b + 3]); }
+        const size_t e_off = b_off + (size_t)(c / X + b) * a.n;
+        if constexpr (MODE == TM_F32) {
+          float* dst = reinterpret_cast<float*>(a.B) + e_off;
+          if constexpr (X == 1) { if (v[b] != 0u) red_f1(dst, __uint_as_float(v[b])); }
+          else if constexpr (X == 2) { if ((v[2 * b] | v[2 * b + 1]) != 0u) red_f2(dst, __uint_as_float(v[2 * b]), __uint_as_float(v[2 * b + 1])); }
+          else { if ((v[4 * b] | v[4 * b + 1] | v[4 * b + 2] | v[4 * b + 3]) != 0u) red_f4(dst, __uint_as_float(v[4 * b]), __uint_as_float(v[4 * b + 1]), __uint_as_float(v[4 * b + 2]), __uint_as_float(v[4 * b + 3])); }
+        } else {
+          uint16_t* dst = reinterpret_cast<uint16_t*>(a.B) + e_off;
+          if constexpr (X == 1) { if (v[b] != 0u) red_p2<OUT>(dst, v[b]); }
+          else if constexpr (X == 2) { if ((v[2 * b] | v[2 * b + 1]) != 0u) red_p4<OUT>(dst, v[2 * b], v[2 * b + 1]); }
+          else { if ((v[4 * b] | v[4 * b + 1] | v[4 * b + 2] | v[4 * b + 3]) != 0u) red_p8<OUT>(dst, v[4 * b], v[4 * b + 1], v[4 * b + 2], v[4 * b + 3]); }
+        }
       }
     }
   }

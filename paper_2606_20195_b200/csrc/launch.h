@@ -34,7 +34,8 @@ inline cudaError_t allow_max_dynamic_smem() {
 cudaError_t launch_flat_f16(const ScatterArgs& a, int zeta, int vec, int rounding, int packed_width, int grid,
                             cudaStream_t st);
 cudaError_t launch_flat_f32(const ScatterArgs& a, int zeta, int vec, int packed_width, int grid, cudaStream_t st);
-cudaError_t launch_generic(const ScatterArgs& a, bool f16, int rounding, int grid, cudaStream_t st);
+cudaError_t launch_flat_bf16(const ScatterArgs& a, int zeta, int vec, int grid, cudaStream_t st);
+cudaError_t launch_generic(const ScatterArgs& a, int out /* OUT_* */, int rounding /* RND_* */, int grid, cudaStream_t st);
 
 // shared-memory-privatised FP16-RN scatter; wpc = warps per CTA = n / 64
 cudaError_t launch_smem_f16(const SmemArgs& g, int zeta, int wpc, int grid, size_t smem_bytes, cudaStream_t st);
@@ -48,21 +49,19 @@ int smem_max_bucket();
 cudaError_t launch_small_f16(const SmallArgs& g, int zeta, int grid, size_t smem_bytes, cudaStream_t st);
 int small_warps();
 
-// tensor-memory-privatised FP16-RN scatter (kernel_tmem.cuh).  Geometry: n = 64 * X * S * CS; lane holds X half2
-// words, S feature slices and BQ bucket groups per CTA, CS column slices across CTAs (gridDim.y), NW consumer warps.
-// tmem_shape picks it, returns false when no geometry fits the 512 TMEM columns of a warp's lane quadrant.
+// tensor-memory-privatised scatter (kernel_tmem.cuh).  mode = TM_* (FP16-RN, bfloat16, FP16 with SR / dither, FP32
+// accumulate).  Geometry: n = 32 FW X S CS with FW = 2 (16-bit modes) or 1 (FP32) features per tensor-memory word; a lane
+// holds X words, S feature slices and BQ bucket groups per CTA, CS column slices across CTAs (gridDim.y), NW consumer
+// warps.  tmem_shape picks it, returns false when no geometry fits the 512 TMEM columns of a warp's lane quadrant.
 struct TmemShape {
   int X, S, BQ, CS, NW, GM;
 };
-bool tmem_shape(int n, int d, int zeta, int64_t lda, int gm_force /* -1 = auto */, TmemShape* out);
+bool tmem_shape(int n, int d, int zeta, int64_t lda, int gm_force /* -1 = auto */, int mode, TmemShape* out);
 bool tmem_tensor_map_ok(int64_t lda, int64_t rows, int n_cta);
 cudaError_t tmem_make_tensor_map(const float* A, int n, int64_t lda, int64_t rows, int n_cta, int box_rows, CUtensorMap* out);
-size_t tmem_smem_bytes_for(int zeta, int n_cta, int bq, int gm);  // n_cta = n / CS
+size_t tmem_smem_bytes_for(int zeta, int n_cta, int bq, int gm, int mode);  // n_cta = n / CS
 int tmem_rows_per_stage(int n_cta, int bq, int zeta);
-cudaError_t launch_tmem_f16(const TmemArgs& g, int zeta, const TmemShape& h, const CUtensorMap* tmap, int grid, cudaStream_t st);
-cudaError_t launch_tmem_z1(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st);
-cudaError_t launch_tmem_z2(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st);
-cudaError_t launch_tmem_z4(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st);
-cudaError_t launch_tmem_z8(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st);
+int tmem_features_per_cta(const TmemShape& h, int mode);
+cudaError_t launch_tmem(const TmemArgs& g, int zeta, int mode, const TmemShape& h, const CUtensorMap* tmap, int grid, cudaStream_t st);
 
 }  // namespace sk

@@ -1,4 +1,5 @@
-// launch_flat_f16.cu -- instantiations of the flat FP16 scatter (RN and SR, on-the-fly and packed hashes).
+// launch_flat_f16.cu -- instantiations of the flat FP16 scatter: RN with on-the-fly or packed hashes, SR and dither
+// (per-contribution conversion; hashes on the fly only).
 #include "kernel_flat.cuh"
 #include "launch.h"
 
@@ -7,9 +8,14 @@ namespace {
 
 template <int ZETA, int VEC, int RND>
 cudaError_t go(const ScatterArgs& a, int pw, int grid, cudaStream_t st) {
-  if (pw == 2) k_flat<ZETA, VEC, true, RND, uint16_t><<<grid, kFlatThreads, 0, st>>>(a);
-  else if (pw == 4) k_flat<ZETA, VEC, true, RND, uint32_t><<<grid, kFlatThreads, 0, st>>>(a);
-  else k_flat<ZETA, VEC, true, RND, uint8_t><<<grid, kFlatThreads, 0, st>>>(a);
+  if constexpr (RND == RND_RN) {
+    if (pw == 2) k_flat<ZETA, VEC, OUT_F16, RND, uint16_t><<<grid, kFlatThreads, 0, st>>>(a);
+    else if (pw == 4) k_flat<ZETA, VEC, OUT_F16, RND, uint32_t><<<grid, kFlatThreads, 0, st>>>(a);
+    else k_flat<ZETA, VEC, OUT_F16, RND, uint8_t><<<grid, kFlatThreads, 0, st>>>(a);
+  } else {
+    if (pw != 0) return kNoKernel;
+    k_flat<ZETA, VEC, OUT_F16, RND, uint8_t><<<grid, kFlatThreads, 0, st>>>(a);
+  }
   return cudaGetLastError();
 }
 
@@ -38,7 +44,12 @@ cudaError_t by_zeta(const ScatterArgs& a, int zeta, int vec, int pw, int grid, c
 
 cudaError_t launch_flat_f16(const ScatterArgs& a, int zeta, int vec, int rounding, int packed_width, int grid,
                             cudaStream_t st) {
-  return rounding ? by_zeta<1>(a, zeta, vec, packed_width, grid, st) : by_zeta<0>(a, zeta, vec, packed_width, grid, st);
+  switch (rounding) {
+    case RND_RN: return by_zeta<RND_RN>(a, zeta, vec, packed_width, grid, st);
+    case RND_SR: return by_zeta<RND_SR>(a, zeta, vec, packed_width, grid, st);
+    case RND_DITHER: return by_zeta<RND_DITHER>(a, zeta, vec, packed_width, grid, st);
+  }
+  return kNoKernel;
 }
 
 }  // namespace sk

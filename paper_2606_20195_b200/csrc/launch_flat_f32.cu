@@ -7,9 +7,9 @@ namespace {
 
 template <int ZETA, int VEC>
 cudaError_t go(const ScatterArgs& a, int pw, int grid, cudaStream_t st) {
-  if (pw == 2) k_flat<ZETA, VEC, false, 0, uint16_t><<<grid, kFlatThreads, 0, st>>>(a);
-  else if (pw == 4) k_flat<ZETA, VEC, false, 0, uint32_t><<<grid, kFlatThreads, 0, st>>>(a);
-  else k_flat<ZETA, VEC, false, 0, uint8_t><<<grid, kFlatThreads, 0, st>>>(a);
+  if (pw == 2) k_flat<ZETA, VEC, OUT_F32, RND_RN, uint16_t><<<grid, kFlatThreads, 0, st>>>(a);
+  else if (pw == 4) k_flat<ZETA, VEC, OUT_F32, RND_RN, uint32_t><<<grid, kFlatThreads, 0, st>>>(a);
+  else k_flat<ZETA, VEC, OUT_F32, RND_RN, uint8_t><<<grid, kFlatThreads, 0, st>>>(a);
   return cudaGetLastError();
 }
 
@@ -35,10 +35,12 @@ cudaError_t launch_flat_f32(const ScatterArgs& a, int zeta, int vec, int packed_
   return kNoKernel;
 }
 
-cudaError_t launch_generic(const ScatterArgs& a, bool f16, int rounding, int grid, cudaStream_t st) {
-  if (!f16) k_generic<false, 0><<<grid, kFlatThreads, 0, st>>>(a);
-  else if (rounding) k_generic<true, 1><<<grid, kFlatThreads, 0, st>>>(a);
-  else k_generic<true, 0><<<grid, kFlatThreads, 0, st>>>(a);
+cudaError_t launch_generic(const ScatterArgs& a, int out, int rounding, int grid, cudaStream_t st) {
+  if (out == OUT_F32) k_generic<OUT_F32, RND_RN><<<grid, kFlatThreads, 0, st>>>(a);
+  else if (out == OUT_BF16) k_generic<OUT_BF16, RND_RN><<<grid, kFlatThreads, 0, st>>>(a);
+  else if (rounding == RND_SR) k_generic<OUT_F16, RND_SR><<<grid, kFlatThreads, 0, st>>>(a);
+  else if (rounding == RND_DITHER) k_generic<OUT_F16, RND_DITHER><<<grid, kFlatThreads, 0, st>>>(a);
+  else k_generic<OUT_F16, RND_RN><<<grid, kFlatThreads, 0, st>>>(a);
   return cudaGetLastError();
 }
 

@@ -50,6 +50,7 @@ struct sketch {
   int smem_per_sm;
   // library-owned scratch
   void* rep;  size_t rep_bytes;        // replicated partial sketches
+  void* sbrep; size_t sbrep_bytes;     // replicated FP32 sketches of a fused right-hand side
   void* packed; size_t packed_bytes; int packed_width;  // 0 = none, 2 = 16-bit entries in sub-step order, 4 = plain 32-bit
   void* stage[2]; size_t stage_bytes;  // host-path staging
   void* bdev; size_t bdev_bytes;
@@ -80,7 +81,14 @@ struct Plan {
   int64_t rows_per_cta;
   int64_t rows_main;  // smem variant: rows handled by k_smem (multiple of its ring rows); the rest go to k_flat
   sk::TmemShape tm;   // tmem variant: geometry
+  int tm_mode;        // tmem variant: TM_* accumulation mode
 };
+
+// tensor-memory accumulation mode of (sketch element type, conversion rule)
+inline int tmem_mode_of(int out, int rounding) {
+  return out == sk::OUT_F32 ? sk::TM_F32 : out == sk::OUT_BF16 ? sk::TM_BF16
+       : rounding == SKETCH_SR ? sk::TM_F16_SR : rounding == SKETCH_DITHER ? sk::TM_F16_DITHER : sk::TM_F16;
+}
 
 int ensure_device(sketch* s) {
   if (s->dev_ready) return SKETCH_OK;
@@ -125,15 +133,16 @@ bool smem_feasible(const sketch* s, int n, int64_t lda, const void* A, const voi
   return true;
 }
 
-bool tmem_feasible(const sketch* s, int n, int64_t lda, int64_t rows, const void* A, const void* B, int gm_force, sk::TmemShape* h) {
+bool tmem_feasible(const sketch* s, int n, int64_t lda, int64_t rows, const void* A, const void* B, int gm_force, int mode,
+                   sk::TmemShape* h) {
   if (!zeta_templated(s->zeta)) return false;
-  if (!sk::tmem_shape(n, s->d, s->zeta, lda, gm_force, h)) return false;
+  if (!sk::tmem_shape(n, s->d, s->zeta, lda, gm_force, mode, h)) return false;
   if (lda % 4 != 0 || !aligned(A, 16) || !aligned(B, 16)) return false;  // TMA bulk copies: 16-byte granules
   if (lda != n / h->CS && !sk::tmem_tensor_map_ok(lda, rows, n / h->CS)) return false;   // the 2-D tensor-map path
-  return sk::tmem_smem_bytes_for(s->zeta, n / h->CS, h->BQ, h->GM) <= (size_t)s->smem_optin;
+  return sk::tmem_smem_bytes_for(s->zeta, n / h->CS, h->BQ, h->GM, mode) <= (size_t)s->smem_optin;
 }
 
-int flat_vec_for(bool f16, int n, int64_t lda, const void* A, const void* B, int want_max) {
+int flat_vec_for(bool f16 /* a 16-bit sketch */, int n, int64_t lda, const void* A, const void* B, int want_max) {
   const int cands_h[3] = {8, 4, 2};
   const int cands_f[4] = {4, 2, 1, 0};  // FP32: one 16-byte RED per lane is the widest single transaction
   const int* c = f16 ? cands_h : cands_f;
@@ -147,8 +156,10 @@ int flat_vec_for(bool f16, int n, int64_t lda, const void* A, const void* B, int
   return 0;
 }
 
-int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool f16, int rounding,
+int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, int out, int rounding,
               const sketch_opts_t* o, int64_t rows, Plan* p) {
+  const bool f16 = out != sk::OUT_F32;                              // a 16-bit sketch
+  const bool h16rn = out == sk::OUT_F16 && rounding == SKETCH_RN;   // the FP16-RN hot path
   int rc = ensure_device(s);
   if (rc) return rc;
   memset(p, 0, sizeof(*p));
@@ -156,18 +167,20 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
   if (want < 0 || want > SKETCH_VARIANT_SMALL) return SKETCH_ERR_INVALID;
   p->hash_mode = (o && o->hash_mode) ? o->hash_mode : 1;
   if (p->hash_mode != 1 && p->hash_mode != 2) return SKETCH_ERR_INVALID;
+  if (f16 && !h16rn) p->hash_mode = 1;   // bfloat16 / SR / dither kernels hash on the fly
   size_t sm_bytes = 0;
   // the privatised kernel is FP16-RN with precomputed hashes; its R-row steps must be aligned in the global
   // row index.  Everything else (FP32, SR, odd shapes) runs the flat / generic kernels.
   const int64_t rb0 = o ? o->row_begin : 0;
-  bool sm_ok = f16 && rounding == SKETCH_RN && smem_feasible(s, n, lda, A, B, &sm_bytes) &&
+  bool sm_ok = h16rn && smem_feasible(s, n, lda, A, B, &sm_bytes) &&
                (rb0 % sk::smem_step_rows(s->zeta) == 0);
   sk::TmemShape tm = {0, 0, 0, 0, 0, 0};
   const int gm_force = (o ? o->tmem_group_mode : 0) - 1;
-  bool tm_ok = f16 && rounding == SKETCH_RN && tmem_feasible(s, n, lda, rows, A, B, gm_force, &tm);
+  const int tm_mode = tmem_mode_of(out, rounding);
+  bool tm_ok = tmem_feasible(s, n, lda, rows, A, B, gm_force, tm_mode, &tm);
   // per-warp shared-memory partials (kernel_small.cuh)
   const size_t small_bytes = (size_t)sk::small_warps() * s->d * n * 2;
-  bool small_ok = f16 && rounding == SKETCH_RN && zeta_templated(s->zeta) && n % 2 == 0 && lda % 2 == 0 && aligned(A, 8) &&
+  bool small_ok = h16rn && zeta_templated(s->zeta) && n % 2 == 0 && lda % 2 == 0 && aligned(A, 8) &&
                   small_bytes <= (size_t)s->smem_optin;
   int vmax = flat_vec_for(f16, n, lda, A, B, 8);
   int vpair = flat_vec_for(f16, n, lda, A, B, f16 ? 2 : 1);
@@ -184,7 +197,9 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
     // (64-feature column slices cut into bucket groups of several blocks -- d = 640 at n = 320 -- measured 2.69 TB/s
     // against 2.80 TB/s of the flat REDs; with one block per warp they get 128-row stages and win: d = 2048 at n = 256
     // 2.99 vs 2.74 TB/s; without bucket groups -- d = 384 at n = 192 -- the same slices run at 4.65 TB/s)
-    if (tm_ok && !(tm.X * tm.S == 1 && tm.BQ > 1 && tm.BQ != s->zeta) && rows * (int64_t)n > (1 << 20)) v = SKETCH_VARIANT_TMEM;
+    // (the FP32 path privatised in tensor memory beats its flat REDs wherever it fits: 1.4 TB/s is the L2-atomic ceiling
+    // of an FP32 zeta = 4 scatter)
+    if (tm_ok && (!f16 || !(tm.X * tm.S == 1 && tm.BQ > 1 && tm.BQ != s->zeta)) && rows * (int64_t)n > (1 << 20)) v = SKETCH_VARIANT_TMEM;
     else if (sm_ok && s->zeta >= 2) v = SKETCH_VARIANT_SMEM;
     // launch-bound inputs into a sketch of a few KiB: the flat REDs queue ~1000 deep on each L2 sector (c1: 10 us);
     // per-warp shared-memory partials need no such queue
@@ -204,8 +219,9 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, bool 
     p->hash_mode = 1;  // the producer warp hashes on the fly
     p->replicas = 1;
     p->tm = tm;
+    p->tm_mode = tm_mode;
     p->wpc = tm.NW + 1;
-    p->smem_bytes = sk::tmem_smem_bytes_for(s->zeta, n / tm.CS, tm.BQ, tm.GM);
+    p->smem_bytes = sk::tmem_smem_bytes_for(s->zeta, n / tm.CS, tm.BQ, tm.GM, tm_mode);
     const int T = sk::tmem_rows_per_stage(n / tm.CS, tm.BQ, s->zeta);
     int64_t stages = (rows + T - 1) / T;
     // one CTA per SM (it owns all 512 TMEM columns); gridDim.y = CS column slices share a row range
@@ -362,6 +378,16 @@ int scratch_release(sketch* s, cudaStream_t st, bool capturing) {
   return SKETCH_OK;
 }
 
+constexpr int kSbReplicas = 64;   // partial FP32 sketches of a fused right-hand side
+
+// fold P partial sketches (k_reduce_replicas) in the sketch's own element type
+int fold_replicas(int out, const void* rep, int64_t stride, int P, void* B, int64_t count, int accumulate, int grid, cudaStream_t st) {
+  if (out == sk::OUT_F16) sk::k_reduce_replicas<sk::OUT_F16><<<grid, 256, 0, st>>>(rep, stride, P, B, count, accumulate);
+  else if (out == sk::OUT_BF16) sk::k_reduce_replicas<sk::OUT_BF16><<<grid, 256, 0, st>>>(rep, stride, P, B, count, accumulate);
+  else sk::k_reduce_replicas<sk::OUT_F32><<<grid, 256, 0, st>>>(rep, stride, P, B, count, accumulate);
+  return launch_check("k_reduce_replicas");
+}
+
 // tensor map of a strided / column-sliced tensor-memory launch, from the handle's cache
 int tensor_map_for(sketch* s, const float* A, int n, int64_t lda, int64_t rows, int n_cta, int box_rows, const CUtensorMap** out) {
   for (int k = 0; k < s->tmap_count; ++k) {
@@ -425,35 +451,82 @@ int validate_apply(const sketch* s, const void* A, int32_t n, int64_t lda, const
   return SKETCH_OK;
 }
 
-int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void* B, bool f16, int rounding,
-                 uint64_t sr_seed, const sketch_opts_t* o, void* stream) {
+// The fused right-hand side (rhs, Sb): b[rows] FP32 is sketched with the same map into Sb[d] FP32.  The
+// tensor-memory kernel does it in the same pass (its producer lanes hold every row's hashes); the other variants run a
+// second, one-column FP32 scatter behind the first.
+int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void* B, int out, int rounding,
+                 uint64_t sr_seed, const sketch_opts_t* o, void* stream, const float* rhs = nullptr, float* Sb = nullptr) {
   sketch* s = const_cast<sketch*>(cs);
+  const bool f16 = out != sk::OUT_F32;   // a 16-bit sketch
   int64_t row_begin = 0, rows = 0;
   int rc = validate_apply(s, A, n, lda, B, f16, o, &row_begin, &rows);
   if (rc) return rc;
-  if (f16 && rounding != SKETCH_RN && rounding != SKETCH_SR) return SKETCH_ERR_INVALID;
+  if ((rhs == nullptr) != (Sb == nullptr)) return SKETCH_ERR_NULL;
+  if (rhs && (!aligned(rhs, 4) || !aligned(Sb, 4))) return SKETCH_ERR_ALIGNMENT;
+  if (out == sk::OUT_F16 ? (rounding != SKETCH_RN && rounding != SKETCH_SR && rounding != SKETCH_DITHER) : rounding != SKETCH_RN)
+    return SKETCH_ERR_INVALID;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   Plan p;
-  rc = make_plan(s, n, lda, A, B, f16, rounding, o, rows, &p);
+  rc = make_plan(s, n, lda, A, B, out, rounding, o, rows, &p);
   if (rc) return rc;
   const int accumulate = o ? o->accumulate : 0;
   const size_t elem = f16 ? 2 : 4;
   const size_t out_bytes = (size_t)s->d * n * elem;
 
+  if (rhs && p.variant != SKETCH_VARIANT_TMEM) {
+    sketch_opts_t ob;
+    memset(&ob, 0, sizeof(ob));
+    ob.accumulate = accumulate;
+    ob.row_begin = row_begin;
+    ob.rows = rows;
+    if (rows == 0) {   // the ABI reads rows = 0 as "through row m - 1": an empty range only zero-fills
+      if (!accumulate) CU_TRY(cudaMemsetAsync(Sb, 0, (size_t)s->d * 4, st));
+    } else {
+      rc = apply_device(cs, rhs, 1, 1, Sb, sk::OUT_F32, SKETCH_RN, 0, &ob, stream);
+      if (rc) return rc;
+    }
+  }
+
   if (p.variant == SKETCH_VARIANT_TMEM) {
     if (!accumulate) CU_TRY(cudaMemsetAsync(B, 0, out_bytes, st));  // a0
+    if (rhs && rows == 0 && !accumulate) CU_TRY(cudaMemsetAsync(Sb, 0, (size_t)s->d * 4, st));
     if (rows > 0) {
       sk::TmemArgs g;
       g.s = make_args(s, A, n, lda, B, row_begin, rows, sr_seed, 1);
       g.d = s->d;
+      g.rhs = rhs;
+      g.Sb = nullptr;
+      g.sb_stride = 0;
+      g.sb_replicas = 1;
+      bool capturing = false;
+      if (rhs) {
+        // FP32 REDs of the m zeta contributions of b into kSbReplicas partial sketches (same-address traffic in L2 spread
+        // over as many lines; every running sum that much shorter), folded into Sb behind the kernel
+        rc = scratch_acquire(s, st, &capturing);
+        if (rc) return rc;
+        g.sb_stride = padded_count(s->d);
+        g.sb_replicas = kSbReplicas;
+        rc = ensure_scratch(&s->sbrep, &s->sbrep_bytes, (size_t)g.sb_stride * 4 * kSbReplicas);
+        if (rc) return rc;
+        g.Sb = static_cast<float*>(s->sbrep);
+        CU_TRY(cudaMemsetAsync(s->sbrep, 0, (size_t)g.sb_stride * 4 * kSbReplicas, st));
+      }
       const CUtensorMap* tmap = nullptr;
       const int n_cta = n / p.tm.CS;
       if (lda != n_cta) {
         rc = tensor_map_for(s, A, n, lda, rows, n_cta, sk::tmem_rows_per_stage(n_cta, p.tm.BQ, s->zeta), &tmap);
         if (rc) return rc;
       }
-      rc = launched(sk::launch_tmem_f16(g, s->zeta, p.tm, tmap, p.grid, st), "k_tmem");
+      rc = launched(sk::launch_tmem(g, s->zeta, p.tm_mode, p.tm, tmap, p.grid, st), "k_tmem");
       if (rc) return rc;
+      if (rhs) {
+        int grid = (s->d + 255) / 256;
+        sk::k_reduce_replicas<sk::OUT_F32><<<grid, 256, 0, st>>>(s->sbrep, g.sb_stride, kSbReplicas, Sb, s->d, accumulate);
+        rc = launch_check("k_reduce_replicas (rhs)");
+        if (rc) return rc;
+        rc = scratch_release(s, st, capturing);
+        if (rc) return rc;
+      }
     }
     return SKETCH_OK;
   }
@@ -525,20 +598,20 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
     a.packed = pw ? s->packed : nullptr;
     if (p.variant == SKETCH_VARIANT_GENERIC) {
       if (f16 && P == 1 && (count & 1)) a.odd_tail = count - 1;
-      rc = launched(sk::launch_generic(a, f16, rounding == SKETCH_SR, p.grid, st), "k_generic");
-    } else if (!f16) {
+      rc = launched(sk::launch_generic(a, out, rounding, p.grid, st), "k_generic");
+    } else if (out == sk::OUT_F32) {
       rc = launched(sk::launch_flat_f32(a, s->zeta, p.vec, pw, p.grid, st), "k_flat<f32>");
+    } else if (out == sk::OUT_BF16) {
+      rc = launched(sk::launch_flat_bf16(a, s->zeta, p.vec, p.grid, st), "k_flat<bf16>");
     } else {
-      rc = launched(sk::launch_flat_f16(a, s->zeta, p.vec, rounding == SKETCH_SR, pw, p.grid, st), "k_flat<f16>");
+      rc = launched(sk::launch_flat_f16(a, s->zeta, p.vec, rounding, pw, p.grid, st), "k_flat<f16>");
     }
     if (rc) return rc;
   }
   if (P > 1) {
     int grid = (int)((count + 255) / 256);
     if (grid > s->sm_count * 8) grid = s->sm_count * 8;
-    if (f16) sk::k_reduce_replicas<true><<<grid, 256, 0, st>>>(target, pstride, P, B, count, accumulate);
-    else sk::k_reduce_replicas<false><<<grid, 256, 0, st>>>(target, pstride, P, B, count, accumulate);
-    rc = launch_check("k_reduce_replicas");
+    rc = fold_replicas(out, target, pstride, P, B, count, accumulate, grid, st);
     if (rc) return rc;
   }
   if (uses_scratch) {
@@ -560,10 +633,10 @@ int ensure_host_path(sketch* s) {
   return SKETCH_OK;
 }
 
-int apply_host_impl(sketch* s, const float* A, int32_t n, int64_t lda, void* B, bool f16, int rounding, uint64_t sr_seed,
+int apply_host_impl(sketch* s, const float* A, int32_t n, int64_t lda, void* B, int out, int rounding, uint64_t sr_seed,
                     const sketch_opts_t* o, int64_t rb, int64_t rows) {
   int rc;
-  const size_t elem = f16 ? 2 : 4;
+  const size_t elem = out != sk::OUT_F32 ? 2 : 4;
   const size_t out_bytes = (size_t)s->d * n * elem;
   const size_t slot_bytes = (size_t)padded_count((int64_t)s->d * n) * elem;   // 16-byte aligned slots (d * n may be odd)
   // staging: two buffers of ~256 MiB, whole rows, row count a multiple of 32
@@ -609,7 +682,7 @@ int apply_host_impl(sketch* s, const float* A, int32_t n, int64_t lda, void* B, 
     oo.row_begin = rb + r0;
     oo.rows = nr;
     oo.accumulate = k >= kSlots ? 1 : 0;
-    rc = apply_device(s, (const float*)s->stage[b], n, n, slots + slot_bytes * (size_t)(k % kSlots), f16, rounding, sr_seed, &oo,
+    rc = apply_device(s, (const float*)s->stage[b], n, n, slots + slot_bytes * (size_t)(k % kSlots), out, rounding, sr_seed, &oo,
                       s->st_comp);
     if (rc) return rc;
     CU_TRY(cudaEventRecord(s->ev_done[b], s->st_comp));
@@ -618,9 +691,7 @@ int apply_host_impl(sketch* s, const float* A, int32_t n, int64_t lda, void* B, 
     const int64_t count = (int64_t)s->d * n;
     int grid = (int)((count + 255) / 256);
     if (grid > s->sm_count * 8) grid = s->sm_count * 8;
-    if (f16) sk::k_reduce_replicas<true><<<grid, 256, 0, s->st_comp>>>(slots, padded_count(count), (int)kSlots, result, count, user_acc);
-    else sk::k_reduce_replicas<false><<<grid, 256, 0, s->st_comp>>>(slots, padded_count(count), (int)kSlots, result, count, user_acc);
-    rc = launch_check("k_reduce_replicas (chunks)");
+    rc = fold_replicas(out, slots, padded_count(count), (int)kSlots, result, count, user_acc, grid, s->st_comp);
     if (rc) return rc;
   }
   CU_TRY(cudaMemcpyAsync(B, result, out_bytes, cudaMemcpyDeviceToHost, s->st_comp));
@@ -628,7 +699,7 @@ int apply_host_impl(sketch* s, const float* A, int32_t n, int64_t lda, void* B, 
   return SKETCH_OK;
 }
 
-int apply_host(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void* B, bool f16, int rounding,
+int apply_host(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void* B, int out, int rounding,
                uint64_t sr_seed, const sketch_opts_t* o) {
   sketch* s = const_cast<sketch*>(cs);
   if (!s || !A || !B) return SKETCH_ERR_NULL;
@@ -642,7 +713,7 @@ int apply_host(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void*
   if (rc) return rc;
   rc = ensure_host_path(s);
   if (rc) return rc;
-  rc = apply_host_impl(s, A, n, lda, B, f16, rounding, sr_seed, o, rb, rows);
+  rc = apply_host_impl(s, A, n, lda, B, out, rounding, sr_seed, o, rb, rows);
   if (rc) {
     // no copy from the caller's A (or into its B) may still be in flight when the call returns
     cudaStreamSynchronize(s->st_copy);
@@ -678,6 +749,7 @@ int sketch_create(int64_t m, int32_t d, int32_t zeta, uint64_t seed, sketch_t** 
 int sketch_destroy(sketch_t* s) {
   if (!s) return SKETCH_OK;
   if (s->rep) cudaFree(s->rep);
+  if (s->sbrep) cudaFree(s->sbrep);
   if (s->packed) cudaFree(s->packed);
   for (int k = 0; k < 2; ++k)
     if (s->stage[k]) cudaFree(s->stage[k]);
@@ -721,33 +793,67 @@ int sketch_precompute_hashes(sketch_t* s, void* stream) {
 }
 
 int sketch_apply_f32acc(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, float* B_dev, void* stream) {
-  return apply_device(s, A_dev, n, lda, B_dev, false, 0, 0, nullptr, stream);
+  return apply_device(s, A_dev, n, lda, B_dev, sk::OUT_F32, SKETCH_RN, 0, nullptr, stream);
 }
 
 int sketch_apply_f16acc(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev, int rounding,
                         uint64_t sr_seed, void* stream) {
-  return apply_device(s, A_dev, n, lda, B_dev, true, rounding, sr_seed, nullptr, stream);
+  return apply_device(s, A_dev, n, lda, B_dev, sk::OUT_F16, rounding, sr_seed, nullptr, stream);
+}
+
+int sketch_apply_bf16acc(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev, void* stream) {
+  return apply_device(s, A_dev, n, lda, B_dev, sk::OUT_BF16, SKETCH_RN, 0, nullptr, stream);
 }
 
 int sketch_apply_f32acc_ex(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, float* B_dev,
                            const sketch_opts_t* opts, void* stream) {
-  return apply_device(s, A_dev, n, lda, B_dev, false, 0, 0, opts, stream);
+  return apply_device(s, A_dev, n, lda, B_dev, sk::OUT_F32, SKETCH_RN, 0, opts, stream);
 }
 
 int sketch_apply_f16acc_ex(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev, int rounding,
                            uint64_t sr_seed, const sketch_opts_t* opts, void* stream) {
-  return apply_device(s, A_dev, n, lda, B_dev, true, rounding, sr_seed, opts, stream);
+  return apply_device(s, A_dev, n, lda, B_dev, sk::OUT_F16, rounding, sr_seed, opts, stream);
+}
+
+int sketch_apply_bf16acc_ex(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev,
+                            const sketch_opts_t* opts, void* stream) {
+  return apply_device(s, A_dev, n, lda, B_dev, sk::OUT_BF16, SKETCH_RN, 0, opts, stream);
+}
+
+int sketch_apply_f16acc_with_rhs(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, const float* b_dev,
+                                 void* B16_dev, float* Sb32_dev, const sketch_opts_t* opts, void* stream) {
+  if (!b_dev || !Sb32_dev) return SKETCH_ERR_NULL;
+  return apply_device(s, A_dev, n, lda, B16_dev, sk::OUT_F16, SKETCH_RN, 0, opts, stream, b_dev, Sb32_dev);
+}
+
+int sketch_apply_f32acc_with_rhs(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, const float* b_dev,
+                                 float* B32_dev, float* Sb32_dev, const sketch_opts_t* opts, void* stream) {
+  if (!b_dev || !Sb32_dev) return SKETCH_ERR_NULL;
+  return apply_device(s, A_dev, n, lda, B32_dev, sk::OUT_F32, SKETCH_RN, 0, opts, stream, b_dev, Sb32_dev);
+}
+
+int sketch_widen(const void* B16_dev, int64_t count, int is_bf16, float* out_dev, void* stream) {
+  if (!B16_dev || !out_dev) return SKETCH_ERR_NULL;
+  if (count < 0) return SKETCH_ERR_INVALID;
+  if (!aligned(B16_dev, 2) || !aligned(out_dev, 4)) return SKETCH_ERR_ALIGNMENT;
+  if (count == 0) return SKETCH_OK;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  int64_t blocks = (count + 255) / 256;
+  int grid = (int)(blocks < 148 * 16 ? blocks : 148 * 16);
+  if (is_bf16) sk::k_widen<sk::OUT_BF16><<<grid, 256, 0, st>>>(static_cast<const uint16_t*>(B16_dev), count, out_dev);
+  else sk::k_widen<sk::OUT_F16><<<grid, 256, 0, st>>>(static_cast<const uint16_t*>(B16_dev), count, out_dev);
+  return launch_check("k_widen");
 }
 
 int sketch_apply_f32acc_host(const sketch_t* s, const float* A_host, int32_t n, int64_t lda, float* B_host,
                              const sketch_opts_t* opts) {
-  return apply_host(s, A_host, n, lda, B_host, false, 0, 0, opts);
+  return apply_host(s, A_host, n, lda, B_host, sk::OUT_F32, SKETCH_RN, 0, opts);
 }
 
 int sketch_apply_f16acc_host(const sketch_t* s, const float* A_host, int32_t n, int64_t lda, void* B_host, int rounding,
                              uint64_t sr_seed, const sketch_opts_t* opts) {
-  if (rounding != SKETCH_RN && rounding != SKETCH_SR) return SKETCH_ERR_INVALID;
-  return apply_host(s, A_host, n, lda, B_host, true, rounding, sr_seed, opts);
+  if (rounding != SKETCH_RN && rounding != SKETCH_SR && rounding != SKETCH_DITHER) return SKETCH_ERR_INVALID;
+  return apply_host(s, A_host, n, lda, B_host, sk::OUT_F16, rounding, sr_seed, opts);
 }
 
 int sketch_red_probe(void* sketch_dev, int32_t d, int32_t n, int32_t kind, int32_t replicas, int32_t grid_ctas,
@@ -779,8 +885,9 @@ int sketch_plan(const sketch_t* cs, int32_t n, int64_t lda, int is_f16, int roun
   if (rows == 0) rows = s->m - rb;
   Plan p;
   // plan for 256-byte aligned buffers (what cudaMalloc returns)
-  int rc = make_plan(s, n, lda, reinterpret_cast<const void*>(256), reinterpret_cast<const void*>(256), is_f16 != 0,
-                     rounding, opts, rows, &p);
+  if (is_f16 < 0 || is_f16 > 2) return SKETCH_ERR_INVALID;
+  int rc = make_plan(s, n, lda, reinterpret_cast<const void*>(256), reinterpret_cast<const void*>(256),
+                     is_f16 == 2 ? sk::OUT_BF16 : is_f16 == 1 ? sk::OUT_F16 : sk::OUT_F32, rounding, opts, rows, &p);
   if (rc) return rc;
   if (variant_out) *variant_out = p.variant;
   if (replicas_out) *replicas_out = p.replicas;

@@ -42,11 +42,12 @@ F32_VARIANTS = ["auto", "flat_pair", "flat_vec", "generic"]
 VID = {"auto": 0, "flat_pair": 1, "flat_vec": 2, "smem": 3, "generic": 4, "tmem": 5, "small": 6}
 
 
-def feasible(ss, sk, A, variant, f16=True, rounding=0, **kw):
+def feasible(ss, sk, A, variant, f16=True, **kw):
     """The host-side plan decides whether a forced variant can run this shape (SKETCH_ERR_UNSUPPORTED = -6 comes from
     make_plan only); any other error is a failure."""
     plan_kw = {k: v for k, v in kw.items() if k in ("row_begin", "rows", "replicas", "hash_mode", "grid_ctas", "tmem_group_mode")}
     plan_kw.setdefault("rows", int(A.shape[0]))
+    rounding = kw.get("rounding", 0)
     try:
         sk.plan(int(A.shape[1]), lda=int(A.stride(0)) if A.shape[0] > 1 else int(A.shape[1]), f16=f16, rounding=rounding,
                 variant=VID[variant], **plan_kw)
@@ -59,7 +60,7 @@ def feasible(ss, sk, A, variant, f16=True, rounding=0, **kw):
 def apply16(ss, sk, A, variant="auto", **kw):
     """Forced variant: must run iff the plan says it can; an infeasible (variant, shape) must fail with -6 and is skipped
     with its reason.  A -6 / -7 on a feasible plan is a test failure."""
-    if not feasible(ss, sk, A, variant, True, kw.get("rounding", 0), **kw):
+    if not feasible(ss, sk, A, variant, True, **kw):
         with pytest.raises(ss.SketchError) as ei:
             sk.apply_f16acc(A, variant=VID[variant], **kw)
         assert ei.value.code == -6
@@ -68,7 +69,7 @@ def apply16(ss, sk, A, variant="auto", **kw):
 
 
 def apply32(ss, sk, A, variant="auto", **kw):
-    if not feasible(ss, sk, A, variant, False, 0, **kw):
+    if not feasible(ss, sk, A, variant, False, **kw):
         with pytest.raises(ss.SketchError) as ei:
             sk.apply_f32acc(A, variant=VID[variant], **kw)
         assert ei.value.code == -6
