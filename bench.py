@@ -54,14 +54,16 @@ PAPER_GBPS = {"e1": (1 << 21) * 1024 * 4 / 7.11e-3 / 1e9}   # PAPER.md:322, H200
 L2_RED_PAYLOAD_GBPS = 6000.0   # measured with sketch_red_probe on this pool's B200 (profiles/r01_red_probe.md)
 VARIANTS = {"auto": 0, "flat_pair": 1, "flat_vec": 2, "smem": 3, "generic": 4, "tmem": 5, "small": 6}
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` captures (profiles/*.md name the commands); None where not captured.
-NCU_TRAFFIC_BYTES = {
-    ("c5", "smem"): 17448452000 + 4160000,   # profiles/r01_smem_c5.md: 17.448 GB read (A 17.180 + packed hashes 0.268) + 4 MB written
-    ("e1", "tmem"): 8594182000 + 3782912,    # profiles/r01_tmem_shapes.md
-    ("c4", "tmem"): 8590524000 + 3837184,
-    ("c5", "tmem"): 17180124000 + 3726080,   # profiles/r01_tmem_c5.md: 17.180 GB read (A only) + 3.7 MB written
-}
+def ncu_traffic(workload, variant):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, FROM THE COMMITTED `ncu --set full`
+    CAPTURES (profiles/ncu_traffic.json: one entry per (workload, variant) with the kernel name and the profile file that
+    holds the capture and its command); None where nothing was captured.  Not a measurement of this run."""
+    try:
+        table = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))
+    except (OSError, ValueError):
+        return None, None
+    e = table.get("%s/%s" % (workload, variant))
+    return (int(e["dram_bytes_read"]) + int(e["dram_bytes_written"]), e) if e else (None, None)
 
 
 def measured_peaks():
@@ -265,6 +267,27 @@ def run_ours(args):
         if dist is not None:
             all_reduce_sketch(out32, dist)
 
+    # like-for-like pairs (same privatisation on both sides): what FP16 PRECISION buys as opposed to what privatisation
+    # buys (Eq. (5)): flat REDs on both sides, and tensor memory on both sides where the FP32 partial fits
+    def flat16():
+        sk.apply_f16acc(A, out=out16, variant=VARIANTS["flat_vec"], row_begin=row_begin, rows=m)
+
+    def flat32():
+        sk.apply_f32acc(A, out=out32, variant=VARIANTS["flat_vec"], row_begin=row_begin, rows=m)
+
+    def tmem16():
+        sk.apply_f16acc(A, out=out16, variant=VARIANTS["tmem"], row_begin=row_begin, rows=m)
+
+    def tmem32():
+        sk.apply_f32acc(A, out=out32, variant=VARIANTS["tmem"], row_begin=row_begin, rows=m)
+
+    def can(f16, variant):
+        try:
+            sk.plan(n, f16=f16, variant=VARIANTS[variant], rows=m, row_begin=row_begin)
+            return True
+        except ss.SketchError:
+            return False
+
     def barrier():
         torch.cuda.synchronize()
         if dist is not None:
@@ -301,6 +324,15 @@ def run_ours(args):
     ms16, per16, launches16, (w0, w1) = timed(step16, args.steps, args.warmup)
     clocks = sampler.stop(w0, w1) if rank == 0 else None
     ms32, _, _, _ = timed(step32, max(2, args.steps // 2), 3)
+    pairs = {}
+    if not args.no_pairs and dist is None:
+        k2 = max(2, args.steps // 2)
+        if can(True, "flat_vec") and can(False, "flat_vec"):
+            a16, a32 = timed(flat16, k2, 3)[0], timed(flat32, k2, 3)[0]
+            pairs["flat"] = {"f16_ms": a16, "f32_ms": a32, "f16_over_f32": a32 / a16}
+        if can(True, "tmem") and can(False, "tmem"):
+            a16, a32 = timed(tmem16, k2, 3)[0], timed(tmem32, k2, 3)[0]
+            pairs["tmem"] = {"f16_ms": a16, "f32_ms": a32, "f16_over_f32": a32 / a16}
     ms16_apply, _, _, _ = timed(apply16, max(2, args.steps // 2), 3) if uses_packed else (ms16, None, None, None)
 
     # end to end through the host-buffer entry point: pinned A on the host, H2D + kernels + D2H inside the call
@@ -349,6 +381,7 @@ def run_ours(args):
         return 0
 
     peaks, peak_src = measured_peaks()
+    traffic, traffic_src = ncu_traffic(args.workload, plan16["variant"])
     abytes = algorithmic_bytes(m, n, d, 2)
     gbs = world * m * n * 4 / (ms16 * 1e-3) / 1e9
     achieved = abytes / (ms16_apply * 1e-3) / 1e9    # per GPU: the event bracket holds memset + scatter (+ fold)
@@ -370,12 +403,15 @@ def run_ours(args):
         "contributions_per_s": zeta * m * n * world / (ms16 * 1e-3),
         "half2_updates_per_s": red_ops * world / (ms16 * 1e-3),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm,
-                     "traffic": NCU_TRAFFIC_BYTES.get((args.workload, plan16["variant"])), "peak_source": peak_src,
+                     "traffic": traffic, "traffic_source": ("committed ncu capture %s (kernel %s)" % (traffic_src["profile"], traffic_src["kernel"])) if traffic_src else None,
+                     "peak_source": peak_src,
                      "frac_of_nominal_8TBps": achieved / 8000.0,
                      "algorithmic_bytes_per_launch": abytes,
                      "note": "dominant kernel = the scatter; CUDA-event bracket on the launching stream = zero-init memset + scatter (+ replica fold), hash-pack excluded"},
         "f32acc": {"ms_per_step": ms32, "GBps": world * m * n * 4 / (ms32 * 1e-3) / 1e9, "variant": plan32["variant"],
-                   "replicas": plan32["replicas"], "f16_speedup_over_f32": ms32 / ms16},
+                   "replicas": plan32["replicas"], "f16_speedup_over_f32": ms32 / ms16,
+                   "like_for_like": pairs,
+                   "note": "f16_speedup_over_f32 compares AUTO with AUTO; like_for_like holds both precisions on the same privatisation"},
         "e2e": e2e if e2e is not None else {"value": None, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0, "skipped": True},
         "gpu_launches": int(launches16),
         "clocks": clocks,
@@ -552,6 +588,7 @@ def main():
     ap.add_argument("--study", default=None, choices=["range", "ls"],
                     help="extra reports: config-5 range / rounding study; GPU sketch-and-solve least squares")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-pairs", action="store_true", help="skip the like-for-like flat/flat and tmem/tmem FP16-vs-FP32 timings")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-rows", type=int, default=1 << 21, help="rows per step of the reference arm's bounded sample")
     args = ap.parse_args()

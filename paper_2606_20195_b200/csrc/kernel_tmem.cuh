@@ -181,11 +181,12 @@ struct TmemGeom {
   // bucket group) a side list of up to T items of RB bytes, then the NPC * BQ item counts.
   static constexpr int RB = tmem_rec_bytes(ZB);
   static constexpr int E_BYTES = DEF ? T * BQ * RB : T * ZETA * 8;
-  // producer warps: one in the chained modes (two at n = 64); the deferral bookkeeping triples the hash stage's work, so there the
-  // stage's 32-row chunks go to NPC warps and the bucket groups of a chunk to NPB warps
+  // producer warps: up to four, one per SM sub-partition.  A producer warp shares its sub-partition's issue slots with one
+  // consumer warp and a stage is released when the SLOWEST consumer is done, so the hash stage is spread evenly: the
+  // stage's 32-row chunks go to NPC warps and the stack blocks (deferral: the bucket groups) of a chunk to NPB warps
   static constexpr int CH = (T + 31) / 32;
-  static constexpr int NPC = DEF ? (CH >= 2 ? 2 : 1) : (CH >= 4 ? 2 : 1);   // n = 64: 4 hashes per 256 B of A, two hash warps
-  static constexpr int NPB = DEF ? (BQ < 4 / NPC ? BQ : 4 / NPC) : 1;
+  static constexpr int NPC = DEF ? (CH >= 2 ? 2 : 1) : (CH >= 4 ? 4 : CH >= 2 ? 2 : 1);
+  static constexpr int NPB = DEF ? (BQ < 4 / NPC ? BQ : 4 / NPC) : (ZETA < 4 / NPC ? ZETA : 4 / NPC);
   static constexpr int NP = NPC * NPB;
   static constexpr int LCAP = T / NPC;         // rows one chunk phase hashes = the most it can defer
   static constexpr int L_BYTES = DEF ? NPC * BQ * LCAP * RB + 128 : 0;
@@ -204,8 +205,10 @@ struct TmemGeom {
 };
 
 __host__ __device__ constexpr int tmem_producers(int n, int bq, int gm, int zeta) {
-  return gm == 0 ? (tmem_stage_rows(n, bq, zeta) >= 128 ? 2 : 1)
-                 : (tmem_stage_rows(n, bq, zeta) >= 64 ? 2 : 1) * (bq < (tmem_stage_rows(n, bq, zeta) >= 64 ? 2 : 4) ? bq : (tmem_stage_rows(n, bq, zeta) >= 64 ? 2 : 4));
+  const int ch = (tmem_stage_rows(n, bq, zeta) + 31) / 32;
+  const int npc = gm == 0 ? (ch >= 4 ? 4 : ch >= 2 ? 2 : 1) : (ch >= 2 ? 2 : 1);
+  const int split = gm == 0 ? zeta : bq;
+  return npc * (split < 4 / npc ? split : 4 / npc);
 }
 // ring of stages | barriers + TMEM base (256 B) | chained bucket-group kernels: two converted (FP16) tiles | deferral:
 // one all-zero FP16 row + 2 KiB of producer scratch (the sketch rows of a 32-row chunk, a 128-byte line per warp and block)
@@ -300,7 +303,7 @@ template <int ZB> SK_DEVINL void sts_rec(uint32_t p, uint32_t head, const uint32
 
 // ---------------------------------------------------------------------------------------- the kernel
 template <int ZETA, int X, int S, int BQ, int NW, int GM, int MODE>
-__global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S, BQ, GM, ZETA)) * 32, 1) k_tmem(TmemArgs g, const __grid_constant__ CUtensorMap tmap) {
+__global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S, BQ, GM, ZETA) + 1) * 32, 1) k_tmem(TmemArgs g, const __grid_constant__ CUtensorMap tmap) {
   constexpr int FW = tm_fw(MODE);
   constexpr int T = tmem_stage_rows(32 * FW * X * S, BQ, ZETA), NS = tmem_stages(32 * FW * X * S);
   using Geo = TmemGeom<ZETA, X, S, BQ, NW, GM, T, MODE>;
@@ -342,7 +345,31 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
   const int64_t col0 = (int64_t)blockIdx.y * N;   // first feature of this CTA's column slice
   const uint32_t dloc = (uint32_t)g.d / BQ;        // sketch rows one warp holds
 
-  if (warp >= NW) {
+  if (warp >= NW + NP) {
+    // ================================================================ right-hand-side warp (launched only with a fused b)
+    // PAPER.md:356 "b in FP32 with the same map": Sb[bucket(i, j)] += +-s b_i, one result-discarding FP32 RED per (row,
+    // block), over the rows of this CTA's stages.  The warp shares nothing with the pipeline (it reads b from global memory
+    // and recomputes the zeta hashes of its rows), so the kernels without a right-hand side carry none of it; with column
+    // slices the CTAs of the first slice do it.
+    if (blockIdx.y == 0 && g.rhs != nullptr) {
+      float* const sb = g.Sb + (size_t)(blockIdx.x % (uint32_t)g.sb_replicas) * (size_t)g.sb_stride;
+      for (int64_t st = blockIdx.x; st < nstages; st += gridDim.x) {
+#pragma unroll 1
+        for (int32_t r = (int32_t)lane; r < T; r += 32) {
+          const int64_t row = st * T + r;
+          if (row < a.rows) {
+            const float bv = __fmul_rn(a.scale, g.rhs[row]);
+            const uint64_t ctr0 = (uint64_t)(a.row_begin + row) * ZETA;
+#pragma unroll
+            for (int j = 0; j < ZETA; ++j) {
+              const uint32_t e = hash_entry(a.seed, ctr0 + j, j, a.db);
+              red_f1(sb + entry_bucket(e), __uint_as_float(__float_as_uint(bv) ^ entry_signmask_f32(e)));
+            }
+          }
+        }
+      }
+    }
+  } else if (warp >= NW) {
     // ================================================================ producers: TMA + hash stage (a1, a2)
     const uint32_t pw = warp - NW;                 // producer warp pw: 32-row chunks cp, cp + NPC, ...; stack blocks [j0, j0 + JB)
     const uint32_t cp = pw % NPC, j0 = (pw / NPC) * JB, b0 = j0 / ZB;
@@ -413,14 +440,6 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
           bk[j] = entry_bucket(e);
           mulw[j] = tm_one(MODE) ^ (MODE == TM_F32 ? entry_signmask_f32(e) : entry_signmask_h2(e));
         }
-        // fused right-hand side ("b in FP32 with the same map"): the lane that hashed row r adds +-s b_r to
-        // the FP32 sketch of b, one result-discarding RED per stack block; the first column slice only
-        if (g.rhs != nullptr && blockIdx.y == 0 && live && row0 + r < a.rows) {
-          const float bv = __fmul_rn(a.scale, g.rhs[row0 + r]);
-          float* const sb = g.Sb + (size_t)(blockIdx.x % (uint32_t)g.sb_replicas) * (size_t)g.sb_stride;
-#pragma unroll
-          for (int j = 0; j < JB; ++j) red_f1(sb + bk[j], __uint_as_float(__float_as_uint(bv) ^ ((mulw[j] & (MODE == TM_F32 ? 0x80000000u : 0x8000u)) ? 0x80000000u : 0u)));
-        }
         // region of the consumer warp that owns (this row, bucket group b) when there is one feature slice
         auto abase = [&](uint32_t b) -> uint32_t {
           if constexpr (!Geo::ABS) return 0u;
@@ -432,14 +451,13 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
           // entry of (row, bucket group) is read by exactly one consumer warp, so it carries that warp's complete
           // tensor-memory address (abase) and the consumer saves an add per (row, block)
           if (live) {
-            const uint32_t p = sE + r * (ZETA * 8);
-            if constexpr (ZETA == 1) asm volatile("st.shared.v2.b32 [%0], {%1,%2};" ::"r"(p), "r"(abase(0) + bk[0] * X), "r"(mulw[0]) : "memory");
+            const uint32_t p = sE + r * (ZETA * 8) + j0 * 8;
+            auto ent = [&](int j) -> uint32_t { const uint32_t bg = (j0 + (uint32_t)j) / ZB; return abase(bg) + (bk[j] - bg * dloc) * X; };
+            if constexpr (JB == 1) asm volatile("st.shared.v2.b32 [%0], {%1,%2};" ::"r"(p), "r"(ent(0)), "r"(mulw[0]) : "memory");
             else {
 #pragma unroll
-              for (int k = 0; k < ZETA / 2; ++k)
-                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p + 16 * k),
-                             "r"(abase((2 * k) / ZB) + (bk[2 * k] - (uint32_t)((2 * k) / ZB) * dloc) * X), "r"(mulw[2 * k]),
-                             "r"(abase((2 * k + 1) / ZB) + (bk[2 * k + 1] - (uint32_t)((2 * k + 1) / ZB) * dloc) * X), "r"(mulw[2 * k + 1]) : "memory");
+              for (int k = 0; k < JB / 2; ++k)
+                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(p + 16 * k), "r"(ent(2 * k)), "r"(mulw[2 * k]), "r"(ent(2 * k + 1)), "r"(mulw[2 * k + 1]) : "memory");
             }
           }
         } else {

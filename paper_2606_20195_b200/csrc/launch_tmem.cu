@@ -23,7 +23,8 @@ cudaError_t go(const TmemArgs& g, const CUtensorMap& tmap, int grid, int cs, cud
     const size_t smem = tmem_smem_bytes(Z, N, BQ, GM, MODE);
     cudaError_t e = allow_max_dynamic_smem<k>();
     if (e != cudaSuccess) return e;
-    k<<<dim3((unsigned)grid, (unsigned)cs), (NW + tmem_producers(N, BQ, GM, Z)) * 32, smem, st>>>(g, tmap);
+    // one more warp when a right-hand side rides along (kernel_tmem.cuh: the right-hand-side warp)
+    k<<<dim3((unsigned)grid, (unsigned)cs), (NW + tmem_producers(N, BQ, GM, Z) + (g.rhs != nullptr ? 1 : 0)) * 32, smem, st>>>(g, tmap);
     return cudaGetLastError();
   }
 }

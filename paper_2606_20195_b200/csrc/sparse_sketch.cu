@@ -435,7 +435,7 @@ int ensure_packed(sketch* s, cudaStream_t st, bool force) {
 
 int validate_apply(const sketch* s, const void* A, int32_t n, int64_t lda, const void* B, bool f16,
                    const sketch_opts_t* o, int64_t* row_begin, int64_t* rows) {
-  if (!s || !A || !B) return SKETCH_ERR_NULL;
+  if (!s || !B) return SKETCH_ERR_NULL;
   if (n <= 0) return SKETCH_ERR_INVALID;
   if (lda < n) return SKETCH_ERR_LDA;
   if (!aligned(A, 4) || !aligned(B, 4)) return SKETCH_ERR_ALIGNMENT;  // f16: packed RED works on 4-byte words
@@ -446,6 +446,7 @@ int validate_apply(const sketch* s, const void* A, int32_t n, int64_t lda, const
   if (rb < 0 || r < 0 || rb > s->m) return SKETCH_ERR_INVALID;
   if (r == 0) r = s->m - rb;
   if (rb + r > s->m) return SKETCH_ERR_INVALID;
+  if (!A && r > 0) return SKETCH_ERR_NULL;   // an empty row range reads nothing: A may be NULL (an empty tensor has no storage)
   *row_begin = rb;
   *rows = r;
   return SKETCH_OK;

@@ -502,16 +502,30 @@ def test_forced_variant_fails_iff_the_plan_says_so_and_auto_never_does(ss):
     assert sk.plan(n)["variant"] == "flat_vec"
     got = sk.apply_f16acc(A)
     assert np.array_equal(oracle.half_bits_to_f64(bits(got)), oracle.f64_sketch(seed, d, zeta, wl.integer_valued(m, n, 21)))
-    # SR / FP32 on the RN-only privatised variants, odd n on the vector variants
+    # SR / dither / FP32 on the RN-only privatised variants (the tensor-memory kernel has every mode), odd n on the vector variants
     sk2 = ss.Sketch(5000, 256, 4, seed)
     A2 = dev(wl.integer_valued(5000, 128, 22))
-    for variant in ("tmem", "smem", "small"):
-        with pytest.raises(ss.SketchError) as ei:
-            sk2.apply_f16acc(A2, variant=VID[variant], rounding=ss.SR, sr_seed=1)
-        assert ei.value.code == -6
+    for variant in ("smem", "small"):
+        for rnd in (ss.SR, ss.DITHER):
+            with pytest.raises(ss.SketchError) as ei:
+                sk2.apply_f16acc(A2, variant=VID[variant], rounding=rnd, sr_seed=1)
+            assert ei.value.code == -6
         with pytest.raises(ss.SketchError) as ei:
             sk2.apply_f32acc(A2, variant=VID[variant])
         assert ei.value.code == -6
+        with pytest.raises(ss.SketchError) as ei:
+            sk2.apply_bf16acc(A2, variant=VID[variant])
+        assert ei.value.code == -6
+    # per-contribution conversion keeps one bucket group in tensor memory: d = 1024 at n = 128 needs two -> refused for SR only
+    sk3 = ss.Sketch(5000, 1024, 4, seed)
+    sk3.apply_f16acc(A2, variant=VID["tmem"])
+    with pytest.raises(ss.SketchError) as ei:
+        sk3.apply_f16acc(A2, variant=VID["tmem"], rounding=ss.SR, sr_seed=1)
+    assert ei.value.code == -6
+    # a rounding rule that does not exist, or one on the wrong element type
+    with pytest.raises(ss.SketchError) as ei:
+        sk2.apply_f16acc(A2, rounding=3)
+    assert ei.value.code == -1
     A3 = dev(wl.integer_valued(5000, 33, 23))
     for variant in ("flat_vec", "flat_pair", "tmem", "smem", "small"):
         with pytest.raises(ss.SketchError) as ei:

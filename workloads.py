@@ -196,3 +196,25 @@ def ls_paper_low_coherence_device(m: int, n: int, seed: int, device):
         e = torch.randn(r1 - r0, generator=g, device=device, dtype=torch.float64)
         b[r0:r1, 0] = (A[r0:r1].double().sum(dim=1) + 0.1 * e).to(torch.float32)
     return A, b
+
+
+def ls_paper_coherent_device(m: int, n: int, seed: int, device):
+    """Device form of `ls_paper_coherent`: A = [I_n; T] with T = 1e-3 G / sqrt(m - n), b = [x0 + nu; T x0],
+    nu_i ~ N(0, 0.5^2), under one row permutation: the n unit rows land at seeded random positions.  Returns (A [m, n] FP32,
+    b [m, 1] FP32)."""
+    import torch
+
+    g = torch.Generator(device=device)
+    g.manual_seed(seed)
+    A = gaussian_device(m, n, seed + 4000003, device)
+    A.mul_(float(1e-3 / np.sqrt(m - n)))
+    x0 = torch.randn(n, generator=g, device=device, dtype=torch.float64)
+    b = torch.empty((m, 1), dtype=torch.float32, device=device)
+    step = 1 << 18
+    for r0 in range(0, m, step):
+        r1 = min(m, r0 + step)
+        b[r0:r1, 0] = (A[r0:r1].double() @ x0).to(torch.float32)
+    pos = torch.randperm(m, generator=g, device=device)[:n]          # where the identity rows sit
+    A[pos] = torch.eye(n, dtype=torch.float32, device=device)
+    b[pos, 0] = (x0 + 0.5 * torch.randn(n, generator=g, device=device, dtype=torch.float64)).to(torch.float32)
+    return A, b
