@@ -177,7 +177,8 @@ struct TmemGeom {
   static constexpr int N = 32 * FW * X * S;    // features of the CTA's column slice
   static constexpr int WC = kTmemCols / (NW / 4);  // tensor-memory columns of one warp's private region
   static constexpr int A_BYTES = T * N * 4;
-  // chained modes: entries [row][zeta] {col, mul}.  Deferral: records [row][BQ] of RB bytes, then per (chunk phase,
+  // chained modes: entries [row][zeta] {col, mul}.  Deferral: records [BQ][row] of RB bytes (a warp's 32 rows of one
+  // bucket group are stored side by side: no bank conflicts), then per (chunk phase,
   // bucket group) a side list of up to T items of RB bytes, then the NPC * BQ item counts.
   static constexpr int RB = tmem_rec_bytes(ZB);
   static constexpr int E_BYTES = DEF ? T * BQ * RB : T * ZETA * 8;
@@ -513,7 +514,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
               co[jj] = abase(b) + (bk[bb * ZB + jj] - b * dloc) * X;
               mm[jj] = mulw[bb * ZB + jj];
             }
-            if (live) sts_rec<ZB>(sE + ((uint32_t)r * BQ + b) * RB, def ? Q0 - slot * (uint32_t)Geo::STAGE_BYTES : (uint32_t)r * Geo::Q_ROW, cm, mm);
+            if (live) sts_rec<ZB>(sE + (b * (uint32_t)T + (uint32_t)r) * RB, def ? Q0 - slot * (uint32_t)Geo::STAGE_BYTES : (uint32_t)r * Geo::Q_ROW, cm, mm);
             const uint32_t m = __ballot_sync(0xFFFFFFFFu, def);
             if (def) sts_rec<ZB>(sL + ((cp * BQ + b) * Geo::LCAP + cnt[bb] + __popc(m & ((1u << lane) - 1u))) * RB, (uint32_t)r, co, mm);
             cnt[bb] += __popc(m);
@@ -567,7 +568,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
     // per-contribution conversion (SR / dither): counter of this lane's first column pair (R14: (row zeta + j) ceil(n/2) + pair)
     [[maybe_unused]] const uint64_t npairs = ((uint64_t)a.n + 1u) >> 1;
     [[maybe_unused]] const uint64_t pair0 = ((uint64_t)col0 + slice * 64 * X + lane * 2 * X) >> 1;
-    const uint32_t e_off = Geo::DEF ? ((rowset * TR) * BQ + bgrp) * RB : (rowset * TR) * (ZETA * 8) + bgrp * (ZB * 8);
+    const uint32_t e_off = Geo::DEF ? (bgrp * T + rowset * TR) * RB : (rowset * TR) * (ZETA * 8) + bgrp * (ZB * 8);
     uint32_t it = 0;
     for (int64_t st = blockIdx.x; st < nstages; st += gridDim.x, ++it) {
       const uint32_t slot = it % NS, ph = (it / NS) & 1;
@@ -602,10 +603,10 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
         constexpr int NG = TR / G;
         uint32_t qo[2][G], col[3][G][ZB], mul[3][G][ZB], q[2][G][1][X];
 #pragma unroll
-        for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + r * (BQ * RB), qo[0][r], col[0][r], mul[0][r]);
+        for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + r * RB, qo[0][r], col[0][r], mul[0][r]);
         if constexpr (NG > 1) {
 #pragma unroll
-          for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + (G + r) * (BQ * RB), qo[1][r], col[1][r], mul[1][r]);
+          for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + (G + r) * RB, qo[1][r], col[1][r], mul[1][r]);
         }
 #pragma unroll
         for (int r = 0; r < G; ++r) lds_q<X>(qlane + qo[0][r], q[0][r][0]);
@@ -617,7 +618,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
           }
           if (gi + 2 < NG) {
 #pragma unroll
-            for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + ((gi + 2) * G + r) * (BQ * RB), qo[gi & 1][r], col[(gi + 2) % 3][r], mul[(gi + 2) % 3][r]);
+            for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + ((gi + 2) * G + r) * RB, qo[gi & 1][r], col[(gi + 2) % 3][r], mul[(gi + 2) % 3][r]);
           }
           // a5: read-modify-write of G x ZB sketch rows in tensor memory, pairwise distinct by construction
           tmem_rmw<G, ZB, X, false>(Geo::ABS ? 0u : region, q[gi & 1], col[gi % 3], mul[gi % 3]);
