@@ -463,28 +463,35 @@ def run_range_study(args):
         A.mul_(float(2.0 ** (k - prev)))      # exact in FP32
         prev = k
         counts = oracle.range_counts(zeta, sample * np.float32(2.0 ** k))
-        for rname, rmode in (("RN", ss.RN), ("SR", ss.SR)):
-            kw = dict(out=out, rounding=rmode, sr_seed=wl.sketch_seed(77))
+        out_bf = torch.empty((d, n), dtype=torch.bfloat16, device=dev)
+        for rname, rmode in (("RN", ss.RN), ("SR", ss.SR), ("dither", ss.DITHER), ("BF16", None)):
+            if rmode is None:
+                fn = lambda: sk.apply_bf16acc(A, out=out_bf)      # the BF16 control
+                res, variant = out_bf, sk.plan(n, f16=2)["variant"]
+            else:
+                kw = dict(out=out, rounding=rmode, sr_seed=wl.sketch_seed(77))
+                fn = lambda: sk.apply_f16acc(A, **kw)
+                res, variant = out, sk.plan(n, rounding=rmode)["variant"]
             for _ in range(2):
-                sk.apply_f16acc(A, **kw)
+                fn()
             torch.cuda.synchronize()
-            reps = 5 if rmode == ss.RN else 2
+            reps = 5 if rname in ("RN", "BF16") else 3
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
             for _ in range(reps):
-                sk.apply_f16acc(A, **kw)
+                fn()
             e1.record()
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1) / reps
-            got = out[:, cols].float().cpu().numpy().astype(np.float64)
+            got = res[:, cols].float().cpu().numpy().astype(np.float64)
             want = B0 * 2.0 ** k
             fin = np.isfinite(got)
             rel = ev.rel_fro(got[fin], want[fin]) if fin.any() else None
             rows_out.append({
-                "k": k, "rounding": rname, "variant": sk.plan(n, rounding=rmode)["variant"], "ms": ms,
+                "k": k, "rounding": rname, "variant": variant, "ms": ms,
                 "GBps": m * n * 4 / (ms * 1e-3) / 1e9,
-                "nonfinite_outputs": int((~torch.isfinite(out)).sum().item()), "nan_outputs": int(torch.isnan(out).sum().item()),
-                "zero_outputs": int((out == 0).sum().item()), "outputs": d * n,
+                "nonfinite_outputs": int((~torch.isfinite(res)).sum().item()), "nan_outputs": int(torch.isnan(res).sum().item()),
+                "zero_outputs": int((res == 0).sum().item()), "outputs": d * n,
                 "relF_vs_f64_sampled_cols_finite": rel,
                 "oracle_contribution_counts_first_65536_rows": {kk: int(v) for kk, v in counts.items()},
             })
@@ -494,64 +501,46 @@ def run_range_study(args):
     return 0
 
 
+def _time_ms(fn, reps=5, warm=2, flush=None):
+    import torch
+
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(reps):
+        if flush is not None:
+            flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        fn()
+        e1.record()
+        torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    ts.sort()
+    return ts[len(ts) // 2]
+
+
 def run_ls_study(args):
-    """SURVEY 8f NEXT-1 (Fig. 6): complete sketch-and-solve least squares on the GPU for the paper's
-    low-coherence family at its own shape (m = 2^21, n = 1024, zeta = 4): sketch A (FP16 or FP32 path of THIS library) and
-    b (FP32, same map), widen exactly, FP32 thin QR + triangular solve (torch.linalg -> cuSOLVER/cuBLAS: library code, as
-    in the paper), original-system residual in FP64.  One JSON line; not the driver's bench line."""
+    """SURVEY 8f NEXT-1 (Fig. 6): complete sketch-and-solve least squares on the GPU at the paper's own
+    shape (m = 2^21, n = 1024, zeta = 4), both of its families, d/n in {2, 4, 8, 16, 32}: [A | b] sketched in ONE pass
+    (sketch_apply_f16acc_with_rhs / _f32acc_with_rhs: A in the chosen precision, b in FP32, same map), exact widening,
+    FP32 Householder QR + projection + triangular solve (cuSOLVER / cuBLAS through torch: library code, as in the paper),
+    original-system residual in FP64.  Median of 5 timed solves per point.  One JSON line; not the driver's bench line."""
     import torch
 
     import paper_2606_20195_b200 as ss
     import workloads as wl
+    from paper_2606_20195_b200 import lstsq
 
     torch.cuda.set_device(0)
     dev = torch.device("cuda", 0)
     m, n, zeta = 1 << 21, 1024, 4
-    A, b = wl.ls_paper_low_coherence_device(m, n, 6, dev)
-    bnorm = float(b.double().norm())
-    rows_out = []
-    for ratio in (2, 4, 8):
-        d = ratio * n
-        sk = ss.Sketch(m, d, zeta, wl.sketch_seed(0))
-        SA16 = torch.empty((d, n), dtype=torch.float16, device=dev)
-        SA32 = torch.empty((d, n), dtype=torch.float32, device=dev)
-        Sb = torch.empty((d, 1), dtype=torch.float32, device=dev)
-
-        def solve(f16):
-            if f16:
-                sk.apply_f16acc(A, out=SA16)
-                M = SA16.float()                      # exact widening (PAPER.md:356)
-            else:
-                sk.apply_f32acc(A, out=SA32)
-                M = SA32
-            sk.apply_f32acc(b, out=Sb)
-            Q, R = torch.linalg.qr(M, mode="reduced")
-            return torch.linalg.solve_triangular(R, Q.T @ Sb, upper=True)
-
-        def timed(f16, reps=5):
-            for _ in range(2):
-                solve(f16)
-            torch.cuda.synchronize()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            for _ in range(reps):
-                x = solve(f16)
-            e1.record()
-            torch.cuda.synchronize()
-            return e0.elapsed_time(e1) / reps, x
-
-        def sketch_only(f16, reps=5):
-            fn = (lambda: sk.apply_f16acc(A, out=SA16)) if f16 else (lambda: sk.apply_f32acc(A, out=SA32))
-            for _ in range(2):
-                fn()
-            torch.cuda.synchronize()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            for _ in range(reps):
-                fn()
-            e1.record()
-            torch.cuda.synchronize()
-            return e0.elapsed_time(e1) / reps
+    fams = []
+    for fam, gen in (("low_coherence", wl.ls_paper_low_coherence_device), ("coherent", wl.ls_paper_coherent_device)):
+        A, b2 = gen(m, n, 6, dev)
+        b = b2[:, 0].contiguous()
+        bnorm = float(b.double().norm())
 
         def residual(x):
             acc = 0.0
@@ -561,18 +550,157 @@ def run_ls_study(args):
                 acc += float((r * r).sum())
             return acc ** 0.5 / bnorm
 
-        t16, x16 = timed(True)
-        t32, x32 = timed(False)
-        r16, r32 = residual(x16), residual(x32)
-        rows_out.append({"d_over_n": ratio, "d": d, "fp16_variant": sk.plan(n)["variant"],
-                         "ls_ms_fp16_sketch": t16, "ls_ms_fp32_sketch": t32, "ls_speedup_fp16_over_fp32": t32 / t16,
-                         "sketch_ms_fp16": sketch_only(True), "sketch_ms_fp32": sketch_only(False),
-                         "residual_fp16": r16, "residual_fp32": r32, "residual_increase_pct": 100.0 * (r16 / r32 - 1.0)})
+        rows_out = []
+        for ratio in (2, 4, 8, 16, 32):
+            d = ratio * n
+            sk = ss.Sketch(m, d, zeta, wl.sketch_seed(0))
+            W = torch.empty((d, n), dtype=torch.float32, device=dev)
+            bufs = {"f16": torch.empty((d, n), dtype=torch.float16, device=dev), "f32": torch.empty((d, n), dtype=torch.float32, device=dev),
+                    "bf16": torch.empty((d, n), dtype=torch.bfloat16, device=dev)}
+            Sb = torch.empty((d,), dtype=torch.float32, device=dev)
+            row = {"d_over_n": ratio, "d": d, "fp16_variant": sk.plan(n, f16=1)["variant"], "fp32_variant": sk.plan(n, f16=0)["variant"]}
+            for prec in ("f16", "f32", "bf16"):
+                solve = lambda: lstsq.sketch_and_solve(sk, A, b, prec, SA=bufs[prec], Sb=Sb, W=W)
+                row["ls_ms_" + prec] = _time_ms(solve)
+                row["sketch_ms_" + prec] = _time_ms(lambda: lstsq.sketch_system(sk, A, b, prec, SA=bufs[prec], Sb=Sb))
+                row["residual_" + prec] = residual(solve())
+            row["ls_speedup_f16_over_f32"] = row["ls_ms_f32"] / row["ls_ms_f16"]
+            row["residual_increase_pct_f16"] = 100.0 * (row["residual_f16"] / row["residual_f32"] - 1.0)
+            row["residual_increase_pct_bf16"] = 100.0 * (row["residual_bf16"] / row["residual_f32"] - 1.0)
+            rows_out.append(row)
+            del W, bufs
+        fams.append({"family": fam, "rows": rows_out})
+        del A, b, b2
+        torch.cuda.empty_cache()
     print(json.dumps({"study": "sketch-and-solve least squares (SURVEY 8f NEXT-1)",
-                      "workload": "paper low-coherence family, m=%d n=%d zeta=%d, sigma linear 100->1, b = A 1 + N(0, 0.1^2)" % (m, n, zeta),
-                      "paper_context": "H200 NVL (PAPER.md:368-370): FP16 SS 13.921 ms at d/n=2, 1.47x over its FP32 pipeline, residual 0.1155, +0.34 % over FP32",
-                      "rows": rows_out}))
+                      "workload": "the paper's two families (PAPER.md:362-366), m=%d n=%d zeta=%d; low-coherence: sigma linear 100->1, b = A 1 + N(0, 0.1^2); "
+                                  "coherent: [I_n; 1e-3 G / sqrt(m-n)] under a row permutation, b = [x0 + N(0, 0.5^2); T x0]" % (m, n, zeta),
+                      "pipeline": "one-pass [A|b] sketch -> sketch_widen -> torch.geqrf -> torch.ormqr -> solve_triangular (paper_2606_20195_b200/lstsq.py)",
+                      "paper_context": "H200 NVL (PAPER.md:368-370): FP16 SS 13.921 ms at d/n=2 -> 35.016 ms at d/n=32, 1.47x / 1.44x over its FP32 pipeline, residual 0.1155 -> 0.08223, +0.34 % / +0.35 % over FP32; BF16 ~20 % above FP32 at d/n=2 (PAPER.md:396)",
+                      "families": fams}))
     return 0
+
+
+def run_grid_study(args):
+    """the paper's complete-sketch timing grid (Fig. 2) as one command: n = 1024,
+    m in {2^19, 2^20, 2^21}, d/n in {2 .. 256}, zeta in {1, 2, 4, 8}, dense (singular values linear 1000 -> 1) and coordinate
+    [I_n 0]^T inputs.  Per point: complete-sketch time of the FP16 and FP32 paths (median of 5, L2 flushed when A < 512 MiB...
+    never at these sizes), the variant AUTO picked, GB/s of A, fraction of the HBM peak and -- for the flat variants -- of the
+    measured L2-atomic payload rate.  One JSON line; not the driver's bench line."""
+    import torch
+
+    import paper_2606_20195_b200 as ss
+    import workloads as wl
+
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    n = 1024
+    quick = args.grid == "quick"
+    ms_list = (1 << 19, 1 << 21) if quick else (1 << 19, 1 << 20, 1 << 21)
+    ratios = (2, 256) if quick else (2, 4, 8, 16, 32, 64, 128, 256)
+    zetas = (1, 4, 8) if quick else (1, 2, 4, 8)
+    peaks, peak_src = measured_peaks()
+    hbm = float(peaks["hbm_gbs"])
+    pts = []
+    for m in ms_list:
+        for kind in ("dense", "coordinate"):
+            if kind == "dense":
+                A = wl.gaussian_device(m, n, 5, dev)
+                A.mul_((torch.linspace(1000.0, 1.0, n, device=dev) / float(m) ** 0.5)[None, :])   # sigma linear 1000 -> 1 (PAPER.md:318)
+            else:
+                A = torch.zeros((m, n), dtype=torch.float32, device=dev)
+                A[:n] = torch.eye(n, device=dev)
+            for ratio in ratios:
+                d = ratio * n
+                o16 = torch.empty((d, n), dtype=torch.float16, device=dev)
+                o32 = torch.empty((d, n), dtype=torch.float32, device=dev)
+                for zeta in zetas:
+                    sk = ss.Sketch(m, d, zeta, wl.sketch_seed(0))
+                    p16, p32 = sk.plan(n, f16=1), sk.plan(n, f16=0)
+                    t16 = _time_ms(lambda: sk.apply_f16acc(A, out=o16), reps=5 if not quick else 3)
+                    t32 = _time_ms(lambda: sk.apply_f32acc(A, out=o32), reps=5 if not quick else 3)
+                    pt = {"m": m, "input": kind, "d_over_n": ratio, "zeta": zeta, "fp16_ms": t16, "fp32_ms": t32, "fp16_over_fp32": t32 / t16,
+                          "fp16_variant": p16["variant"], "fp32_variant": p32["variant"], "fp16_GBps": m * n * 4 / t16 / 1e6,
+                          "fp16_frac_hbm": (4 * m * n + 2 * d * n) / (t16 * 1e-3) / 1e9 / hbm,
+                          "fp32_frac_hbm": (4 * m * n + 4 * d * n) / (t32 * 1e-3) / 1e9 / hbm}
+                    if p16["variant"] in ("flat_vec", "flat_pair"):
+                        pt["fp16_frac_l2_atomic"] = 2.0 * zeta * m * n / (t16 * 1e-3) / 1e9 / L2_RED_PAYLOAD_GBPS
+                    if p32["variant"] in ("flat_vec", "flat_pair"):
+                        pt["fp32_frac_l2_atomic"] = 4.0 * zeta * m * n / (t32 * 1e-3) / 1e9 / L2_RED_PAYLOAD_GBPS
+                    pts.append(pt)
+                    sk.close()
+                del o16, o32
+            del A
+            torch.cuda.empty_cache()
+    print(json.dumps({"study": "paper timing grid (SURVEY 8f NEXT-2; PAPER.md:318-322)", "n": n, "hbm_peak_GBps": hbm, "peak_source": peak_src,
+                      "l2_atomic_payload_GBps": L2_RED_PAYLOAD_GBPS,
+                      "paper_context": "H200 NVL: FP16 SS 7.11 ms at m=2^21, d=2n, zeta=4 (PAPER.md:322); FP16 up to 1.91x its FP32 scatter (PAPER.md:320)",
+                      "points": pts}))
+    return 0
+
+
+def run_graph_study(args):
+    """Launch-bound config 1 (256 KiB of A): the complete FP16 and FP32 sketches captured once into a CUDA graph each (the ABI
+    neither synchronises nor allocates after the first call) and replayed; per-replay time from events around 200 replays."""
+    import torch
+
+    import paper_2606_20195_b200 as ss
+    import workloads as wl
+
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    out = []
+    for name in ("c1", "c2"):
+        m, n, d, zeta, mseed = WORKLOADS[name]
+        A = wl.gaussian_device(m, n, mseed, dev)
+        sk = ss.Sketch(m, d, zeta, wl.sketch_seed(0))
+        o16 = torch.empty((d, n), dtype=torch.float16, device=dev)
+        o32 = torch.empty((d, n), dtype=torch.float32, device=dev)
+        row = {"workload": name, "fp16_variant": sk.plan(n, f16=1)["variant"], "fp32_variant": sk.plan(n, f16=0)["variant"]}
+        st = torch.cuda.Stream()
+        for key, fn in (("fp16", lambda: sk.apply_f16acc(A, out=o16, stream=st)), ("fp32", lambda: sk.apply_f32acc(A, out=o32, stream=st))):
+            with torch.cuda.stream(st):
+                fn()
+                st.synchronize()
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=st):
+                    fn()
+                for _ in range(20):
+                    g.replay()
+                st.synchronize()
+                reps = 200
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(st)
+                for _ in range(reps):
+                    g.replay()
+                e1.record(st)
+                st.synchronize()
+                row[key + "_us_per_replay_warm_L2"] = e0.elapsed_time(e1) / reps * 1e3
+        row["fp16_over_fp32"] = row["fp32_us_per_replay_warm_L2"] / row["fp16_us_per_replay_warm_L2"]
+        out.append(row)
+    print(json.dumps({"study": "CUDA-graph replay of the launch-bound configs (warm L2: back-to-back replays of a 256 KiB / 256 MiB input)", "rows": out}))
+    return 0
+
+
+def self_launch(args):
+    """`python bench.py --gpus N` without a torchrun environment: re-run this very command under torch.distributed.run
+    with N ranks on this node (one process per GPU, rendezvous on 127.0.0.1), so the line printed carries n_gpus = N only
+    when N communicator ranks exist.  NCCL's own INFO lines stay on stderr for whoever wants to count the ranks."""
+    import socket
+
+    import torch
+
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        raise SystemExit("bench.py --gpus %d: this node has %d GPU(s)" % (args.gpus, have))
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus), "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd, env=env)
 
 
 def main():
@@ -585,8 +713,10 @@ def main():
     ap.add_argument("--variant", default="auto", choices=sorted(VARIANTS))
     ap.add_argument("--replicas", type=int, default=0)
     ap.add_argument("--hash-mode", type=int, default=0)
-    ap.add_argument("--study", default=None, choices=["range", "ls"],
-                    help="extra reports: config-5 range / rounding study; GPU sketch-and-solve least squares")
+    ap.add_argument("--study", default=None, choices=["range", "ls", "grid", "graph"],
+                    help="extra reports: config-5 range / rounding study; GPU sketch-and-solve least squares; the paper's timing "
+                         "grid (PAPER.md:318-322); launch-bound config 1 replayed from a CUDA graph")
+    ap.add_argument("--grid", default="full", choices=["full", "quick"], help="--study grid: every point, or the corners")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-pairs", action="store_true", help="skip the like-for-like flat/flat and tmem/tmem FP16-vs-FP32 timings")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -596,10 +726,16 @@ def main():
         args.warmup = 3                           # timing rule: W >= 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.study is None:
+        return self_launch(args)
     if args.study == "range":
         return run_range_study(args)
     if args.study == "ls":
         return run_ls_study(args)
+    if args.study == "grid":
+        return run_grid_study(args)
+    if args.study == "graph":
+        return run_graph_study(args)
     return run_ours(args)
 
 

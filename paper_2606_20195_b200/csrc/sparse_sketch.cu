@@ -199,7 +199,8 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, int o
     // 2.99 vs 2.74 TB/s; without bucket groups -- d = 384 at n = 192 -- the same slices run at 4.65 TB/s)
     // (the FP32 path privatised in tensor memory beats its flat REDs wherever it fits: 1.4 TB/s is the L2-atomic ceiling
     // of an FP32 zeta = 4 scatter)
-    if (tm_ok && (!f16 || !(tm.X * tm.S == 1 && tm.BQ > 1 && tm.BQ != s->zeta)) && rows * (int64_t)n > (1 << 20)) v = SKETCH_VARIANT_TMEM;
+    // (at zeta = 8 the flat REDs carry twice the payload: n = 1024, d = 2048 runs 4.68 ms in tensor memory against 6.04 ms flat)
+    if (tm_ok && (!f16 || s->zeta > 4 || !(tm.X * tm.S == 1 && tm.BQ > 1 && tm.BQ != s->zeta)) && rows * (int64_t)n > (1 << 20)) v = SKETCH_VARIANT_TMEM;
     else if (sm_ok && s->zeta >= 2) v = SKETCH_VARIANT_SMEM;
     // launch-bound inputs into a sketch of a few KiB: the flat REDs queue ~1000 deep on each L2 sector (c1: 10 us);
     // per-warp shared-memory partials need no such queue
