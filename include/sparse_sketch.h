@@ -185,6 +185,15 @@ int sketch_apply_f16acc_host(const sketch_t* s, const float* A_host, int32_t n, 
 int sketch_red_probe(void* sketch_dev, int32_t d, int32_t n, int32_t kind, int32_t replicas,
                      int32_t grid_ctas, int32_t iters, uint64_t* red_ops_out, void* stream);
 
+/* The conversion step in isolation, for tests: out_dev[k] (16-bit pattern) = conversion of p_dev[k] under
+ * kind with the random bits rbits_dev[k]:  0 = RN16;  1 = SR16, reading R13 with r24 = rbits & 0xFFFFFF
+ * (PAPER.md:203-207);  2 = dither, Eq. (6), same r24;  3 = bfloat16 RN;  4 / 5 = the hardware
+ * cvt.rs.f16x2.f32 d, a, b, rbits with p in both sources: the half converted from b / from a.  The library's SR kernels
+ * use rule 1, never the hardware instruction: the two agree on the FP16 normal grid under a fixed bit mapping and
+ * differ below 2^-14 (tests/test_gpu_modes.py).  rbits_dev may be NULL for kinds 0 and 3.  Device pointers. */
+int sketch_convert_probe(const float* p_dev, const uint32_t* rbits_dev, int64_t count, int32_t kind, uint16_t* out_dev,
+                         void* stream);
+
 /* Which variant / replica count / hash mode AUTO resolves to for this shape; host-only, no launch.
  * is_f16: 0 = f32acc, 1 = f16acc, 2 = bf16acc.  Any out pointer may be NULL. */
 int sketch_plan(const sketch_t* s, int32_t n, int64_t lda, int is_f16, int rounding, const sketch_opts_t* opts,

@@ -21,6 +21,7 @@ from .binding import (  # noqa: F401
     SketchOpts,
     lib,
     library_path,
+    sketch_convert_probe,
     sketch_launch_count,
     sketch_red_probe,
     sketch_strerror,

@@ -58,6 +58,7 @@ SYMBOLS = {
     "sketch_apply_f32acc_host": (_int, [_vp, _vp, _i32, _i64, _vp, _OP]),
     "sketch_apply_f16acc_host": (_int, [_vp, _vp, _i32, _i64, _vp, _int, _u64, _OP]),
     "sketch_red_probe": (_int, [_vp, _i32, _i32, _i32, _i32, _i32, _i32, C.POINTER(_u64), _vp]),
+    "sketch_convert_probe": (_int, [_vp, _vp, _i64, _i32, _vp, _vp]),
     "sketch_plan": (_int, [_vp, _i32, _i64, _int, _int, _OP, C.POINTER(_i32), C.POINTER(_i32), C.POINTER(_i32), C.POINTER(_i32)]),
     "sketch_launch_count": (_u64, []),
     "sketch_strerror": (C.c_char_p, [_int]),
@@ -135,6 +136,25 @@ def sketch_widen(B16, out=None, stream=None):
     rc = lib().sketch_widen(B16.data_ptr(), B16.numel(), int(B16.dtype == torch.bfloat16), out.data_ptr(), _stream_ptr(stream))
     if rc:
         raise SketchError(rc, "sketch_widen")
+    return out
+
+
+def sketch_convert_probe(p, rbits, kind: int, out=None, stream=None):
+    """The conversion step alone (sketch_convert_probe): p FP32 CUDA tensor, rbits int32 CUDA tensor of the same size or
+    None; returns the 16-bit patterns as an int16 tensor."""
+    import torch
+
+    _check_cuda(p, torch.float32, "p")
+    if rbits is not None:
+        _check_cuda(rbits, torch.int32, "rbits")
+        assert rbits.is_contiguous() and rbits.numel() == p.numel()
+    assert p.is_contiguous()
+    if out is None:
+        out = torch.empty(p.shape, dtype=torch.int16, device=p.device)
+    rc = lib().sketch_convert_probe(p.data_ptr(), rbits.data_ptr() if rbits is not None else None, p.numel(), kind, out.data_ptr(),
+                                    _stream_ptr(stream))
+    if rc:
+        raise SketchError(rc, "sketch_convert_probe")
     return out
 
 

@@ -2,6 +2,7 @@
 //   k_hash_dump / k_hash_pack32   a1  hash stage (dump for tests; plain 32-bit packed array)
 //   k_reduce_replicas<...>        folds the P L2-resident partial sketches of the flat variant
 //   k_red_probe<...>              L2 atomic-throughput microbenchmark (roofline term 2)
+//   k_convert_probe               a4 in isolation: RN / SR / dither / bfloat16 / the hardware cvt.rs, element by element
 #pragma once
 
 #include "args.h"
@@ -97,6 +98,33 @@ __global__ void __launch_bounds__(kFlatThreads) k_red_probe(void* sketch, int32_
     else if constexpr (KIND == 3) red_f1(reinterpret_cast<float*>(base) + off, fv);
     else if constexpr (KIND == 4) red_f2(reinterpret_cast<float*>(base) + off, fv, fv);
     else red_f4(reinterpret_cast<float*>(base) + off, fv, fv, fv, fv);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a4 in isolation (tests; SURVEY 8c row 14 "the hardware cvt.rs.f16x2.f32 may be used only if shown bit-identical"):
+// out[k] = the 16-bit conversion of p[k] under `kind` with the random bits r[k].
+//   0 RN16   1 SR16 (R13, r24 = r & 0xFFFFFF)   2 dither (R20, same r24)   3 bfloat16 RN
+//   4 / 5    hardware cvt.rs.f16x2.f32 d, a, b, rbits with p in BOTH sources: the half converted from b (low, 4) / a (high, 5)
+// ------------------------------------------------------------------------------------------------
+__global__ void k_convert_probe(const float* __restrict__ p, const uint32_t* __restrict__ r, int64_t count, int kind, uint16_t* __restrict__ out) {
+  int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < count; k += stride) {
+    const float x = p[k];
+    const uint32_t rb = r ? r[k] : 0u;
+    uint32_t v;
+    switch (kind) {
+      case 0: v = pack_rn(x, x) & 0xFFFFu; break;
+      case 1: v = sr16_bits(x, rb & 0xFFFFFFu); break;
+      case 2: v = pack_rn(dither_f32(x, rb & 0xFFFFFFu), 0.f) & 0xFFFFu; break;
+      case 3: v = pack_bf16_rn(x, x) & 0xFFFFu; break;
+      default: {
+        uint32_t d;
+        asm("cvt.rs.f16x2.f32 %0, %1, %2, %3;" : "=r"(d) : "f"(x), "f"(x), "r"(rb));
+        v = kind == 4 ? (d & 0xFFFFu) : (d >> 16);
+      }
+    }
+    out[k] = (uint16_t)v;
   }
 }
 

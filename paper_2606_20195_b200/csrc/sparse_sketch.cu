@@ -877,6 +877,17 @@ int sketch_red_probe(void* sketch_dev, int32_t d, int32_t n, int32_t kind, int32
   return launch_check("k_red_probe");
 }
 
+int sketch_convert_probe(const float* p_dev, const uint32_t* rbits_dev, int64_t count, int32_t kind, uint16_t* out_dev, void* stream) {
+  if (!p_dev || !out_dev) return SKETCH_ERR_NULL;
+  if (count < 0 || kind < 0 || kind > 5) return SKETCH_ERR_INVALID;
+  if ((kind == 1 || kind == 2 || kind >= 4) && !rbits_dev) return SKETCH_ERR_NULL;
+  if (count == 0) return SKETCH_OK;
+  int64_t blocks = (count + 255) / 256;
+  int grid = (int)(blocks < 148 * 16 ? blocks : 148 * 16);
+  sk::k_convert_probe<<<grid, 256, 0, reinterpret_cast<cudaStream_t>(stream)>>>(p_dev, rbits_dev, count, kind, out_dev);
+  return launch_check("k_convert_probe");
+}
+
 int sketch_plan(const sketch_t* cs, int32_t n, int64_t lda, int is_f16, int rounding, const sketch_opts_t* opts,
                 int32_t* variant_out, int32_t* replicas_out, int32_t* hash_mode_out, int32_t* grid_out) {
   sketch* s = const_cast<sketch*>(cs);
