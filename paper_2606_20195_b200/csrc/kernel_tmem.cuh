@@ -147,18 +147,21 @@ __host__ __device__ constexpr int tmem_stage_rows(int n, int bq, int zeta) {
   return n <= 64 ? ((bq == 1 || zeta == bq) ? 128 : 64) : n <= 128 ? 64 : n == 256 ? 32 : 16;
 }
 __host__ __device__ constexpr int tmem_stages(int n) { return n <= 512 ? 4 : 3; }
-// bytes of one (row, bucket group) record / side-list item of the deferral modes: {q offset | row, 0, then (col, mul) x ZB}
+// bytes of one (row, bucket group) side-list item of the deferral modes: {row | slot << 16, 0, then (col, mul) x ZB}
 __host__ __device__ constexpr int tmem_rec_bytes(int zb) { return zb == 1 ? 16 : 16 + 8 * zb; }
 
 // GM = group mode: how two rows of one group that hit the same sketch row are kept from losing an update.
 //   0      groups of G = 2 (4 for short block lists) rows; same-bucket rows are chained in registers.  Works for any
 //          d, costs O(G^2) compares and selects per block, so G stays small and few LDTMs are in flight.
-//   1, 2   DEFERRAL, groups of 4 / 8 rows, bucket-group kernels only (BQ > 1).  The producer finds every row that
-//          shares a sketch row with a LATER row of its group (rare when d / zeta >> G^2), points that row's main-loop
-//          record at an all-zero FP16 row and, in the clashing blocks, at a substitute sketch row that no row of the
-//          group touches (adding +0 there changes nothing), and appends the row to a per-stage side list that the
-//          consumers apply one row at a time after the main loop.  The main loop then has pairwise distinct TMEM
-//          addresses within a group by construction: no compares, no selects, 8 read-modify-writes in flight.
+//   1, 2   DEFERRAL, groups of 4 / 8 rows, bucket-group kernels only (BQ > 1).  The producers find every row that
+//          shares a sketch row -- in any stack block -- with a LATER row of its group (rare when d / zeta >> G^2).  Such a
+//          row is deferred as a whole: its converted FP16 words are moved to a side buffer (the upper half of the stage's
+//          FP32 tile, free once the stage is converted in place) and its tile row is zeroed, its main-loop records point,
+//          in the clashing blocks, at a substitute sketch row that no row of the group touches (adding +0 there changes
+//          nothing), and it is appended to per-stage side lists that the consumers apply one row at a time after the main
+//          loop.  The main loop then has pairwise distinct TMEM addresses within a group by construction -- no compares, no
+//          selects, 8 read-modify-writes in flight -- reads every row's FP16 words at a compile-time offset, and its records
+//          are bare {address, multiplier} pairs (two rows per 16-byte load with one block per warp).
 template <int ZETA, int X, int S, int BQ, int NW, int GM, int T, int MODE = TM_F16>
 struct TmemGeom {
   static constexpr int FW = tm_fw(MODE);
@@ -180,8 +183,9 @@ struct TmemGeom {
   // chained modes: entries [row][zeta] {col, mul}.  Deferral: records [BQ][row] of RB bytes (a warp's 32 rows of one
   // bucket group are stored side by side: no bank conflicts), then per (chunk phase,
   // bucket group) a side list of up to T items of RB bytes, then the NPC * BQ item counts.
-  static constexpr int RB = tmem_rec_bytes(ZB);
-  static constexpr int E_BYTES = DEF ? T * BQ * RB : T * ZETA * 8;
+  static constexpr int RB = tmem_rec_bytes(ZB);      // side-list item
+  static constexpr int REC = 8 * ZB;                 // main-loop record {col, mul} x ZB
+  static constexpr int E_BYTES = DEF ? T * BQ * REC : T * ZETA * 8;
   // producer warps: up to four, one per SM sub-partition.  A producer warp shares its sub-partition's issue slots with one
   // consumer warp and a stage is released when the SLOWEST consumer is done, so the hash stage is spread evenly: the
   // stage's 32-row chunks go to NPC warps and the stack blocks (deferral: the bucket groups) of a chunk to NPB warps
@@ -216,9 +220,9 @@ __host__ __device__ constexpr int tmem_producers(int n, int bq, int gm, int zeta
 constexpr size_t tmem_smem_bytes(int zeta, int n, int bq, int gm, int mode = TM_F16) {
   const size_t t = (size_t)tmem_stage_rows(n, bq, zeta);
   const size_t rb = (size_t)tmem_rec_bytes(zeta / bq);
-  const size_t e = gm ? 2 * t * bq * rb + 128 : t * zeta * 8;   // records + side lists (T rows in all) + counts
+  const size_t e = gm ? t * bq * (8 * (size_t)(zeta / bq)) + t * bq * rb + 128 : t * zeta * 8;   // records + side lists (T rows in all) + counts
   const bool shq = bq > 1 && (mode == TM_F16 || mode == TM_BF16);
-  return (size_t)tmem_stages(n) * (t * n * 4 + e) + 256 + (gm ? (size_t)n * 2 + 2048 : shq ? 2 * t * n * 2 : 0);
+  return (size_t)tmem_stages(n) * (t * n * 4 + e) + 256 + (gm ? 256 + 2048 : shq ? 2 * t * n * 2 : 0);
 }
 
 // a5 for R rows x ZB stack blocks of one warp: LDTM, one RN16 add per half (fma.rn.f16x2 by +-1), STTM.
@@ -311,7 +315,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
   constexpr int TR = Geo::TR, G = Geo::G, N = Geo::N, ZB = Geo::ZB, RB = Geo::RB, NP = Geo::NP, NPC = Geo::NPC, NPB = Geo::NPB;
   static_assert(NP == tmem_producers(N, BQ, GM, ZETA), "producer warps");
   constexpr int JB = ZETA / NPB;                     // stack blocks one producer warp hashes
-  constexpr uint32_t Q0 = NS * Geo::STAGE_BYTES + 256;   // first converted tile (chained modes) / the zero row (deferral)
+  constexpr uint32_t Q0 = NS * Geo::STAGE_BYTES + 256;   // first converted tile (chained modes) / producer scratch (deferral)
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   const ScatterArgs& a = g.s;
   const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -333,9 +337,6 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async;" ::: "memory");
-  }
-  if constexpr (Geo::DEF) {                    // the all-zero FP16 row the deferred rows' records point at
-    for (uint32_t i = tid * 4; i < (uint32_t)Geo::Q_ROW; i += (NW + NP) * 32 * 4) *reinterpret_cast<uint32_t*>(smem_raw + Q0 + i) = 0u;
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
@@ -391,8 +392,9 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
     // ================================================================ producers: TMA + hash stage (a1, a2)
     const uint32_t pw = warp - NW;                 // producer warp pw: 32-row chunks cp, cp + NPC, ...; stack blocks [j0, j0 + JB)
     const uint32_t cp = pw % NPC, j0 = (pw / NPC) * JB, b0 = j0 / ZB;
-    unsigned char* const scr = smem_raw + Q0 + Geo::Q_ROW + pw * (JB * 128);   // deferral: [JB][32] sketch rows
-    static_assert(!Geo::DEF || NP * JB * 128 <= 2048, "producer scratch");
+    unsigned char* const scr = smem_raw + Q0 + 256 + pw * (JB * 128);   // deferral: [JB][32] sketch rows
+    uint32_t* const xch = reinterpret_cast<uint32_t*>(smem_raw + Q0);  // deferral: [NPC][2][NPB] row masks exchanged by the warps of a chunk phase
+    static_assert(!Geo::DEF || (NP * JB * 128 <= 2048 && NP * 2 * 4 <= 256), "producer scratch");
     const uint64_t policy = l2_evict_first_policy();
     const bool contiguous = (a.lda == N);          // implies a single column slice
     // a2: TMA copy of this CTA's k-th stage (producer warp 0).  Waits until the consumers have released the slot;
@@ -443,9 +445,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
         else mbar_wait(empty, ph ^ 1);
       }
       // a1: rows lane, lane + 32, ... of the stage
-      uint32_t cnt[BQ];                        // deferral: side-list lengths (warp-uniform)
-#pragma unroll
-      for (int b = 0; b < BQ; ++b) cnt[b] = 0;
+      uint32_t cnt = 0;                        // deferral: rows deferred so far in this chunk phase (warp-uniform)
 #pragma unroll
       for (int rr = (int)cp; rr < (T + 31) / 32; rr += NPC) {
         const int32_t r = rr * 32 + (int32_t)lane;
@@ -501,6 +501,17 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
             if ((eq >> (pg + 1)) != 0u) ls |= 1u << j;
           }
           if (!live) ls = 0;
+          // the row is deferred as a whole when any block clashes: OR over the NPB warps that share this chunk (they walk
+          // the chunks in lockstep; masks through shared memory, one named barrier per chunk phase)
+          uint32_t dmask = __ballot_sync(0xFFFFFFFFu, ls != 0u);
+          if constexpr (NPB > 1) {
+            const uint32_t par = ((uint32_t)rr / NPC) & 1u;          // double-buffered: the next chunk's store cannot overtake a partner's read
+            if (lane == 0) xch[(cp * 2 + par) * NPB + pw / NPC] = dmask;
+            asm volatile("bar.sync %0, %1;" ::"r"(3 + cp), "n"(NPB * 32) : "memory");
+#pragma unroll
+            for (int k = 0; k < NPB; ++k) dmask |= xch[(cp * 2 + par) * NPB + k];
+          }
+          const bool def = (dmask >> lane) & 1u;
           uint32_t fb[JB];                     // sketch row the main loop touches
 #pragma unroll
           for (int j = 0; j < JB; ++j) fb[j] = bk[j];
@@ -521,9 +532,12 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
             }
           }
 #pragma unroll
+          // side-buffer slot of a deferred row = its position among the deferred rows of this chunk phase (the same in
+          // every bucket group's list)
+          const uint32_t pos = cnt + __popc(dmask & ((1u << lane) - 1u));
+#pragma unroll
           for (int bb = 0; bb < BQ / NPB; ++bb) {  // my bucket groups b0 + bb
             const uint32_t b = b0 + bb;
-            const bool def = ((ls >> (bb * ZB)) & ((1u << ZB) - 1u)) != 0u;
             uint32_t cm[ZB], co[ZB], mm[ZB];
 #pragma unroll
             for (int jj = 0; jj < ZB; ++jj) {
@@ -531,17 +545,22 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
               co[jj] = abase(b) + (bk[bb * ZB + jj] - b * dloc) * X;
               mm[jj] = mulw[bb * ZB + jj];
             }
-            if (live) sts_rec<ZB>(sE + (b * (uint32_t)T + (uint32_t)r) * RB, def ? Q0 - slot * (uint32_t)Geo::STAGE_BYTES : (uint32_t)r * Geo::Q_ROW, cm, mm);
-            const uint32_t m = __ballot_sync(0xFFFFFFFFu, def);
-            if (def) sts_rec<ZB>(sL + ((cp * BQ + b) * Geo::LCAP + cnt[bb] + __popc(m & ((1u << lane) - 1u))) * RB, (uint32_t)r, co, mm);
-            cnt[bb] += __popc(m);
+            if (live) {
+              const uint32_t pr = sE + (b * (uint32_t)T + (uint32_t)r) * Geo::REC;
+              if constexpr (ZB == 1) asm volatile("st.shared.v2.b32 [%0], {%1,%2};" ::"r"(pr), "r"(cm[0]), "r"(mm[0]) : "memory");
+              else {
+#pragma unroll
+                for (int k = 0; k < ZB / 2; ++k)
+                  asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(pr + 16 * k), "r"(cm[2 * k]), "r"(mm[2 * k]), "r"(cm[2 * k + 1]), "r"(mm[2 * k + 1]) : "memory");
+              }
+            }
+            if (def) sts_rec<ZB>(sL + ((cp * BQ + b) * Geo::LCAP + pos) * RB, (uint32_t)r | ((cp * (uint32_t)Geo::LCAP + pos) << 16), co, mm);
           }
+          cnt += __popc(dmask);
         }
       }
       if constexpr (Geo::DEF) {
-#pragma unroll
-        for (int bb = 0; bb < BQ / NPB; ++bb)
-          if (lane == bb) asm volatile("st.shared.b32 [%0], %1;" ::"r"(sL + NPC * BQ * Geo::LCAP * RB + (cp * BQ + b0 + bb) * 4), "r"(cnt[bb]) : "memory");
+        if (lane < BQ / NPB) asm volatile("st.shared.b32 [%0], %1;" ::"r"(sL + NPC * BQ * Geo::LCAP * RB + (cp * BQ + b0 + lane) * 4), "r"(cnt) : "memory");
       }
       if constexpr (Geo::PCONV) {
         // a3, a4 once per element, in place: FP16 word pair k of the tile lands on bytes [8k, 8k + 8), i.e. on FP32 data
@@ -565,6 +584,23 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
           for (int i = 0; i < CB; ++i)
             qt[(uint32_t)(i0 + i) * P + ptid] = make_uint2(pack_rn(t[i].x * scale, t[i].y * scale), pack_rn(t[i].z * scale, t[i].w * scale));
         }
+        // deferred rows (a few per thousand): FP16 words -> side buffer (upper half of the tile), tile row <- 0.  The warps
+        // that hold the first bucket groups of a chunk phase move the rows of that phase, once every warp's stores are in.
+        if constexpr (NP > 1) asm volatile("bar.sync 2, %0;" ::"n"(P) : "memory");
+        else __syncwarp();
+        if (pw < NPC && cnt != 0u) {
+          unsigned char* const q0 = smem_raw + slot * Geo::STAGE_BYTES;
+          unsigned char* const sq = q0 + T * Geo::Q_ROW;
+          const unsigned char* const items = smem_raw + slot * Geo::STAGE_BYTES + Geo::A_BYTES + Geo::E_BYTES + (cp * BQ + b0) * Geo::LCAP * RB;
+          for (uint32_t i = 0; i < cnt; ++i) {
+            const uint32_t head = *reinterpret_cast<const uint32_t*>(items + i * RB);
+            const uint32_t row = head & 0xFFFFu, sl = head >> 16;
+            for (uint32_t o = lane * 4; o < (uint32_t)Geo::Q_ROW; o += 128) {
+              *reinterpret_cast<uint32_t*>(sq + sl * Geo::Q_ROW + o) = *reinterpret_cast<const uint32_t*>(q0 + row * Geo::Q_ROW + o);
+              *reinterpret_cast<uint32_t*>(q0 + row * Geo::Q_ROW + o) = 0u;
+            }
+          }
+        }
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(full);
@@ -585,7 +621,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
     // per-contribution conversion (SR / dither): counter of this lane's first column pair (R14: (row zeta + j) ceil(n/2) + pair)
     [[maybe_unused]] const uint64_t npairs = ((uint64_t)a.n + 1u) >> 1;
     [[maybe_unused]] const uint64_t pair0 = ((uint64_t)col0 + slice * 64 * X + lane * 2 * X) >> 1;
-    const uint32_t e_off = Geo::DEF ? (bgrp * T + rowset * TR) * RB : (rowset * TR) * (ZETA * 8) + bgrp * (ZB * 8);
+    const uint32_t e_off = Geo::DEF ? (bgrp * T + rowset * TR) * Geo::REC : (rowset * TR) * (ZETA * 8) + bgrp * (ZB * 8);
     uint32_t it = 0;
     for (int64_t st = blockIdx.x; st < nstages; st += gridDim.x, ++it) {
       const uint32_t slot = it % NS, ph = (it / NS) & 1;
@@ -618,25 +654,38 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
         // software pipeline over the groups of the stage: records two groups ahead, FP16 words one group ahead of the
         // read-modify-write that uses them (their shared-memory latency hides under the tensor-memory round trip)
         constexpr int NG = TR / G;
-        uint32_t qo[2][G], col[3][G][ZB], mul[3][G][ZB], q[2][G][1][X];
+        uint32_t col[3][G][ZB], mul[3][G][ZB], q[2][G][1][X];
+        // records of a group of G rows: {col, mul} x ZB per row, rows side by side (ZB = 1: two rows per 16-byte load)
+        auto lds_group = [&](int gi, uint32_t (&c)[G][ZB], uint32_t (&m)[G][ZB]) {
+          const unsigned char* pg = sE + gi * G * Geo::REC;
+          if constexpr (ZB == 1) {
 #pragma unroll
-        for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + r * RB, qo[0][r], col[0][r], mul[0][r]);
-        if constexpr (NG > 1) {
+            for (int r = 0; r < G; r += 2) {
+              const uint4 t = *reinterpret_cast<const uint4*>(pg + r * 8);
+              c[r][0] = t.x; m[r][0] = t.y; c[r + 1][0] = t.z; m[r + 1][0] = t.w;
+            }
+          } else {
 #pragma unroll
-          for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + (G + r) * RB, qo[1][r], col[1][r], mul[1][r]);
-        }
+            for (int r = 0; r < G; ++r)
 #pragma unroll
-        for (int r = 0; r < G; ++r) lds_q<X>(qlane + qo[0][r], q[0][r][0]);
+              for (int k = 0; k < ZB / 2; ++k) {
+                const uint4 t = *reinterpret_cast<const uint4*>(pg + r * Geo::REC + 16 * k);
+                c[r][2 * k] = t.x; m[r][2 * k] = t.y; c[r][2 * k + 1] = t.z; m[r][2 * k + 1] = t.w;
+              }
+          }
+        };
+        const unsigned char* const qrow = qlane + (rowset * TR) * Geo::Q_ROW;
+        lds_group(0, col[0], mul[0]);
+        if constexpr (NG > 1) lds_group(1, col[1], mul[1]);
+#pragma unroll
+        for (int r = 0; r < G; ++r) lds_q<X>(qrow + r * Geo::Q_ROW, q[0][r][0]);
 #pragma unroll
         for (int gi = 0; gi < NG; ++gi) {
           if (gi + 1 < NG) {
 #pragma unroll
-            for (int r = 0; r < G; ++r) lds_q<X>(qlane + qo[(gi + 1) & 1][r], q[(gi + 1) & 1][r][0]);
+            for (int r = 0; r < G; ++r) lds_q<X>(qrow + ((gi + 1) * G + r) * Geo::Q_ROW, q[(gi + 1) & 1][r][0]);
           }
-          if (gi + 2 < NG) {
-#pragma unroll
-            for (int r = 0; r < G; ++r) lds_rec<ZB>(sE + ((gi + 2) * G + r) * RB, qo[gi & 1][r], col[(gi + 2) % 3][r], mul[(gi + 2) % 3][r]);
-          }
+          if (gi + 2 < NG) lds_group(gi + 2, col[(gi + 2) % 3], mul[(gi + 2) % 3]);
           // a5: read-modify-write of G x ZB sketch rows in tensor memory, pairwise distinct by construction
           tmem_rmw<G, ZB, X, false>(Geo::ABS ? 0u : region, q[gi & 1], col[gi % 3], mul[gi % 3]);
         }
@@ -710,10 +759,10 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
           const uint32_t cnt = *reinterpret_cast<const uint32_t*>(sL + NPC * BQ * Geo::LCAP * RB + (pl * BQ + bgrp) * 4);
 #pragma unroll 1
           for (uint32_t i = 0; i < cnt; ++i) {
-            uint32_t row, q1[1][1][X], c1[1][ZB], m1[1][ZB];
-            lds_rec<ZB>(sL + ((pl * BQ + bgrp) * Geo::LCAP + i) * RB, row, c1[0], m1[0]);
-            if (row / TR != rowset) continue;
-            lds_q<X>(qlane + row * Geo::Q_ROW, q1[0][0]);
+            uint32_t head, q1[1][1][X], c1[1][ZB], m1[1][ZB];
+            lds_rec<ZB>(sL + ((pl * BQ + bgrp) * Geo::LCAP + i) * RB, head, c1[0], m1[0]);
+            if ((head & 0xFFFFu) / TR != rowset) continue;
+            lds_q<X>(qlane + (T + (head >> 16)) * Geo::Q_ROW, q1[0][0]);   // the row's FP16 words, from the side buffer
             tmem_rmw<1, ZB, X, false>(Geo::ABS ? 0u : region, q1, c1, m1);
           }
         }
