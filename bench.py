@@ -251,7 +251,8 @@ def run_ours(args):
     uses_packed = plan16["hash_mode"] == 2
 
     def apply16():
-        sk.apply_f16acc(A, out=out16, variant=vid, row_begin=row_begin, rows=m, replicas=args.replicas, hash_mode=args.hash_mode)
+        sk.apply_f16acc(A, out=out16, variant=vid, row_begin=row_begin, rows=m, replicas=args.replicas, hash_mode=args.hash_mode,
+                        tmem_group_mode=args.tmem_group_mode)
         if dist is not None:
             all_reduce_sketch(out16, dist)
 
@@ -713,6 +714,7 @@ def main():
     ap.add_argument("--variant", default="auto", choices=sorted(VARIANTS))
     ap.add_argument("--replicas", type=int, default=0)
     ap.add_argument("--hash-mode", type=int, default=0)
+    ap.add_argument("--tmem-group-mode", type=int, default=0, help="sketch_opts_t.tmem_group_mode (tuning: 0 = auto)")
     ap.add_argument("--study", default=None, choices=["range", "ls", "grid", "graph"],
                     help="extra reports: config-5 range / rounding study; GPU sketch-and-solve least squares; the paper's timing "
                          "grid (PAPER.md:318-322); launch-bound config 1 replayed from a CUDA graph")

@@ -197,10 +197,12 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, int o
     // (64-feature column slices cut into bucket groups of several blocks -- d = 640 at n = 320 -- measured 2.69 TB/s
     // against 2.80 TB/s of the flat REDs; with one block per warp they get 128-row stages and win: d = 2048 at n = 256
     // 2.99 vs 2.74 TB/s; without bucket groups -- d = 384 at n = 192 -- the same slices run at 4.65 TB/s)
-    // (the FP32 path privatised in tensor memory beats its flat REDs wherever it fits: 1.4 TB/s is the L2-atomic ceiling
-    // of an FP32 zeta = 4 scatter)
+    // (the FP32 path privatised in tensor memory beats its flat REDs -- 1.4 TB/s is the L2-atomic ceiling of an FP32
+    // zeta = 4 scatter -- with up to two bucket groups: c5 3.4 vs 12.1 ms, c4-512 2.3 vs 6.0 ms; with four, every warp
+    // converts the whole FP32 tile for itself and the kernel loses: c4 7.0, n = 1024 / d = 1024 7.2 vs 6.0 ms flat)
     // (at zeta = 8 the flat REDs carry twice the payload: n = 1024, d = 2048 runs 4.68 ms in tensor memory against 6.04 ms flat)
-    if (tm_ok && (!f16 || s->zeta > 4 || !(tm.X * tm.S == 1 && tm.BQ > 1 && tm.BQ != s->zeta)) && rows * (int64_t)n > (1 << 20)) v = SKETCH_VARIANT_TMEM;
+    if (tm_ok && (f16 ? (s->zeta > 4 || !(tm.X * tm.S == 1 && tm.BQ > 1 && tm.BQ != s->zeta)) : tm.BQ <= 2) && rows * (int64_t)n > (1 << 20))
+      v = SKETCH_VARIANT_TMEM;
     else if (sm_ok && s->zeta >= 2) v = SKETCH_VARIANT_SMEM;
     // launch-bound inputs into a sketch of a few KiB: the flat REDs queue ~1000 deep on each L2 sector (c1: 10 us);
     // per-warp shared-memory partials need no such queue
