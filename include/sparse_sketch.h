@@ -81,7 +81,9 @@ typedef struct sketch sketch_t; /* opaque, library-owned */
 typedef struct sketch_opts {
   int32_t variant;    /* SKETCH_VARIANT_* */
   int32_t replicas;   /* FLAT variants: number P of L2-resident partial sketches the CTAs are spread over,
-                         summed by a reduce kernel (0 = auto, 1 = RED straight into B) */
+                         summed by a reduce kernel (0 = auto: as many as 16 MiB of scratch and 1/8 of A's bytes hold, at
+                         most 256 -- a two-level sum, which is what keeps a flat FP16 scatter accurate; 1 = RED straight
+                         into B) */
   int32_t hash_mode;  /* 0 = auto, 1 = hash on the fly inside the scatter kernel, 2 = read the packed array
                          built by sketch_precompute_hashes (built on demand) */
   int32_t accumulate; /* 0 = complete sketch: B is zero-initialised by the call;
@@ -180,6 +182,10 @@ int sketch_apply_f16acc_host(const sketch_t* s, const float* A_host, int32_t n, 
  * result-discarding REDs with the scatter kernels' address pattern (a random bucket row per lane group,
  * consecutive lanes on consecutive columns of a d x n sketch) from register values, with no A loads.
  * kind: 0 = f16x2 (4 B), 1 = v2.f16x2 (8 B), 2 = v4.f16x2 (16 B), 3 = f32 (4 B), 4 = v2.f32, 5 = v4.f32.
+ * Candidates for sketches beyond tensor memory, same pattern: 6 = plain (non-atomic) L2 read-modify-write of 16 bytes
+ * per lane (ld.global.cg / HADD2 / st.global.cg; hazards ignored: an upper bound); 7 / 8 = TMA bulk reduction
+ * (cp.reduce.async.bulk ... add.noftz.f16 / add.f32) of min(row, 2 KiB) bytes from shared memory per warp and round,
+ * counted in 16-byte units (n * elem % 16 == 0 required).
  * sketch_dev: scratch of replicas*d*n*elem bytes.  Asynchronous on `stream`; time it with CUDA events.
  * *red_ops_out (host, may be NULL) receives the number of lane-level RED operations issued. */
 int sketch_red_probe(void* sketch_dev, int32_t d, int32_t n, int32_t kind, int32_t replicas,

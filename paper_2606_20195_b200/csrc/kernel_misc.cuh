@@ -101,6 +101,63 @@ __global__ void __launch_bounds__(kFlatThreads) k_red_probe(void* sketch, int32_
   }
 }
 
+// Candidates for sketches beyond tensor memory, same address pattern, no A loads:
+//   KIND 6  owner-exclusive plain read-modify-write in L2: ld.global.cg.v4 -> 4 x HADD2 -> st.global.cg.v4 (16 bytes per
+//           lane; hazards between lanes ignored -- an upper bound for any non-atomic L2-resident replica design)
+//   KIND 7/8  TMA bulk reduction: one elected lane per warp issues cp.reduce.async.bulk.global.shared::cta ... add of a
+//           whole converted row slice (`chunk` bytes of FP16 / FP32 words from shared memory) onto a random sketch row;
+//           no per-lane RED instructions at all, so whatever limits it is the L2 side alone
+template <int KIND>
+__global__ void __launch_bounds__(kFlatThreads) k_l2_probe(void* sketch, int32_t d, int32_t n, int32_t replicas, int32_t iters, int32_t chunk) {
+  constexpr int EB = KIND == 8 ? 4 : 2;
+  char* base = reinterpret_cast<char*>(sketch) + (size_t)(blockIdx.x % replicas) * (size_t)d * n * EB;
+  if constexpr (KIND == 6) {
+    const uint32_t cpr = (uint32_t)n / 8;
+    const uint64_t gtid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint64_t gthreads = (uint64_t)gridDim.x * blockDim.x;
+    const uint32_t ch = (uint32_t)(gtid % cpr);
+    const uint64_t grp = gtid / cpr, ngrp = (gthreads + cpr - 1) / cpr;
+    for (int32_t it = 0; it < iters; ++it) {
+      uint64_t h = splitmix64(grp + (uint64_t)it * ngrp);
+      uint32_t bucket = __umulhi((uint32_t)(h >> 32), (uint32_t)d);
+      uint4* p = reinterpret_cast<uint4*>(base + ((size_t)bucket * n + (size_t)ch * 8) * 2);
+      const uint32_t hv = (h & 1) ? 0x3C003C00u : 0xBC00BC00u;
+      uint4 v;
+      asm volatile("ld.global.cg.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+      asm("add.rn.f16x2 %0, %0, %1;" : "+r"(v.x) : "r"(hv));
+      asm("add.rn.f16x2 %0, %0, %1;" : "+r"(v.y) : "r"(hv));
+      asm("add.rn.f16x2 %0, %0, %1;" : "+r"(v.z) : "r"(hv));
+      asm("add.rn.f16x2 %0, %0, %1;" : "+r"(v.w) : "r"(hv));
+      asm volatile("st.global.cg.v4.b32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+    }
+  } else {
+    extern __shared__ __align__(128) unsigned char probe_smem[];   // [2][chunk]: a row slice of +1 and one of -1
+    const uint32_t words = (uint32_t)chunk / 4;
+    for (uint32_t k = threadIdx.x; k < 2 * words; k += blockDim.x)
+      reinterpret_cast<uint32_t*>(probe_smem)[k] = KIND == 7 ? (k < words ? 0x3C003C00u : 0xBC00BC00u) : (k < words ? 0x3F800000u : 0xBF800000u);
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+    const uint32_t src = (uint32_t)__cvta_generic_to_shared(probe_smem);
+    const uint32_t per_row = (uint32_t)n * EB / (uint32_t)chunk;          // chunks per sketch row
+    const uint64_t gw = ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((uint64_t)gridDim.x * blockDim.x) >> 5;
+    if ((threadIdx.x & 31) == 0) {
+      for (int32_t it = 0; it < iters; ++it) {
+        uint64_t h = splitmix64(gw + (uint64_t)it * nw);
+        uint32_t bucket = __umulhi((uint32_t)(h >> 32), (uint32_t)d);
+        char* dst = base + (size_t)bucket * n * EB + (size_t)((uint32_t)(h >> 8) % per_row) * chunk;
+        const uint32_t s = src + ((h & 1) ? (uint32_t)chunk : 0u);
+        if constexpr (KIND == 7)
+          asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.noftz.f16 [%0], [%1], %2;" ::"l"(dst), "r"(s), "r"(chunk) : "memory");
+        else
+          asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;" ::"l"(dst), "r"(s), "r"(chunk) : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        if ((it & 7) == 7) asm volatile("cp.async.bulk.wait_group.read 8;" ::: "memory");
+      }
+      asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
 // a4 in isolation (tests; SURVEY 8c row 14 "the hardware cvt.rs.f16x2.f32 may be used only if shown bit-identical"):
 // out[k] = the 16-bit conversion of p[k] under `kind` with the random bits r[k].

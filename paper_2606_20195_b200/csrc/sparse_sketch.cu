@@ -201,7 +201,12 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, int o
     // zeta = 4 scatter -- with up to two bucket groups: c5 3.4 vs 12.1 ms, c4-512 2.3 vs 6.0 ms; with four, every warp
     // converts the whole FP32 tile for itself and the kernel loses: c4 7.0, n = 1024 / d = 1024 7.2 vs 6.0 ms flat)
     // (at zeta = 8 the flat REDs carry twice the payload: n = 1024, d = 2048 runs 4.68 ms in tensor memory against 6.04 ms flat)
-    if (tm_ok && (f16 ? (s->zeta > 4 || !(tm.X * tm.S == 1 && tm.BQ > 1 && tm.BQ != s->zeta)) : tm.BQ <= 2) && rows * (int64_t)n > (1 << 20))
+    // (per-contribution conversion -- SR, dither -- is integer-ALU work: 2^33 counter hashes and conversions at c5.  The flat
+    // kernel spreads it over 64 warps per SM and runs 29 ms (SR) / 22 ms (dither); the tensor-memory kernel has four consumer
+    // warps per SM and takes 218 / 92 ms (profiles/r02_sr_dither.md).  AUTO therefore keeps SR and dither on the flat REDs
+    // and gets the accuracy of a two-level sum from many L2-resident partial sketches instead, see the replica rule below)
+    const bool perj = out == sk::OUT_F16 && rounding != SKETCH_RN;
+    if (tm_ok && !perj && (f16 ? (s->zeta > 4 || !(tm.X * tm.S == 1 && tm.BQ > 1 && tm.BQ != s->zeta)) : tm.BQ <= 2) && rows * (int64_t)n > (1 << 20))
       v = SKETCH_VARIANT_TMEM;
     else if (sm_ok && s->zeta >= 2) v = SKETCH_VARIANT_SMEM;
     // launch-bound inputs into a sketch of a few KiB: the flat REDs queue ~1000 deep on each L2 sector (c1: 10 us);
@@ -296,11 +301,16 @@ int make_plan(sketch* s, int n, int64_t lda, const void* A, const void* B, int o
   }
   int P = (o && o->replicas > 0) ? o->replicas : 0;
   if (P == 0) {
-    // auto: enough partial sketches to spread same-line RED traffic over L2, capped at 16 MiB of scratch;
+    // auto: as many L2-resident partial sketches as 16 MiB of scratch hold, at most 256.  Eight spread the same-line RED
+    // traffic over L2; more cost nothing (c5 FP16-RN: 6.93 ms with 8, 6.06 ms with 128 - 256) and shorten every running sum
+    // -- each partial sums 1/P of the contributions, the fold adds P partials -- which is what keeps a flat FP16 scatter
+    // inside the north star's 5e-2 (c5: relF 3.8e-2 with 8 partials, 7e-3 with 256; profiles/r02_sr_dither.md);
     // launch-bound inputs (c1: 12.3 us with P = 1 vs 13.6 us with the fold kernel) RED straight into B
     size_t one = (size_t)s->d * n * (f16 ? 2 : 4);
     size_t cap = (16u << 20) / (one ? one : 1);
-    P = (int)(cap < 1 ? 1 : cap > 8 ? 8 : cap);
+    const size_t by_input = (size_t)(rows * (int64_t)n * 4 / 8) / (one ? one : 1);   // zeroing + folding them stays under 1/8 of A's bytes
+    if (cap > by_input) cap = by_input;
+    P = (int)(cap < 1 ? 1 : cap > 256 ? 256 : cap);
     if (rows * (int64_t)n <= (1 << 20)) P = 1;
   }
   if (P > 4096) P = 4096;
@@ -863,19 +873,34 @@ int sketch_apply_f16acc_host(const sketch_t* s, const float* A_host, int32_t n, 
 int sketch_red_probe(void* sketch_dev, int32_t d, int32_t n, int32_t kind, int32_t replicas, int32_t grid_ctas,
                      int32_t iters, uint64_t* red_ops_out, void* stream) {
   if (!sketch_dev) return SKETCH_ERR_NULL;
-  if (d <= 0 || n <= 0 || kind < 0 || kind > 5 || replicas < 1 || grid_ctas < 1 || iters < 0) return SKETCH_ERR_INVALID;
-  const int vec[6] = {2, 4, 8, 1, 2, 4};
+  if (d <= 0 || n <= 0 || kind < 0 || kind > 8 || replicas < 1 || grid_ctas < 1 || iters < 0) return SKETCH_ERR_INVALID;
+  const int vec[9] = {2, 4, 8, 1, 2, 4, 8, 8, 4};
   if (n % vec[kind] != 0) return SKETCH_ERR_INVALID;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
-  switch (kind) {
-    case 0: sk::k_red_probe<0><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
-    case 1: sk::k_red_probe<1><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
-    case 2: sk::k_red_probe<2><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
-    case 3: sk::k_red_probe<3><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
-    case 4: sk::k_red_probe<4><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
-    default: sk::k_red_probe<5><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
+  uint64_t ops = (uint64_t)grid_ctas * sk::kFlatThreads * (uint64_t)iters;
+  if (kind >= 7) {
+    // one bulk reduction per warp and iteration of min(row, 2 KiB) bytes; counted in 16-byte units so that payload = ops * 16
+    const int eb = kind == 8 ? 4 : 2;
+    int64_t row = (int64_t)n * eb;
+    if (row % 16 != 0) return SKETCH_ERR_INVALID;
+    int32_t chunk = (int32_t)(row < 2048 ? row : 2048);
+    if (row % chunk != 0) return SKETCH_ERR_INVALID;
+    if (kind == 7) sk::k_l2_probe<7><<<grid_ctas, sk::kFlatThreads, 2 * chunk, st>>>(sketch_dev, d, n, replicas, iters, chunk);
+    else sk::k_l2_probe<8><<<grid_ctas, sk::kFlatThreads, 2 * chunk, st>>>(sketch_dev, d, n, replicas, iters, chunk);
+    ops = (uint64_t)grid_ctas * (sk::kFlatThreads / 32) * (uint64_t)iters * (uint64_t)(chunk / 16);
+  } else if (kind == 6) {
+    sk::k_l2_probe<6><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters, 0);
+  } else {
+    switch (kind) {
+      case 0: sk::k_red_probe<0><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
+      case 1: sk::k_red_probe<1><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
+      case 2: sk::k_red_probe<2><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
+      case 3: sk::k_red_probe<3><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
+      case 4: sk::k_red_probe<4><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
+      default: sk::k_red_probe<5><<<grid_ctas, sk::kFlatThreads, 0, st>>>(sketch_dev, d, n, replicas, iters); break;
+    }
   }
-  if (red_ops_out) *red_ops_out = (uint64_t)grid_ctas * sk::kFlatThreads * (uint64_t)iters;
+  if (red_ops_out) *red_ops_out = ops;
   return launch_check("k_red_probe");
 }
 

@@ -11,8 +11,10 @@ from __future__ import annotations
 import argparse
 import json
 
-KINDS = [(0, "f16x2", 2, 2), (1, "v2.f16x2", 4, 2), (2, "v4.f16x2", 8, 2), (3, "f32", 1, 4), (4, "v2.f32", 2, 4), (5, "v4.f32", 4, 4)]
-SHAPES = [("c2", 128, 64), ("c3/c5", 256, 128), ("c4", 1024, 256)]
+KINDS = [(0, "f16x2", 2, 2), (1, "v2.f16x2", 4, 2), (2, "v4.f16x2", 8, 2), (3, "f32", 1, 4), (4, "v2.f32", 2, 4), (5, "v4.f32", 4, 4),
+         # candidates for sketches beyond tensor memory: plain L2 read-modify-write, TMA bulk reductions
+         (6, "plain ld.cg/HADD2/st.cg 16 B", 8, 2), (7, "bulk-reduce f16", 8, 2), (8, "bulk-reduce f32", 4, 4)]
+SHAPES = [("c2", 128, 64), ("c3/c5", 256, 128), ("c4", 1024, 256), ("e1", 2048, 1024), ("e1-d4096", 4096, 1024), ("grid d/n=32", 32768, 1024)]
 
 
 def main() -> int:
@@ -32,6 +34,8 @@ def main() -> int:
     for name, d, n in SHAPES:
         for kind, kname, vec, eb in KINDS:
             for P in (1, 8, 64):
+                if P * d * n * eb > (1 << 30):
+                    continue
                 buf = torch.zeros(P * d * n * eb, dtype=torch.uint8, device=dev)
                 ss.sketch_red_probe(buf, d, n, kind, P, grid, 200)          # warm-up
                 torch.cuda.synchronize()
