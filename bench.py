@@ -645,6 +645,48 @@ def run_grid_study(args):
     return 0
 
 
+def run_coherence_study(args):
+    """The paper's geometry sweep (Sec. V-C, Fig. 5) with direct sketching of U: U(theta) =
+    orth((1 - theta) Q_rand + theta [I_n 0]^T), eleven theta values, m = 2^20, n = 1024, d/n in {2, 4, 8, 16}, zeta = 4 (plus
+    zeta in {1, 2, 8} at d = 2n for the rank statement of PAPER.md:352).  Per point: coherence (Eq. 2), distortion (Eq. 4) of
+    the FP16 and FP32 sketches = max |sigma_i(S U) - 1| from an FP64 SVD of the returned d x n matrix, their difference, the
+    smallest singular value (rank).  One JSON line; not the driver's bench line."""
+    import torch
+
+    import paper_2606_20195_b200 as ss
+    import workloads as wl
+
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    quick = args.grid == "quick"
+    m, n = (1 << 18, 256) if quick else (1 << 20, 1024)
+    thetas = [0.0, 0.5, 1.0] if quick else [k / 10.0 for k in range(11)]
+    cases = [(r, 4) for r in (2, 4, 8, 16)] + [(2, z) for z in (1, 2, 8)]
+    sks = {(r, z): ss.Sketch(m, r * n, z, wl.sketch_seed(0)) for r, z in cases}
+
+    def eta(SU):
+        sv = torch.linalg.svdvals(SU.double())
+        return float(torch.maximum((sv.max() - 1.0).abs(), (1.0 - sv.min()).abs())), float(sv.min())
+
+    pts = []
+    for theta, U, mu in wl.coherence_basis_device(m, n, thetas, 9, dev):
+        for (r, z), sk in sks.items():
+            e16, smin16 = eta(sk.apply_f16acc(U))
+            e32, smin32 = eta(sk.apply_f32acc(U))
+            pts.append({"theta": theta, "coherence": mu, "d_over_n": r, "zeta": z, "eta_fp16": e16, "eta_fp32": e32,
+                        "abs_diff": abs(e16 - e32), "sigma_min_fp16": smin16, "sigma_min_fp32": smin32,
+                        "variant_fp16": sk.plan(n, f16=1)["variant"], "sqrt_n_over_d": (1.0 / r) ** 0.5})
+        del U
+    z4 = [p for p in pts if p["zeta"] == 4]
+    print(json.dumps({"study": "coherence sweep with direct sketching of U (SURVEY 8f NEXT-2; PAPER.md:344-352)", "m": m, "n": n,
+                      "largest_abs_diff_zeta4": max(p["abs_diff"] for p in z4),
+                      "paper_context": "H200 NVL, PAPER.md:348-352: largest individual FP16-FP32 distortion difference 0.00492, largest case-median 7.80e-4; "
+                                       "u sqrt(n) = 1/64 is Prop. 2's conversion-only scale; coordinate endpoint, d/n = 16: FP32 SparseStack distortion 0.364; "
+                                       "at d = 2n coordinate sketches keep full rank at zeta = 4, 8 and lose it at zeta = 1 (and in the zeta = 2 runs tried)",
+                      "points": pts}))
+    return 0
+
+
 def run_graph_study(args):
     """Launch-bound config 1 (256 KiB of A): the complete FP16 and FP32 sketches captured once into a CUDA graph each (the ABI
     neither synchronises nor allocates after the first call) and replayed; per-replay time from events around 200 replays."""
@@ -720,10 +762,10 @@ def main():
     ap.add_argument("--replicas", type=int, default=0)
     ap.add_argument("--hash-mode", type=int, default=0)
     ap.add_argument("--tmem-group-mode", type=int, default=0, help="sketch_opts_t.tmem_group_mode (tuning: 0 = auto)")
-    ap.add_argument("--study", default=None, choices=["range", "ls", "grid", "graph"],
+    ap.add_argument("--study", default=None, choices=["range", "ls", "grid", "graph", "coherence"],
                     help="extra reports: config-5 range / rounding study; GPU sketch-and-solve least squares; the paper's timing "
-                         "grid (PAPER.md:318-322); launch-bound config 1 replayed from a CUDA graph")
-    ap.add_argument("--grid", default="full", choices=["full", "quick"], help="--study grid: every point, or the corners")
+                         "grid (PAPER.md:318-322); launch-bound config 1 replayed from a CUDA graph; the U(theta) coherence sweep (PAPER.md:344-352)")
+    ap.add_argument("--grid", default="full", choices=["full", "quick"], help="--study grid / coherence: every point, or the corners / a small instance")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-pairs", action="store_true", help="skip the like-for-like flat/flat and tmem/tmem FP16-vs-FP32 timings")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -743,6 +785,8 @@ def main():
         return run_grid_study(args)
     if args.study == "graph":
         return run_graph_study(args)
+    if args.study == "coherence":
+        return run_coherence_study(args)
     return run_ours(args)
 
 

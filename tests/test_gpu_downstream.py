@@ -174,3 +174,33 @@ def test_coordinate_subspace_rank_countsketch_vs_sparsestack(ss):
         if zeta == 1:
             assert rank == distinct < n          # rank of a CountSketch on unit rows = number of distinct buckets hit
         assert (rank == n) == full, (zeta, rank)
+
+
+@pytest.mark.parametrize("ratio", [2, 8])
+def test_coherence_sweep_direct_sketch_of_U(ss, ratio):
+    # PAPER.md:344-352 (Sec. V-C, Fig. 5): U(theta) = orth((1 - theta) Q_rand + theta [I_n 0]^T), sketched directly;
+    # distortion (Eq. 4) = max |sigma_i(S U) - 1| of the returned matrix.  A small instance (m = 2^17, n = 256, zeta = 4) of
+    # bench.py --study coherence with the oracle beside it: GPU-FP32 within 1 % of the FP64 oracle's distortion (R19), and
+    # GPU-FP16 within 1e-2 of GPU-FP32 (the paper's largest individual difference is 0.00492 at n = 1024; Prop. 2's
+    # conversion-only scale u sqrt(n) is 1/128 here) and within Prop. 2's perturbation bound.
+    m, n, zeta = 1 << 17, 256, 4
+    d = ratio * n
+    seed = sketch_seed(300 + ratio)
+    sk = ss.Sketch(m, d, zeta, seed)
+    mus = []
+    for theta, U, mu in wl.coherence_basis_device(m, n, [0.0, 0.5, 0.9, 1.0], 11, torch.device("cuda")):
+        mus.append(mu)
+        Uh = U.cpu().numpy()
+        assert np.abs(Uh.astype(np.float64).T @ Uh.astype(np.float64) - np.eye(n)).max() < 1e-5     # orthonormal input
+        B64 = oracle.f64_sketch(seed, d, zeta, Uh, threads=THREADS)
+        D16, D32 = f16_to_f64(sk.apply_f16acc(U)), sk.apply_f32acc(U).cpu().numpy().astype(np.float64)
+        e64, e16, e32 = ev.eta_of(B64), ev.eta_of(D16), ev.eta_of(D32)
+        print("theta %.1f d/n %d: coherence %.4f, eta f64 %.5f gpu f32 %.5f gpu f16 %.5f" % (theta, ratio, mu, e64, e32, e16))
+        assert abs(e32 - e64) <= 0.01 * e64, (theta, e32, e64)
+        assert abs(e16 - e32) <= 1e-2, (theta, e16, e32)
+        for D, e in ((D16, e16), (D32, e32)):
+            assert abs(e - e64) <= np.linalg.norm(D - B64) * (1 + 1e-9) + 1e-12       # Prop. 2, Eq. (10)
+        if theta == 1.0:   # the coordinate subspace: entries 0 / 1, every sum exact in FP16 -> the sketch itself is exact
+            assert np.array_equal(D16, B64) and np.array_equal(D32, B64)
+            assert np.linalg.matrix_rank(D16) == n                                  # zeta = 4 keeps full rank
+    assert mus[0] < 0.02 and abs(mus[-1] - 1.0) < 1e-6 and all(a <= b + 1e-9 for a, b in zip(mus, mus[1:]))   # coherence rises to 1

@@ -848,3 +848,34 @@ def test_tmem_geometry_sweep(ss, m, n, d, zeta):
         assert np.array_equal(oracle.half_bits_to_f64(bits(got)), want)
     else:
         assert ev.rel_fro(oracle.half_bits_to_f64(bits(got)), want) <= 2e-3
+
+
+# bucket-group geometries under every group mode (sketch_opts_t::tmem_group_mode): chained, deferral with groups of 4 / 8
+# rows.  Small d / zeta makes rows of one group collide often, which is what the chains and the deferral lists exist for.
+@pytest.mark.parametrize("mode", [1, 2, 3])
+@pytest.mark.parametrize("m,n,d,zeta", [
+    (5003, 256, 256, 4),      # X = 4, two bucket groups of two blocks, d / zeta = 64: a clash in most groups
+    (4999, 256, 1024, 4),     # c4's geometry: X = 2, four bucket groups, two column slices
+    (6007, 256, 2048, 4),     # c4-2048's: X = 1, 128-row stages, four column slices
+    (2203, 1024, 2048, 4),    # e1's: sixteen column slices
+    (5501, 256, 512, 8),      # zeta = 8: four bucket groups of two blocks, d / zeta = 64
+    (7001, 128, 384, 4),      # d / zeta = 96: groups of 8 allowed (>= 72)
+    (3301, 512, 1024, 2),     # two bucket groups of one block
+])
+def test_tmem_group_modes(ss, m, n, d, zeta, mode):
+    seed = sketch_seed(7100 + m)
+    sk = ss.Sketch(m, d, zeta, seed)
+    try:
+        sk.plan(n, variant=VID["tmem"], tmem_group_mode=mode)
+    except ss.SketchError:
+        pytest.skip("plan: no tensor-memory geometry for n=%d d=%d zeta=%d" % (n, d, zeta))
+    exact = zeta in (1, 4)
+    A = wl.integer_valued(m, n, m) if exact else wl.gaussian(m, n, m)
+    Ad = dev(A)
+    want = oracle.f64_sketch(seed, d, zeta, A)
+    for grid in (0, 3 * 16):        # the full grid, and a few CTAs with many stages each
+        got = sk.apply_f16acc(Ad, variant=VID["tmem"], tmem_group_mode=mode, grid_ctas=grid)
+        if exact:
+            assert np.array_equal(oracle.half_bits_to_f64(bits(got)), want), (mode, grid)
+        else:
+            assert ev.rel_fro(oracle.half_bits_to_f64(bits(got)), want) <= 2e-3, (mode, grid)

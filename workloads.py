@@ -218,3 +218,27 @@ def ls_paper_coherent_device(m: int, n: int, seed: int, device):
     A[pos] = torch.eye(n, dtype=torch.float32, device=device)
     b[pos, 0] = (x0 + 0.5 * torch.randn(n, generator=g, device=device, dtype=torch.float64)).to(torch.float32)
     return A, b
+
+
+def coherence_basis_device(m: int, n: int, thetas, seed: int, device):
+    """The paper's coherence sweep (Sec. V-C): U(theta) = orth((1 - theta) Q_rand + theta [I_n 0]^T) with
+    Q_rand an orthogonalised m x n Gaussian matrix.  Yields (theta, U FP32 [m, n] on `device`, coherence of Eq. (2) =
+    max_i ||U_i||^2).  The orthogonalisations run in FP64 (library QR), so U's columns are orthonormal to FP32 rounding;
+    theta = 1 is the coordinate subspace [I_n 0]^T exactly."""
+    import torch
+
+    Q = gaussian_device(m, n, seed + 5000011, device).double()
+    Q = torch.linalg.qr(Q, mode="reduced")[0]
+    for theta in thetas:
+        theta = float(theta)
+        if theta >= 1.0:
+            U = torch.zeros((m, n), dtype=torch.float64, device=device)
+            U[:n] = torch.eye(n, dtype=torch.float64, device=device)
+        else:
+            M = Q * (1.0 - theta)
+            M[:n] += theta * torch.eye(n, dtype=torch.float64, device=device)
+            U = torch.linalg.qr(M, mode="reduced")[0] if theta > 0.0 else Q
+            del M
+        mu = float((U * U).sum(dim=1).max())
+        yield theta, U.to(torch.float32).contiguous(), mu    # library QR returns column-major factors
+        del U
