@@ -341,6 +341,23 @@ def run_ours(args):
             pairs["tmem"] = {"f16_ms": a16, "f32_ms": a32, "f16_over_f32": a32 / a16}
     ms16_apply, _, _, _ = timed(apply16, max(2, args.steps // 2), 3) if uses_packed else (ms16, None, None, None)
 
+    # step a2 alone: how fast this GPU delivers A when it is only read (sketch_stream_probe; context for roofline.frac, whose
+    # denominator is a COPY rate).  Plain 256-bit loads and k_tmem's TMA ring without consumers, median of 5 passes over A.
+    stream_probe = {}
+    if dist is None and m * n * 4 >= (1 << 28):
+        for key, kind in (("ld256", 0), ("tma_ring", 1)):
+            ts = []
+            for rep_i in range(7):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                nb = ss.sketch_stream_probe(A, kind)
+                e1.record()
+                torch.cuda.synchronize()
+                if rep_i >= 2:
+                    ts.append(e0.elapsed_time(e1))
+            ts.sort()
+            stream_probe[key + "_GBps"] = nb / (ts[len(ts) // 2] * 1e-3) / 1e9
+
     # end to end through the host-buffer entry point: pinned A on the host, H2D + kernels + D2H inside the call
     e2e = None
     if not args.no_e2e:
@@ -412,6 +429,8 @@ def run_ours(args):
                      "traffic": traffic, "traffic_source": ("committed ncu capture %s (kernel %s)" % (traffic_src["profile"], traffic_src["kernel"])) if traffic_src else None,
                      "peak_source": peak_src,
                      "frac_of_nominal_8TBps": achieved / 8000.0,
+                     "read_only_stream": dict(stream_probe, note="sketch_stream_probe over the same A in this run: what a kernel that only READS can reach; "
+                                                                 "`peak` is a copy rate (read + write)") if stream_probe else None,
                      "algorithmic_bytes_per_launch": abytes,
                      "note": "dominant kernel = the scatter; CUDA-event bracket on the launching stream = zero-init memset + scatter (+ replica fold), hash-pack excluded"},
         "f32acc": {"ms_per_step": ms32, "GBps": world * m * n * 4 / (ms32 * 1e-3) / 1e9, "variant": plan32["variant"],

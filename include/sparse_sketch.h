@@ -42,7 +42,7 @@ typedef struct sketch sketch_t; /* opaque, library-owned */
 #define SKETCH_ERR_NULL (-2)        /* a required pointer is NULL */
 #define SKETCH_ERR_DIVISIBILITY (-3)/* d % zeta != 0 ("Let d be divisible by zeta") */
 #define SKETCH_ERR_LDA (-4)         /* lda < n */
-#define SKETCH_ERR_ALIGNMENT (-5)   /* A not 4-byte, B not 2-byte (f16) / 4-byte (f32) aligned */
+#define SKETCH_ERR_ALIGNMENT (-5)   /* A or B not 4-byte aligned (the 16-bit sketches too: their REDs work on 4-byte words) */
 #define SKETCH_ERR_UNSUPPORTED (-6) /* the forced variant cannot run this shape (AUTO never returns it) */
 #define SKETCH_ERR_CUDA (-7)        /* CUDA runtime error; text via sketch_last_error() */
 #define SKETCH_ERR_NOMEM (-8)       /* host or device allocation failed */
@@ -112,9 +112,10 @@ int sketch_destroy(sketch_t* s);
  * h & 1) for all i in [0,m), j in [0,zeta) to DEVICE buffers of m*zeta elements each. */
 int sketch_hashes_dump(const sketch_t* s, int32_t* bucket_dev, uint8_t* signbit_dev, void* stream);
 
-/* Build (once) the packed per-(row,block) hash array the hash_mode=2 kernels read:
- * uint16 = bucket | signbit<<15 when d <= 32768, else uint32 = bucket | signbit<<31; m*zeta entries,
- * library-owned.  Counted in "complete sketch" time by bench.py when that mode is used. */
+/* Build (once) the packed per-(row,block) hash array the hash_mode=2 kernels read; m*zeta entries, library-owned:
+ * uint16 = bucket | reload<<14 | signbit<<15 in the sub-step order of the SMEM variant (entry (row, t) at row*zeta + t holds
+ * block (row mod R + t) mod zeta, R = min(zeta, 4)) when zeta is 1, 2, 4 or 8 and d <= 2047, else uint32 = bucket | signbit<<31
+ * at row*zeta + j.  Counted in "complete sketch" time by bench.py when that mode is used. */
 int sketch_precompute_hashes(sketch_t* s, void* stream);
 
 /* ---- scatter kernels ------------------------------------------------- */
@@ -190,6 +191,15 @@ int sketch_apply_f16acc_host(const sketch_t* s, const float* A_host, int32_t n, 
  * *red_ops_out (host, may be NULL) receives the number of lane-level RED operations issued. */
 int sketch_red_probe(void* sketch_dev, int32_t d, int32_t n, int32_t kind, int32_t replicas,
                      int32_t grid_ctas, int32_t iters, uint64_t* red_ops_out, void* stream);
+
+/* Read-only streaming probe (step a2 in isolation): reads `bytes` (multiple of 32 KiB is read in full; a tail is skipped)
+ * from src_dev once and discards them -- kind 0: 256-bit no-allocate / evict-first loads, grid-stride over grid_ctas CTAs of
+ * 256 threads; kind 1: TMA bulk copies of 32 KiB into a 4-slot shared-memory ring per CTA (k_tmem's producer with the
+ * consumers removed; use one CTA per SM).  Time it with CUDA events: bytes / time is the rate at which this GPU delivers a
+ * buffer that is read and never written, the ceiling of any complete sketch; bench.py prints it beside the COPY rate of
+ * MEASURED_PEAKS.json that roofline.frac is quoted against.  src_dev 32-byte aligned; sink_dev: 8 device bytes or NULL
+ * (never written in practice).  Asynchronous on `stream`. */
+int sketch_stream_probe(const void* src_dev, int64_t bytes, int32_t kind, int32_t grid_ctas, void* sink_dev, void* stream);
 
 /* The conversion step in isolation, for tests: out_dev[k] (16-bit pattern) = conversion of p_dev[k] under
  * kind with the random bits rbits_dev[k]:  0 = RN16;  1 = SR16, reading R13 with r24 = rbits & 0xFFFFFF

@@ -24,6 +24,7 @@ from .binding import (  # noqa: F401
     sketch_convert_probe,
     sketch_launch_count,
     sketch_red_probe,
+    sketch_stream_probe,
     sketch_strerror,
     sketch_widen,
     sketch_version,

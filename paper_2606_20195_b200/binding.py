@@ -59,6 +59,7 @@ SYMBOLS = {
     "sketch_apply_f16acc_host": (_int, [_vp, _vp, _i32, _i64, _vp, _int, _u64, _OP]),
     "sketch_red_probe": (_int, [_vp, _i32, _i32, _i32, _i32, _i32, _i32, C.POINTER(_u64), _vp]),
     "sketch_convert_probe": (_int, [_vp, _vp, _i64, _i32, _vp, _vp]),
+    "sketch_stream_probe": (_int, [_vp, _i64, _i32, _i32, _vp, _vp]),
     "sketch_plan": (_int, [_vp, _i32, _i64, _int, _int, _OP, C.POINTER(_i32), C.POINTER(_i32), C.POINTER(_i32), C.POINTER(_i32)]),
     "sketch_launch_count": (_u64, []),
     "sketch_strerror": (C.c_char_p, [_int]),
@@ -121,6 +122,22 @@ def sketch_red_probe(scratch, d: int, n: int, kind: int, replicas: int, grid_cta
     if rc:
         raise SketchError(rc, "sketch_red_probe")
     return int(ops.value)
+
+
+def sketch_stream_probe(src, kind: int = 1, grid_ctas: int = 0, stream=None) -> int:
+    """Read the CUDA tensor `src` once and discard it (sketch_stream_probe); returns the bytes read.  Time it with events."""
+    import torch
+
+    if not src.is_cuda or not src.is_contiguous():
+        raise TypeError("src must be a contiguous CUDA tensor")
+    nbytes = src.numel() * src.element_size()
+    if grid_ctas <= 0:
+        sms = torch.cuda.get_device_properties(src.device).multi_processor_count
+        grid_ctas = sms if kind == 1 else sms * 8
+    rc = lib().sketch_stream_probe(src.data_ptr(), nbytes, kind, grid_ctas, None, _stream_ptr(stream))
+    if rc:
+        raise SketchError(rc, "sketch_stream_probe")
+    return nbytes // 32768 * 32768 if kind == 1 else nbytes // 32 * 32
 
 
 def sketch_widen(B16, out=None, stream=None):

@@ -7,6 +7,7 @@
 
 #include "args.h"
 #include "device_util.cuh"
+#include "kernel_tmem.cuh"   // mbarrier / TMA wrappers for the streaming probe
 
 namespace sk {
 
@@ -154,6 +155,50 @@ __global__ void __launch_bounds__(kFlatThreads) k_l2_probe(void* sketch, int32_t
         if ((it & 7) == 7) asm volatile("cp.async.bulk.wait_group.read 8;" ::: "memory");
       }
       asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Read-only streaming probe: how fast this GPU delivers a buffer that is read once and never written -- the ceiling of
+// step a2, next to which MEASURED_PEAKS.json's COPY rate (read + write) is the contract's denominator.
+//   KIND 0  256-bit ld.global.nc.L1::no_allocate.L2::evict_first loads, grid-stride (the flat kernels' loads)
+//   KIND 1  TMA bulk copies of 32 KiB into a 4-slot shared-memory ring per CTA, one CTA per SM, completion on mbarriers,
+//           nobody reads the tiles (k_tmem's producer with the consumers removed)
+// `sink` (8 bytes, device) is written only if the XOR of everything read equals a value it cannot have by accident.
+// ------------------------------------------------------------------------------------------------
+template <int KIND>
+__global__ void __launch_bounds__(256) k_stream_probe(const float* __restrict__ src, int64_t bytes, uint64_t* sink) {
+  if constexpr (KIND == 0) {
+    const int64_t vecs = bytes / 32;
+    uint32_t acc = 0;
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < vecs; k += (int64_t)gridDim.x * blockDim.x) {
+      float v[8];
+      ld_stream<8>(src + k * 8, v);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) acc ^= __float_as_uint(v[i]);
+    }
+    if (acc == 0x7FC12345u && sink) *sink = acc;
+  } else {
+    constexpr uint32_t TILE = 32768, NS = 4;
+    extern __shared__ __align__(1024) unsigned char probe_ring[];
+    const uint32_t ring = smem_u32(probe_ring), bars = ring + NS * TILE;
+    if (threadIdx.x == 0) {
+      for (uint32_t k = 0; k < NS; ++k) mbar_init(bars + 8 * k, 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      asm volatile("fence.proxy.async;" ::: "memory");
+      const uint64_t policy = l2_evict_first_policy();
+      const int64_t tiles = bytes / TILE;
+      uint32_t it = 0;
+      for (int64_t t = blockIdx.x; t < tiles; t += gridDim.x, ++it) {
+        const uint32_t slot = it % NS;
+        if (it >= NS) mbar_wait(bars + 8 * slot, ((it / NS) - 1) & 1);   // the copy that used this slot last has landed
+        mbar_expect_tx(bars + 8 * slot, TILE);
+        bulk_g2s(ring + slot * TILE, reinterpret_cast<const unsigned char*>(src) + t * TILE, TILE, bars + 8 * slot, policy);
+        mbar_arrive(bars + 8 * slot);
+      }
+      for (uint32_t k = (it > NS ? it - NS : 0); k < it; ++k) mbar_wait(bars + 8 * (k % NS), (k / NS) & 1);
+      if (sink && probe_ring[0] == 0xA5 && probe_ring[TILE - 1] == 0x5A && bytes < 0) *sink = 1;
     }
   }
 }

@@ -904,6 +904,22 @@ int sketch_red_probe(void* sketch_dev, int32_t d, int32_t n, int32_t kind, int32
   return launch_check("k_red_probe");
 }
 
+int sketch_stream_probe(const void* src_dev, int64_t bytes, int32_t kind, int32_t grid_ctas, void* sink_dev, void* stream) {
+  if (!src_dev) return SKETCH_ERR_NULL;
+  if (bytes < 0 || kind < 0 || kind > 1 || grid_ctas < 1) return SKETCH_ERR_INVALID;
+  if (!aligned(src_dev, 32)) return SKETCH_ERR_ALIGNMENT;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  if (kind == 0) {
+    sk::k_stream_probe<0><<<grid_ctas, 256, 0, st>>>(reinterpret_cast<const float*>(src_dev), bytes, reinterpret_cast<uint64_t*>(sink_dev));
+  } else {
+    const size_t smem = 4 * 32768 + 64;
+    cudaError_t e = sk::allow_max_dynamic_smem<sk::k_stream_probe<1>>();
+    if (e != cudaSuccess) return cuda_fail(e, "cudaFuncSetAttribute(k_stream_probe)");
+    sk::k_stream_probe<1><<<grid_ctas, 32, smem, st>>>(reinterpret_cast<const float*>(src_dev), bytes, reinterpret_cast<uint64_t*>(sink_dev));
+  }
+  return launch_check("k_stream_probe");
+}
+
 int sketch_convert_probe(const float* p_dev, const uint32_t* rbits_dev, int64_t count, int32_t kind, uint16_t* out_dev, void* stream) {
   if (!p_dev || !out_dev) return SKETCH_ERR_NULL;
   if (count < 0 || kind < 0 || kind > 5) return SKETCH_ERR_INVALID;

@@ -68,6 +68,9 @@ def test_apply_rejects_bad_arguments_before_any_cuda_call():
     assert L.sketch_hashes_dump(s._h, None, fake, None) == -2
     assert L.sketch_red_probe(None, 8, 8, 0, 1, 1, 1, None, None) == -2
     assert L.sketch_red_probe(fake, 8, 8, 9, 1, 1, 1, None, None) == -1
+    assert L.sketch_stream_probe(None, 1 << 20, 0, 1, None, None) == -2
+    assert L.sketch_stream_probe(fake, 1 << 20, 2, 1, None, None) == -1
+    assert L.sketch_stream_probe(C.c_void_p(4100), 1 << 20, 0, 1, None, None) == -5
     assert ss.sketch_launch_count() == 0                                       # nothing was launched
     s.close()
 

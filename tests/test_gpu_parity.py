@@ -879,3 +879,15 @@ def test_tmem_group_modes(ss, m, n, d, zeta, mode):
             assert np.array_equal(oracle.half_bits_to_f64(bits(got)), want), (mode, grid)
         else:
             assert ev.rel_fro(oracle.half_bits_to_f64(bits(got)), want) <= 2e-3, (mode, grid)
+
+
+def test_stream_probe_reads_and_returns(ss):
+    # step a2 in isolation (sketch_stream_probe): both kinds run to completion on a buffer with a ragged tail and on an
+    # empty one, leave the data untouched, and report the bytes they read
+    x = torch.arange(3 * (1 << 20) + 100, dtype=torch.float32, device="cuda")
+    ref = x.clone()
+    assert ss.sketch_stream_probe(x, 0) == x.numel() * 4 // 32 * 32
+    assert ss.sketch_stream_probe(x, 1) == x.numel() * 4 // 32768 * 32768
+    assert ss.sketch_stream_probe(x[:4096], 1, grid_ctas=7) == 4096 * 4 // 32768 * 32768 == 0
+    torch.cuda.synchronize()
+    assert torch.equal(x, ref)
