@@ -204,9 +204,11 @@ int sketch_stream_probe(const void* src_dev, int64_t bytes, int32_t kind, int32_
 /* The conversion step in isolation, for tests: out_dev[k] (16-bit pattern) = conversion of p_dev[k] under
  * kind with the random bits rbits_dev[k]:  0 = RN16;  1 = SR16, reading R13 with r24 = rbits & 0xFFFFFF
  * (PAPER.md:203-207);  2 = dither, Eq. (6), same r24;  3 = bfloat16 RN;  4 / 5 = the hardware
- * cvt.rs.f16x2.f32 d, a, b, rbits with p in both sources: the half converted from b / from a.  The library's SR kernels
- * use rule 1, never the hardware instruction: the two agree on the FP16 normal grid under a fixed bit mapping and
- * differ below 2^-14 (tests/test_gpu_modes.py).  rbits_dev may be NULL for kinds 0 and 3.  Device pointers. */
+ * cvt.rs.f16x2.f32 d, a, b, rbits with p in both sources: the half converted from b / from a;  6 / 7 = the library's SR pair
+ * conversion with p and r24 in both halves (low / high half).  The two agree on the FP16 normal grid [2^-14, 65504) under a
+ * fixed bit mapping and differ below 2^-14 (tests/test_gpu_modes.py, R22), so the library's SR kernels use the
+ * hardware instruction exactly where both values of a pair lie on that grid and the integer rule 1 everywhere else: kinds
+ * 6 / 7 equal kind 1 bit for bit on every input.  rbits_dev may be NULL for kinds 0 and 3.  Device pointers. */
 int sketch_convert_probe(const float* p_dev, const uint32_t* rbits_dev, int64_t count, int32_t kind, uint16_t* out_dev,
                          void* stream);
 

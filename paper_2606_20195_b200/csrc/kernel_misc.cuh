@@ -208,6 +208,7 @@ __global__ void __launch_bounds__(256) k_stream_probe(const float* __restrict__ 
 // out[k] = the 16-bit conversion of p[k] under `kind` with the random bits r[k].
 //   0 RN16   1 SR16 (R13, r24 = r & 0xFFFFFF)   2 dither (R20, same r24)   3 bfloat16 RN
 //   4 / 5    hardware cvt.rs.f16x2.f32 d, a, b, rbits with p in BOTH sources: the half converted from b (low, 4) / a (high, 5)
+//   6 / 7    the library's SR pair conversion pack_sr_bits(p, p, r24 in both fields): low (6) / high (7) half
 // ------------------------------------------------------------------------------------------------
 __global__ void k_convert_probe(const float* __restrict__ p, const uint32_t* __restrict__ r, int64_t count, int kind, uint16_t* __restrict__ out) {
   int64_t stride = (int64_t)gridDim.x * blockDim.x;
@@ -220,6 +221,12 @@ __global__ void k_convert_probe(const float* __restrict__ p, const uint32_t* __r
       case 1: v = sr16_bits(x, rb & 0xFFFFFFu); break;
       case 2: v = pack_rn(dither_f32(x, rb & 0xFFFFFFu), 0.f) & 0xFFFFu; break;
       case 3: v = pack_bf16_rn(x, x) & 0xFFFFu; break;
+      case 6: case 7: {   // the library's pair conversion (fast path on the normal grid, integer rule elsewhere): r24 in both fields of R
+        const uint64_t R = ((uint64_t)(rb & 0xFFFFFFu) << 40) | ((uint64_t)(rb & 0xFFFFFFu) << 16);
+        const uint32_t d = pack_sr_bits(x, x, R);
+        v = kind == 6 ? (d & 0xFFFFu) : (d >> 16);
+        break;
+      }
       default: {
         uint32_t d;
         asm("cvt.rs.f16x2.f32 %0, %1, %2, %3;" : "=r"(d) : "f"(x), "f"(x), "r"(rb));

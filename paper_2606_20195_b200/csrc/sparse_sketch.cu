@@ -922,7 +922,7 @@ int sketch_stream_probe(const void* src_dev, int64_t bytes, int32_t kind, int32_
 
 int sketch_convert_probe(const float* p_dev, const uint32_t* rbits_dev, int64_t count, int32_t kind, uint16_t* out_dev, void* stream) {
   if (!p_dev || !out_dev) return SKETCH_ERR_NULL;
-  if (count < 0 || kind < 0 || kind > 5) return SKETCH_ERR_INVALID;
+  if (count < 0 || kind < 0 || kind > 7) return SKETCH_ERR_INVALID;
   if ((kind == 1 || kind == 2 || kind >= 4) && !rbits_dev) return SKETCH_ERR_NULL;
   if (count == 0) return SKETCH_OK;
   int64_t blocks = (count + 255) / 256;

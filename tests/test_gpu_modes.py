@@ -307,6 +307,8 @@ def test_conversion_probe_matches_the_oracle_rules(ss):
     pn, rn = p.cpu().numpy(), r.cpu().numpy().astype(np.uint32)
     assert np.array_equal(_probe(ss, p, None, 0), oracle.rn16(pn))
     assert np.array_equal(_probe(ss, p, r, 1), oracle.sr16(pn, rn))
+    assert np.array_equal(_probe(ss, p, r, 6), oracle.sr16(pn, rn))      # the library's pair conversion (hardware fast path
+    assert np.array_equal(_probe(ss, p, r, 7), oracle.sr16(pn, rn))      # on the normal grid): both halves
     assert np.array_equal(_probe(ss, p, r, 2), oracle.dither16(pn, rn))
     assert np.array_equal(_probe(ss, p, None, 3), oracle.bf16_rn(pn))
 
@@ -315,7 +317,8 @@ def test_hardware_cvt_rs_against_the_sr_rule(ss, capsys):
     """the hardware cvt.rs.f16x2.f32 may replace the integer rule R13 only if bit-identical.  2^30 samples:
     on the FP16 NORMAL grid (13 discarded bits) the instruction is rule R13 with r24's top 13 bits = the complement of 13
     bits of its 16-bit random field; below 2^-14 (more discarded bits than the field has) it is NOT -- counter-example
-    printed -- so the library keeps R13."""
+    printed -- so the library uses it exactly on that grid and keeps the integer rule elsewhere (R22); the hybrid is
+    checked against the rule on every one of the 2^30 samples."""
     g = torch.Generator(device="cuda").manual_seed(9)
     chunk, chunks = 1 << 26, 16
     found, sub_mismatch, example = None, 0, None
@@ -343,6 +346,11 @@ def test_hardware_cvt_rs_against_the_sr_rule(ss, capsys):
             found = ok
         for k in found:
             assert cands[k][0] == 0, (k, cands[k][:2])
+        # the library's pair conversion (kinds 6 / 7: cvt.rs where both values are on the normal grid, rule R13 elsewhere) must
+        # equal rule R13 (kind 1) on EVERY sample, whatever the regime
+        r24 = (bitsr & 0xFFFFFF).contiguous()
+        rule = ss.sketch_convert_probe(p, r24, 1)
+        assert bool((ss.sketch_convert_probe(p, r24, 6) == rule).all()) and bool((ss.sketch_convert_probe(p, r24, 7) == rule).all())
         normal_total += int(normal.sum())
         sub_total += int(sub.sum())
         k0 = found[0]
