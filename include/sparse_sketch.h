@@ -91,8 +91,10 @@ typedef struct sketch_opts {
   int64_t row_begin;  /* global index of the first row stored at A (rows are hashed by global index) */
   int64_t rows;       /* number of rows at A; 0 = m - row_begin */
   int32_t grid_ctas;  /* 0 = auto; tuning / tests only */
-  int32_t tmem_group_mode; /* 0 = auto; tuning / tests only, TMEM variant with bucket groups: 1 = chained groups,
-                              2 / 3 = deferral with groups of 4 / 8 rows (ignored where the geometry has no such mode) */
+  int32_t tmem_group_mode; /* 0 = auto; tuning / tests only, TMEM variant: 1 = chained groups (every geometry), 2 / 3 =
+                              deferral with groups of 4 / 8 rows (bucket-group geometries; ignored where the geometry has
+                              no such mode).  AUTO also has replicated rows for sketches a quarter of a warp's
+                              tensor-memory region or smaller */
 } sketch_opts_t;
 
 /* ---- handle ------------------------------------------------------------------------------- */

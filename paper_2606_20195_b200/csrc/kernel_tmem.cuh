@@ -162,20 +162,26 @@ __host__ __device__ constexpr int tmem_rec_bytes(int zb) { return zb == 1 ? 16 :
 //          loop.  The main loop then has pairwise distinct TMEM addresses within a group by construction -- no compares, no
 //          selects, 8 read-modify-writes in flight -- reads every row's FP16 words at a compile-time offset, and its records
 //          are bare {address, multiplier} pairs (two rows per 16-byte load with one block per warp).
+//   5      REPLICATED rows, for sketches a quarter the size of a warp's tensor-memory region or smaller (G (d / BQ) X <= 512
+//          columns; c2: d = 128, X = 1): row r of a group adds into private copy r % G of the partial sketch, so the G
+//          read-modify-writes of a block never share an address -- no compares, no selects, G = 4 in flight -- and the
+//          copies are added in registers at the flush.  Classic privatisation one level further down; chained groups
+//          spend about half of the consumer's instructions on the O(G^2) chain (c2: 161 instructions per KiB of A).
 template <int ZETA, int X, int S, int BQ, int NW, int GM, int T, int MODE = TM_F16>
 struct TmemGeom {
   static constexpr int FW = tm_fw(MODE);
-  static_assert(GM == 0 || MODE == TM_F16, "deferral modes exist for the FP16-RN path only");
+  static_assert(!(GM == 1 || GM == 2) || MODE == TM_F16, "deferral modes exist for the FP16-RN path only");
   static_assert(!tm_perj(MODE) || BQ == 1, "per-contribution conversion: one bucket group");
   static_assert(NW % 4 == 0 && NW % (S * BQ) == 0, "consumer warps: whole lane quadrants, whole slice x bucket-group sets");
   static_assert(ZETA % BQ == 0, "bucket groups are whole stack blocks");
-  static_assert(GM == 0 || BQ > 1, "deferral needs the shared FP16 tile of the bucket-group kernels");
+  static_assert(!(GM == 1 || GM == 2) || BQ > 1, "deferral needs the shared FP16 tile of the bucket-group kernels");
   static constexpr int ZB = ZETA / BQ;         // stack blocks one warp accumulates
   static constexpr int RS = NW / (S * BQ);     // row-sets per stage
   static constexpr int TR = T / RS;            // rows of a stage one warp processes
-  static constexpr bool DEF = GM != 0;
+  static constexpr bool DEF = GM == 1 || GM == 2;
+  static constexpr bool REPL = GM == 5;
   static constexpr bool ABS = S == 1;             // entries hold absolute tensor-memory addresses (see the producer)
-  static constexpr int G = GM == 1 ? 4 : GM == 2 ? 8 : (ZB >= 4 || (BQ > 1 && ZB >= 2)) ? 2 : 4;  // rows per group (LDTMs in flight = G * ZB)
+  static constexpr int G = GM == 1 ? 4 : GM == 2 ? 8 : REPL ? (ZB >= 8 ? 2 : 4) : (ZB >= 4 || (BQ > 1 && ZB >= 2)) ? 2 : 4;  // rows per group (LDTMs in flight = G * ZB)
   static_assert(TR % G == 0 && 32 % G == 0, "whole groups");
   static constexpr int N = 32 * FW * X * S;    // features of the CTA's column slice
   static constexpr int WC = kTmemCols / (NW / 4);  // tensor-memory columns of one warp's private region
@@ -211,13 +217,15 @@ struct TmemGeom {
 
 __host__ __device__ constexpr int tmem_producers(int n, int bq, int gm, int zeta) {
   const int ch = (tmem_stage_rows(n, bq, zeta) + 31) / 32;
-  const int npc = gm == 0 ? (ch >= 4 ? 4 : ch >= 2 ? 2 : 1) : (ch >= 2 ? 2 : 1);
-  const int split = gm == 0 ? zeta : bq;
+  const bool def = gm == 1 || gm == 2;
+  const int npc = !def ? (ch >= 4 ? 4 : ch >= 2 ? 2 : 1) : (ch >= 2 ? 2 : 1);
+  const int split = !def ? zeta : bq;
   return npc * (split < 4 / npc ? split : 4 / npc);
 }
 // ring of stages | barriers + TMEM base (256 B) | chained bucket-group kernels: two converted (FP16) tiles | deferral:
 // one all-zero FP16 row + 2 KiB of producer scratch (the sketch rows of a 32-row chunk, a 128-byte line per warp and block)
-constexpr size_t tmem_smem_bytes(int zeta, int n, int bq, int gm, int mode = TM_F16) {
+constexpr size_t tmem_smem_bytes(int zeta, int n, int bq, int gm_, int mode = TM_F16) {
+  const int gm = (gm_ == 1 || gm_ == 2) ? gm_ : 0;   // only the deferral modes change the layout
   const size_t t = (size_t)tmem_stage_rows(n, bq, zeta);
   const size_t rb = (size_t)tmem_rec_bytes(zeta / bq);
   const size_t e = gm ? t * bq * (8 * (size_t)(zeta / bq)) + t * bq * rb + 128 : t * zeta * 8;   // records + side lists (T rows in all) + counts
@@ -470,7 +478,9 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
           // tensor-memory address (abase) and the consumer saves an add per (row, block)
           if (live) {
             const uint32_t p = sE + r * (ZETA * 8) + j0 * 8;
-            auto ent = [&](int j) -> uint32_t { const uint32_t bg = (j0 + (uint32_t)j) / ZB; return abase(bg) + (bk[j] - bg * dloc) * X; };
+            // replicated rows: row r of a group adds into private copy r % G of the warp's partial sketch
+            const uint32_t copy = Geo::REPL ? ((uint32_t)r % (uint32_t)G) * (dloc * X) : 0u;
+            auto ent = [&](int j) -> uint32_t { const uint32_t bg = (j0 + (uint32_t)j) / ZB; return abase(bg) + (bk[j] - bg * dloc) * X + copy; };
             if constexpr (JB == 1) asm volatile("st.shared.v2.b32 [%0], {%1,%2};" ::"r"(p), "r"(ent(0)), "r"(mulw[0]) : "memory");
             else {
 #pragma unroll
@@ -612,8 +622,8 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
     // ================================================================ consumers: a3, a4, a5 in tensor memory
     const uint32_t slice = warp % S, bgrp = (warp / S) % BQ, rowset = warp / (S * BQ);
     const uint32_t region = tbase + (((warp & 3u) * 32u) << 16) + (warp >> 2) * (uint32_t)Geo::WC;
-    const uint32_t ncols = dloc * X;  // multiple of 8, <= WC (host check)
-    for (uint32_t c = 0; c < ncols; c += 8) tmem_st8_zero(region + c);   // a0 (private part)
+    const uint32_t ncols = dloc * X;  // multiple of 8, <= WC (host check); replicated rows: G copies, G * ncols <= WC
+    for (uint32_t c = 0; c < ncols * (Geo::REPL ? G : 1); c += 8) tmem_st8_zero(region + c);   // a0 (private part)
     tmem_wait_st();
 
     const float scale = a.scale;
@@ -748,7 +758,7 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
           }
         }
         // a5: read-modify-write of G x ZB sketch rows in tensor memory; same-bucket rows chained in registers
-        tmem_rmw<G, ZB, X, true, MODE>(Geo::ABS ? 0u : region, q, col, mul);
+        tmem_rmw<G, ZB, X, !Geo::REPL, MODE>(Geo::ABS ? 0u : region, q, col, mul);
       }
       }
       if constexpr (Geo::DEF) {
@@ -778,9 +788,23 @@ __global__ void __launch_bounds__((NW + tmem_producers(32 * tm_fw(MODE) * X * S,
     for (uint32_t c = 0; c < ncols; c += 8) {
       uint32_t v[8];
       tmem_ld8(region + c, v);
-      tmem_wait_ld();
+      if constexpr (Geo::REPL) {
+        // the G private copies of these sketch rows, added in the mode's own arithmetic (one more level of the hierarchy)
+        uint32_t w[G - 1][8];
 #pragma unroll
-      for (int k = 0; k < 8; ++k) tmem_tie(v[k]);
+        for (int cp = 1; cp < G; ++cp) tmem_ld8(region + cp * ncols + c, w[cp - 1]);
+        tmem_wait_ld();
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          tmem_tie(v[k]);
+#pragma unroll
+          for (int cp = 1; cp < G; ++cp) { tmem_tie(w[cp - 1][k]); v[k] = tm_fma<MODE>(w[cp - 1][k], tm_one(MODE), v[k]); }
+        }
+      } else {
+        tmem_wait_ld();
+#pragma unroll
+        for (int k = 0; k < 8; ++k) tmem_tie(v[k]);
+      }
 #pragma unroll
       for (int b = 0; b < 8 / X; ++b) {
         const size_t e_off = b_off + (size_t)(c / X + b) * a.n;

@@ -16,7 +16,7 @@ constexpr int Z = SK_TMEM_ZETA, MODE = SK_TMEM_MODE;
 template <int X, int S, int BQ, int NW, int GM>
 cudaError_t go(const TmemArgs& g, const CUtensorMap& tmap, int grid, int cs, cudaStream_t st) {
   constexpr int N = 32 * tm_fw(MODE) * X * S;
-  if constexpr (Z % BQ != 0 || (GM != 0 && MODE != TM_F16) || (tm_perj(MODE) && BQ != 1)) {
+  if constexpr (Z % BQ != 0 || ((GM == 1 || GM == 2) && MODE != TM_F16) || (tm_perj(MODE) && (BQ != 1 || GM == 5))) {
     return kNoKernel;
   } else {
     constexpr auto k = k_tmem<Z, X, S, BQ, NW, GM, MODE>;
@@ -39,10 +39,10 @@ cudaError_t by_gm(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap
 cudaError_t dispatch(const TmemArgs& g, const TmemShape& h, const CUtensorMap& tmap, int grid, cudaStream_t st) {
   if (h.NW == 4) {
     switch (h.X * 100 + h.S * 10 + h.BQ) {
-      case 111: return go<1, 1, 1, 4, 0>(g, tmap, grid, h.CS, st);
-      case 121: return go<1, 2, 1, 4, 0>(g, tmap, grid, h.CS, st);
-      case 141: return go<1, 4, 1, 4, 0>(g, tmap, grid, h.CS, st);
-      case 211: return go<2, 1, 1, 4, 0>(g, tmap, grid, h.CS, st);
+      case 111: return h.GM == 5 ? go<1, 1, 1, 4, 5>(g, tmap, grid, h.CS, st) : go<1, 1, 1, 4, 0>(g, tmap, grid, h.CS, st);
+      case 121: return h.GM == 5 ? go<1, 2, 1, 4, 5>(g, tmap, grid, h.CS, st) : go<1, 2, 1, 4, 0>(g, tmap, grid, h.CS, st);
+      case 141: return h.GM == 5 ? go<1, 4, 1, 4, 5>(g, tmap, grid, h.CS, st) : go<1, 4, 1, 4, 0>(g, tmap, grid, h.CS, st);
+      case 211: return h.GM == 5 ? go<2, 1, 1, 4, 5>(g, tmap, grid, h.CS, st) : go<2, 1, 1, 4, 0>(g, tmap, grid, h.CS, st);
       case 221: return go<2, 2, 1, 4, 0>(g, tmap, grid, h.CS, st);
       case 241: return go<2, 4, 1, 4, 0>(g, tmap, grid, h.CS, st);
       case 411: return go<4, 1, 1, 4, 0>(g, tmap, grid, h.CS, st);

@@ -42,7 +42,12 @@ bool tmem_shape(int n, int d, int zeta, int64_t lda, int gm_force, int mode, Tme
           // Only the FP16-RN path has the deferral kernels.
           const double zb = (double)zeta / bq, dbk = (double)d / zeta;
           out->GM = (mode == TM_F16 && bq == 4 && zb * 6.0 / dbk <= 0.15 && dbk >= 20) ? 1 : 0;
+          // sketches a quarter of a warp's tensor-memory region or smaller (one bucket group): replicated rows -- each row of a
+          // group adds into its own private copy, no chain (kernel_tmem.cuh GM = 5; c2: 70.7 -> 64.9 us per step)
+          // (instantiated for X = 1 and for X = 2 with one feature slice, convert-once modes: d = 2n shapes only fit it at X = S = 1)
+          if (bq == 1 && (x == 1 || (x == 2 && s == 1)) && !tm_perj(mode) && (int64_t)(zeta >= 8 ? 2 : 4) * cols <= kTmemCols / (NW / 4)) out->GM = 5;
           // tuning / tests (sketch_opts_t::tmem_group_mode): forced where the mode exists for this geometry
+          if (gm_force == 0) out->GM = 0;   // chained groups exist for every geometry and mode
           if (mode == TM_F16 && gm_force >= 0 && bq > 1 && (gm_force == 0 || (gm_force == 1 && dbk >= 20) || (gm_force == 2 && dbk >= 72))) out->GM = gm_force;
         }
       }

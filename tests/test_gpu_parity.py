@@ -891,3 +891,32 @@ def test_stream_probe_reads_and_returns(ss):
     assert ss.sketch_stream_probe(x[:4096], 1, grid_ctas=7) == 4096 * 4 // 32768 * 32768 == 0
     torch.cuda.synchronize()
     assert torch.equal(x, ref)
+
+
+# small sketches (a quarter of a warp's tensor-memory region or less): AUTO's replicated-rows mode -- every row of a group adds
+# into its own private copy, the copies are summed at the flush -- against the chained groups (tmem_group_mode = 1) and the oracle
+@pytest.mark.parametrize("m,n,d,zeta", [
+    (9001, 64, 128, 4),       # c2's geometry: X = 1, four copies of a 128-row partial
+    (6011, 64, 64, 8),        # zeta = 8: two copies
+    (7013, 128, 64, 2),       # X = 2, one feature slice
+    (5003, 256, 32, 1),       # X = 1, four feature slices (column offsets relative to the warp's region)
+])
+def test_tmem_replicated_rows(ss, m, n, d, zeta):
+    seed = sketch_seed(7200 + m)
+    sk = ss.Sketch(m, d, zeta, seed)
+    exact = zeta in (1, 4)
+    A = wl.integer_valued(m, n, m) if exact else wl.gaussian(m, n, m)
+    Ad = dev(A)
+    want = oracle.f64_sketch(seed, d, zeta, A)
+    # irrational scale: the north star's rule against the sequential-FP16 oracle (L = m zeta / d is up to 750 terms here)
+    tol16 = None if exact else 1.5 * ev.rel_fro(oracle.half_bits_to_f64(oracle.seq16_sketch(seed, d, zeta, A)), want)
+    for mode in (0, 1):
+        for grid in (0, 5):
+            got16 = sk.apply_f16acc(Ad, variant=VID["tmem"], tmem_group_mode=mode, grid_ctas=grid)
+            got32 = sk.apply_f32acc(Ad, variant=VID["tmem"], tmem_group_mode=mode, grid_ctas=grid)
+            if exact:
+                assert np.array_equal(oracle.half_bits_to_f64(bits(got16)), want), (mode, grid)
+                assert np.array_equal(got32.cpu().numpy().astype(np.float64), want), (mode, grid)
+            else:
+                assert ev.rel_fro(oracle.half_bits_to_f64(bits(got16)), want) <= tol16, (mode, grid)
+                assert ev.rel_fro(got32.cpu().numpy(), want) <= 1e-5, (mode, grid)
