@@ -302,6 +302,8 @@ def run_ours(args):
 
     def timed(fn, steps, warmup):
         for _ in range(warmup):
+            if flush is not None:
+                flush.zero_()                      # warm-up steps look like timed steps (the first flush loads its own kernel)
             fn()
         barrier()
         evs = []
@@ -706,6 +708,46 @@ def run_coherence_study(args):
     return 0
 
 
+def run_replica_study(args):
+    """Conversion rule x where the partial sums live, at the workload's full size (default c5): FP16 RN / SR / dither through the
+    flat REDs with P in {8, 32, 128, 256} L2-resident partial sketches and through the tensor-memory kernel -- time per complete
+    sketch and relF against the FP64 oracle on sampled columns.  What AUTO's replica rule and its SR / dither rule rest on
+    (DESIGN.md section 5.2).  One JSON line; not the driver's bench line."""
+    import numpy as np
+    import torch
+
+    import evaluation as ev
+    import oracle
+    import paper_2606_20195_b200 as ss
+    import workloads as wl
+
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    m, n, d, zeta, mseed = WORKLOADS[args.workload]
+    seed = wl.sketch_seed(0)
+    sk = ss.Sketch(m, d, zeta, seed)
+    A = wl.gaussian_device(m, n, mseed, dev)
+    cols = sorted({0, 1, n // 2 - 1, n // 2, n - 2, n - 1})
+    oracle.build()
+    B0 = oracle.f64_sketch(seed, d, zeta, np.ascontiguousarray(A[:, cols].cpu().numpy()), threads=min(os.cpu_count() or 1, 64))
+    out = torch.empty((d, n), dtype=torch.float16, device=dev)
+    rows_out = []
+    for rname, rmode in (("RN", ss.RN), ("SR", ss.SR), ("dither", ss.DITHER)):
+        for var, P in (("flat_vec", 8), ("flat_vec", 32), ("flat_vec", 128), ("flat_vec", 256), ("tmem", 0), ("auto", 0)):
+            kw = dict(out=out, rounding=rmode, sr_seed=wl.sketch_seed(77), variant=VARIANTS[var], replicas=P)
+            try:
+                plan = sk.plan(n, rounding=rmode, variant=VARIANTS[var], replicas=P)
+            except ss.SketchError:
+                continue
+            ms = _time_ms(lambda: sk.apply_f16acc(A, **kw), reps=3, warm=1)
+            got = out[:, cols].float().cpu().numpy().astype(np.float64)
+            rows_out.append({"rounding": rname, "requested": var, "variant": plan["variant"], "replicas": plan["replicas"], "ms": ms,
+                             "GBps": m * n * 4 / ms / 1e6, "relF_vs_f64_sampled_cols": ev.rel_fro(got, B0)})
+    print(json.dumps({"study": "conversion rule x partial-sum placement", "workload": "%s: m=%d n=%d d=%d zeta=%d, N(0,1)" % (args.workload, m, n, d, zeta),
+                      "sampled_columns": cols, "rows": rows_out}))
+    return 0
+
+
 def run_graph_study(args):
     """Launch-bound config 1 (256 KiB of A): the complete FP16 and FP32 sketches captured once into a CUDA graph each (the ABI
     neither synchronises nor allocates after the first call) and replayed; per-replay time from events around 200 replays."""
@@ -781,9 +823,9 @@ def main():
     ap.add_argument("--replicas", type=int, default=0)
     ap.add_argument("--hash-mode", type=int, default=0)
     ap.add_argument("--tmem-group-mode", type=int, default=0, help="sketch_opts_t.tmem_group_mode (tuning: 0 = auto)")
-    ap.add_argument("--study", default=None, choices=["range", "ls", "grid", "graph", "coherence"],
+    ap.add_argument("--study", default=None, choices=["range", "ls", "grid", "graph", "coherence", "replicas"],
                     help="extra reports: config-5 range / rounding study; GPU sketch-and-solve least squares; the paper's timing "
-                         "grid (PAPER.md:318-322); launch-bound config 1 replayed from a CUDA graph; the U(theta) coherence sweep (PAPER.md:344-352)")
+                         "grid (PAPER.md:318-322); launch-bound config 1 replayed from a CUDA graph; the U(theta) coherence sweep (PAPER.md:344-352); RN / SR / dither against the number of partial sketches")
     ap.add_argument("--grid", default="full", choices=["full", "quick"], help="--study grid / coherence: every point, or the corners / a small instance")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-pairs", action="store_true", help="skip the like-for-like flat/flat and tmem/tmem FP16-vs-FP32 timings")
@@ -806,6 +848,8 @@ def main():
         return run_graph_study(args)
     if args.study == "coherence":
         return run_coherence_study(args)
+    if args.study == "replicas":
+        return run_replica_study(args)
     return run_ours(args)
 
 
