@@ -220,7 +220,7 @@ def run_ours(args):
 
     import paper_2606_20195_b200 as ss
     import workloads as wl
-    from paper_2606_20195_b200.sharding import all_reduce_sketch, shard_rows
+    from paper_2606_20195_b200.sharding import shard_rows
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -233,7 +233,10 @@ def run_ours(args):
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
     torch.cuda.set_device(local)
     dist = None
-    if world > 1:
+    multi = world > 1
+    if "RANK" in os.environ and "WORLD_SIZE" in os.environ:
+        # under torchrun the NCCL communicator is created and used even with ONE rank: the collective leg (init, FP16 / FP32
+        # all-reduce of the sketch, barrier, max-over-ranks timing) then runs on whatever box this is, not only on N > 1
         import torch.distributed as dist_
 
         dist = dist_
@@ -259,7 +262,7 @@ def run_ours(args):
         sk.apply_f16acc(A, out=out16, variant=vid, row_begin=row_begin, rows=m, replicas=args.replicas, hash_mode=args.hash_mode,
                         tmem_group_mode=args.tmem_group_mode)
         if dist is not None:
-            all_reduce_sketch(out16, dist)
+            dist.all_reduce(out16)       # sum of the ranks' partial sketches: one more level of the FP16 hierarchy (sharding.py)
 
     def step16():
         # complete sketch ("initialization, map generation, and application"): when the scatter
@@ -271,7 +274,7 @@ def run_ours(args):
     def step32():
         sk.apply_f32acc(A, out=out32, row_begin=row_begin, rows=m)
         if dist is not None:
-            all_reduce_sketch(out32, dist)
+            dist.all_reduce(out32)
 
     # like-for-like pairs (same privatisation on both sides): what FP16 PRECISION buys as opposed to what privatisation
     # buys (Eq. (5)): flat REDs on both sides, and tensor memory on both sides where the FP32 partial fits
@@ -333,7 +336,7 @@ def run_ours(args):
     clocks = sampler.stop(w0, w1) if rank == 0 else None
     ms32, _, _, _ = timed(step32, max(2, args.steps // 2), 3)
     pairs = {}
-    if not args.no_pairs and dist is None:
+    if not args.no_pairs and not multi:
         k2 = max(2, args.steps // 2)
         if can(True, "flat_vec") and can(False, "flat_vec"):
             a16, a32 = timed(flat16, k2, 3)[0], timed(flat32, k2, 3)[0]
@@ -346,7 +349,7 @@ def run_ours(args):
     # step a2 alone: how fast this GPU delivers A when it is only read (sketch_stream_probe; context for roofline.frac, whose
     # denominator is a COPY rate).  Plain 256-bit loads and k_tmem's TMA ring without consumers, median of 5 passes over A.
     stream_probe = {}
-    if dist is None and m * n * 4 >= (1 << 28):
+    if not multi and m * n * 4 >= (1 << 28):
         for key, kind in (("ld256", 0), ("tma_ring", 1)):
             ts = []
             for rep_i in range(7):
@@ -421,7 +424,8 @@ def run_ours(args):
                                % (args.workload, zeta, m, n, d, m * n * 4 / 2**30),
                    "variant": plan16["variant"], "replicas": plan16["replicas"], "hash_mode": plan16["hash_mode"], "grid": plan16["grid"],
                    "l2": "input %s L2; %s" % ("<" if small else ">", "512 MiB flush write between steps" if small else "no flush needed"),
-                   "sharding": "rows; rank r hashes global rows [r*m,(r+1)*m); one NCCL all-reduce of the d x n sketch" if world > 1 else "single GPU"},
+                   "sharding": ("rows; rank r hashes global rows [r*m,(r+1)*m); one NCCL all-reduce of the d x n sketch (%d rank%s)" % (world, "" if world == 1 else "s"))
+                               if dist is not None else "single GPU"},
         "apply_only": {"ms_per_step": ms16_apply, "GBps": world * m * n * 4 / (ms16_apply * 1e-3) / 1e9,
                        "note": "hash-pack kernel excluded (map reused, as when A and b share one sketch, PAPER.md:356)"},
         "sketches_per_s": 1e3 / ms16,
