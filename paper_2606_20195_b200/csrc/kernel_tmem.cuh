@@ -1,4 +1,4 @@
-// kernel_tmem.cuh -- tensor-memory-privatised FP16-RN scatter for sm_100a.
+// kernel_tmem.cuh -- tensor-memory-privatised scatter (FP16 RN / SR / dither, bfloat16, FP32 accumulate) for sm_100a.
 //
 // The partial sketch of a warp lives in TENSOR MEMORY (TMEM: 128 lanes x 512 columns x 32 bit per SM, the
 // tcgen05 accumulator store), not in shared memory.  What makes that possible: every feature of one input
@@ -11,8 +11,9 @@
 // per FP16 half), and the SM's L1/shared data pipe -- 81 % busy in the shared-memory kernel
 // (profiles/r01_smem_c5.md) -- only carries A itself.
 //
-// CTA = NW = 4 consumer warps + 1 producer warp (2 at n = 64, up to 4 in the deferral modes), one CTA per SM (it
-// allocates all 512 TMEM columns), persistent over stages of T rows (32 KiB of A, a ring of NS shared-memory slots).
+// CTA = NW = 4 consumer warps + up to 4 producer warps, one per SM sub-partition (+ 1 right-hand-side warp when a fused b
+// rides along), one CTA per SM (it allocates all 512 TMEM columns), persistent over stages of T rows (32 KiB of A, a ring
+// of NS shared-memory slots).
 //   producers : one TMA copy per stage -- cp.async.bulk for a contiguous tile, a 2-D tensor-map box
 //               {N features x T rows} (cp.async.bulk.tensor.2d; rows past the end zero-filled) for strided rows and
 //               column slices -- L2 evict-first, completion on an mbarrier; meanwhile their lanes compute the stage's
@@ -24,8 +25,9 @@
 //               w % S and bucket group (w / S) % BQ of the rows of row-set w / (S*BQ) of every stage.
 //               Rows are processed in groups of G: all LDTMs of a group are issued, then one tcgen05.wait::ld, then
 //               the HFMA2s and STTMs; tcgen05.wait::st orders a group's LDTMs behind the previous group's STTMs.
-//               Two rows of a group that hit the same sketch row are either chained in registers or kept apart by the
-//               producers (deferral) -- see TmemGeom.
+//               Two rows of a group that hit the same sketch row are chained in registers, kept apart by the producers
+//               (deferral), or -- small sketches -- sent to private copies of the partial sketch (replicated rows);
+//               see TmemGeom.
 //   flush     : LDTM.x8 -> result-discarding vector REDs into B.
 //
 // Sketches larger than one warp's 512 TMEM columns (d * X > 512) are split two ways:
@@ -36,7 +38,8 @@
 //   CS column slices : gridDim.y CTAs (1..16) share a row range, CTA y takes the features [y * N, (y + 1) * N) of
 //               every row; the hashes are recomputed per slice.  n = 256: d = 1024 -> X = 2, BQ = 4, CS = 2;
 //               d = 2048 -> X = 1, BQ = 4, CS = 4; the paper's n = 1024, d = 2048 -> X = 1, BQ = 4, CS = 16.
-// Accumulation is FP16 RN throughout; the hierarchy is (warp-private partial) -> RED into B.
+// Accumulation is in the MODE's own arithmetic throughout (FP16 RN on the hot path); the hierarchy is
+// (warp-private partial [x G copies]) -> RED into B.
 #pragma once
 
 #include <cuda.h>  // CUtensorMap (type only; the encoder is fetched with cudaGetDriverEntryPoint)
