@@ -46,6 +46,8 @@ typedef struct sketch sketch_t; /* opaque, library-owned */
 #define SKETCH_ERR_UNSUPPORTED (-6) /* the forced variant cannot run this shape (AUTO never returns it) */
 #define SKETCH_ERR_CUDA (-7)        /* CUDA runtime error; text via sketch_last_error() */
 #define SKETCH_ERR_NOMEM (-8)       /* host or device allocation failed */
+#define SKETCH_ERR_SCRATCH_LIMIT (-9) /* sketch_apply_f16acc_noalloc only: two partial sketches of this d x n do not fit
+                                         the built-in scratch (SKETCH_NOALLOC_SCRATCH_BYTES); sizes in sketch_last_error() */
 
 /* conversion rule of the FP16 path (Sec. III-D) */
 #define SKETCH_RN 0 /* round-to-nearest-even, __float2half semantics */
@@ -152,6 +154,46 @@ int sketch_apply_f16acc_ex(const sketch_t* s, const float* A_dev, int32_t n, int
 
 int sketch_apply_bf16acc_ex(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev,
                             const sketch_opts_t* opts, void* stream);
+
+/* ---- for callers that must not allocate device memory ---------------------------------------- */
+
+/* Size of the scratch array built into the library's device image.  Every GPU on which the library's module is loaded
+ * holds this much for as long as the process lives, whether or not the entry point below is ever called. */
+#define SKETCH_NOALLOC_SCRATCH_BYTES (8u << 20) /* 8 MiB */
+
+/* sketch_apply_f16acc for programs that cannot call cudaMalloc while they run.
+ *
+ * Who that is: an application that gave all device memory to its own pool at start-up (nothing is left for us to
+ * allocate, and going around its pool defeats its accounting); a latency-bound or certified pipeline whose device memory
+ * map is frozen after initialisation (cudaMalloc / cudaFree synchronise the whole device, and an allocation that can fail
+ * in steady state is not acceptable there); a plug-in running inside a host program that forbids allocation in its
+ * callbacks.  Every other apply in this header may grow a library-owned buffer on some call; this one never does: it
+ * calls no cudaMalloc, no cudaFree and no routine that allocates on its behalf.
+ *
+ * What it computes: the complete FP16-accumulate sketch B = S*A of all m rows (Listing 2), exactly as
+ * sketch_apply_f16acc_ex does with variant = SKETCH_VARIANT_FLAT_VEC (SKETCH_VARIANT_GENERIC where n, lda or the
+ * alignment rule out vector REDs) and several L2-resident partial sketches: the same kernels, the same conversions
+ * (rounding = SKETCH_RN / SKETCH_SR / SKETCH_DITHER, sr_seed as there) and the same FP16 RN adds; only the home of the
+ * partial sketches differs -- a fixed array inside the library instead of a buffer from cudaMalloc.  It is not the
+ * fastest path for shapes the tensor-memory kernel takes (that kernel needs no scratch either: plain sketch_apply_f16acc
+ * already allocates nothing for those shapes as long as no right-hand side is fused).
+ * A_dev, B_dev, lda, stream: as for sketch_apply_f16acc; the caller passes (and owns) input and output as usual.
+ *
+ * Limit: two partial sketches must fit the array, i.e. 2 * roundup8(d * n) * 2 bytes <= SKETCH_NOALLOC_SCRATCH_BYTES
+ * (d * n <= 2 097 152, e.g. d = 2048 at n = 1024).  Larger sketches are refused with SKETCH_ERR_SCRATCH_LIMIT before
+ * anything is enqueued; sketch_last_error() then carries the sizes.  Within the limit it uses as many partial sketches
+ * as fit, at most 256.
+ *
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress, with that device current; this
+ * can make the CUDA runtime load the library's module there) and caches it per device ordinal (ordinals 0..63).  Make that
+ * first call during your own initialisation, on every device you will use, and before any stream capture begins.
+ *
+ * Sharing: there is ONE array per device, shared by every handle, stream and host thread of the process, and it keeps
+ * whatever the previous call left in it.  Each call zeroes the part it is about to use, on `stream`, before its kernels.
+ * Two calls whose GPU work can overlap (different streams without an ordering between them, or two host threads) add
+ * into the same partial sketches and both results are garbage: order such calls yourself (same stream, or an event). */
+int sketch_apply_f16acc_noalloc(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev, int rounding,
+                                uint64_t sr_seed, void* stream);
 
 /* ---- least-squares front end (PAPER.md:356 Sec. V-D; :312) ---------------------------------- */
 

@@ -32,7 +32,7 @@ class SketchOpts(C.Structure):
 class SketchError(RuntimeError):
     def __init__(self, code: int, where: str):
         self.code = code
-        detail = lib().sketch_last_error().decode() if code == -7 else ""
+        detail = lib().sketch_last_error().decode() if code in (-7, -9) else ""
         super().__init__("%s failed: %s (%d) %s" % (where, lib().sketch_strerror(code).decode(), code, detail))
 
 
@@ -49,6 +49,7 @@ SYMBOLS = {
     "sketch_apply_f32acc": (_int, [_vp, _vp, _i32, _i64, _vp, _vp]),
     "sketch_apply_f16acc": (_int, [_vp, _vp, _i32, _i64, _vp, _int, _u64, _vp]),
     "sketch_apply_bf16acc": (_int, [_vp, _vp, _i32, _i64, _vp, _vp]),
+    "sketch_apply_f16acc_noalloc": (_int, [_vp, _vp, _i32, _i64, _vp, _int, _u64, _vp]),
     "sketch_apply_bf16acc_ex": (_int, [_vp, _vp, _i32, _i64, _vp, _OP, _vp]),
     "sketch_apply_f16acc_with_rhs": (_int, [_vp, _vp, _i32, _i64, _vp, _vp, _vp, _OP, _vp]),
     "sketch_apply_f32acc_with_rhs": (_int, [_vp, _vp, _i32, _i64, _vp, _vp, _vp, _OP, _vp]),
@@ -266,6 +267,23 @@ class Sketch:
             rc = lib().sketch_apply_f16acc(self._h, ap, n, lda, out.data_ptr(), rounding, sr_seed & (2**64 - 1), _stream_ptr(stream))
         if rc:
             raise SketchError(rc, "sketch_apply_f16acc")
+        return out
+
+    def apply_f16acc_noalloc(self, A, out, rounding: int = RN, sr_seed: int = 0, stream=None):
+        """sketch_apply_f16acc_noalloc: the complete FP16 sketch of A (all m rows) for callers that may not allocate device
+        memory while running -- the partial sketches live in an 8 MiB array built into the library instead of a
+        cudaMalloc'ed buffer.  `out` is required (this wrapper allocates nothing either).  Raises SketchError -9 when two
+        partial sketches of d x n do not fit that array.  All calls on a device share the array: do not let two overlap."""
+        import torch
+
+        ap, n, lda = self._A_args(A)
+        _check_cuda(out, torch.float16, "out")
+        assert out.is_contiguous() and tuple(out.shape) == (self.d, n)
+        if A.shape[0] != self.m:
+            raise ValueError("A has %d rows, sketch was created for m=%d" % (A.shape[0], self.m))
+        rc = lib().sketch_apply_f16acc_noalloc(self._h, ap, n, lda, out.data_ptr(), rounding, sr_seed & (2**64 - 1), _stream_ptr(stream))
+        if rc:
+            raise SketchError(rc, "sketch_apply_f16acc_noalloc")
         return out
 
     def apply_bf16acc(self, A, out=None, stream=None, **opts):

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "kernel_misc.cuh"
@@ -739,6 +740,56 @@ int apply_host(const sketch_t* cs, const float* A, int32_t n, int64_t lda, void*
 }  // namespace
 
 // =================================================================================================
+// Built-in scratch of sketch_apply_f16acc_noalloc (include/sparse_sketch.h).
+//
+// Some programs that link this library must not allocate device memory once they are running: a solver that has handed
+// the whole GPU to its own memory pool at start-up, a real-time or safety-reviewed pipeline whose memory map is frozen
+// after initialisation (a cudaMalloc there is both forbidden and a latency spike, since it synchronises the device),
+// or a plug-in that is called in a context whose owner forbids allocation.  The ordinary flat scatter keeps its partial
+// sketches in a cudaMalloc'ed buffer that grows on demand, which these callers cannot use.  For them the partial
+// sketches live in the array below: it is part of the library's device image, so the driver reserves it when the module
+// is loaded on a GPU and gives it back when the process exits -- SKETCH_NOALLOC_SCRATCH_BYTES on every GPU that loads
+// the library, whether or not the entry point is ever called.
+//
+// On the host the identifier g_noalloc_scratch is only a handle for the runtime's symbol table -- its host address is
+// not a device address and must never reach a kernel.  noalloc_scratch_ptr() asks the runtime for the real address on
+// the CURRENT device (cudaGetSymbolAddress), once per device ordinal, and that is the only pointer the launches see.
+// =================================================================================================
+static __device__ __align__(256) unsigned char g_noalloc_scratch[SKETCH_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+void* g_noalloc_ptr[kNoallocMaxDevices];   // device address of g_noalloc_scratch per device ordinal; nullptr = not asked yet
+
+// Device address of the built-in scratch on the current device.  The first call on a device performs the symbol lookup
+// (which may also make the runtime load this library's module on that device); later calls only read the cached pointer.
+int noalloc_scratch_ptr(void** out) {
+  int dev = -1;
+  CU_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kNoallocMaxDevices) {
+    snprintf(g_last_error, sizeof(g_last_error), "sketch_apply_f16acc_noalloc: device ordinal %d outside [0, %d)", dev, kNoallocMaxDevices);
+    return SKETCH_ERR_CUDA;
+  }
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_ptr[dev]) {
+    void* p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(g_noalloc_scratch)");
+    if (!p) {
+      snprintf(g_last_error, sizeof(g_last_error), "cudaGetSymbolAddress(g_noalloc_scratch) returned a null address on device %d", dev);
+      return SKETCH_ERR_CUDA;
+    }
+    g_noalloc_ptr[dev] = p;
+  }
+  *out = g_noalloc_ptr[dev];
+  return SKETCH_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
 extern "C" {
 
 int sketch_create(int64_t m, int32_t d, int32_t zeta, uint64_t seed, sketch_t** out) {
@@ -832,6 +883,62 @@ int sketch_apply_f16acc_ex(const sketch_t* s, const float* A_dev, int32_t n, int
 int sketch_apply_bf16acc_ex(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, void* B_dev,
                             const sketch_opts_t* opts, void* stream) {
   return apply_device(s, A_dev, n, lda, B_dev, sk::OUT_BF16, SKETCH_RN, 0, opts, stream);
+}
+
+// The flat FP16 scatter with its partial sketches in g_noalloc_scratch instead of the handle's cudaMalloc'ed buffer.
+// Same kernels and the same arithmetic as sketch_apply_f16acc_ex with variant FLAT_VEC (GENERIC for shapes the vector REDs
+// cannot take) and `replicas` partial sketches; nothing on this path calls cudaMalloc, cudaFree or a library routine that
+// allocates (cudaMemsetAsync, the two launches and -- first call on a device only -- cudaGetSymbolAddress are all it uses).
+int sketch_apply_f16acc_noalloc(const sketch_t* cs, const float* A_dev, int32_t n, int64_t lda, void* B_dev, int rounding,
+                                uint64_t sr_seed, void* stream) {
+  sketch* s = const_cast<sketch*>(cs);
+  int64_t row_begin = 0, rows = 0;
+  int rc = validate_apply(s, A_dev, n, lda, B_dev, true, nullptr, &row_begin, &rows);
+  if (rc) return rc;
+  if (rounding != SKETCH_RN && rounding != SKETCH_SR && rounding != SKETCH_DITHER) return SKETCH_ERR_INVALID;
+  // at least two partial sketches must fit: with one, the scatter would go straight into B and need no scratch at all
+  const int64_t count = (int64_t)s->d * n;
+  const int64_t pstride = padded_count(count);
+  const uint64_t slot_bytes = (uint64_t)pstride * 2;
+  const uint64_t fit = (uint64_t)SKETCH_NOALLOC_SCRATCH_BYTES / slot_bytes;
+  if (fit < 2) {
+    snprintf(g_last_error, sizeof(g_last_error),
+             "sketch_apply_f16acc_noalloc: a %d x %d FP16 sketch takes %llu bytes per partial sketch; two of them do not fit the "
+             "built-in scratch of %llu bytes (limit: d * n <= %llu)",
+             s->d, n, (unsigned long long)slot_bytes, (unsigned long long)SKETCH_NOALLOC_SCRATCH_BYTES,
+             (unsigned long long)SKETCH_NOALLOC_SCRATCH_BYTES / 4);
+    return SKETCH_ERR_SCRATCH_LIMIT;
+  }
+  // as many partial sketches as fit, at most 256, and no more than keep zeroing + folding under 1/8 of A's bytes
+  // (the rule of the allocating path, make_plan)
+  uint64_t P = fit < 256 ? fit : 256;
+  const uint64_t by_input = (uint64_t)rows * (uint64_t)n * 4 / 8 / slot_bytes;
+  if (P > by_input) P = by_input < 2 ? 2 : by_input;
+  sketch_opts_t o;
+  memset(&o, 0, sizeof(o));
+  o.variant = SKETCH_VARIANT_FLAT_VEC;
+  o.replicas = (int32_t)P;
+  Plan p;
+  rc = make_plan(s, n, lda, A_dev, B_dev, sk::OUT_F16, rounding, &o, rows, &p);   // host only
+  if (rc == SKETCH_ERR_UNSUPPORTED) {
+    o.variant = SKETCH_VARIANT_GENERIC;
+    rc = make_plan(s, n, lda, A_dev, B_dev, sk::OUT_F16, rounding, &o, rows, &p);
+  }
+  if (rc) return rc;
+  void* scratch = nullptr;
+  rc = noalloc_scratch_ptr(&scratch);
+  if (rc) return rc;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  // the array keeps what the previous call left in it: every partial sketch this call adds into starts at zero
+  CU_TRY(cudaMemsetAsync(scratch, 0, (size_t)(slot_bytes * P), st));
+  sk::ScatterArgs a = make_args(s, A_dev, n, lda, scratch, row_begin, rows, sr_seed, p.vec);
+  a.replicas = (int32_t)P;
+  if (p.variant == SKETCH_VARIANT_GENERIC) rc = launched(sk::launch_generic(a, sk::OUT_F16, rounding, p.grid, st), "k_generic (noalloc)");
+  else rc = launched(sk::launch_flat_f16(a, s->zeta, p.vec, rounding, 0, p.grid, st), "k_flat<f16> (noalloc)");
+  if (rc) return rc;
+  int grid = (int)((count + 255) / 256);
+  if (grid > s->sm_count * 8) grid = s->sm_count * 8;
+  return fold_replicas(sk::OUT_F16, scratch, pstride, (int)P, B_dev, count, 0, grid, st);   // overwrites B: a complete sketch
 }
 
 int sketch_apply_f16acc_with_rhs(const sketch_t* s, const float* A_dev, int32_t n, int64_t lda, const float* b_dev,
@@ -965,6 +1072,7 @@ const char* sketch_strerror(int code) {
     case SKETCH_ERR_UNSUPPORTED: return "the forced variant does not support this shape";
     case SKETCH_ERR_CUDA: return "CUDA runtime error (see sketch_last_error)";
     case SKETCH_ERR_NOMEM: return "out of memory";
+    case SKETCH_ERR_SCRATCH_LIMIT: return "sketch too large for the built-in scratch of sketch_apply_f16acc_noalloc (see sketch_last_error)";
   }
   return "unknown error code";
 }
