@@ -17,13 +17,23 @@
  *     the handle, its scratch (replicated partial sketches, optional packed hash array,
  *     staging buffers) and frees them in sketch_destroy;
  *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  apply/dump calls
- *     are asynchronous on that stream and never synchronise, except the first call that has
- *     to grow a scratch buffer (cudaMalloc) and the *_host entry points (which return after
- *     the result is in host memory);
+ *     are asynchronous on that stream and never synchronise, except a call that has to grow a
+ *     scratch buffer (cudaMalloc; the first call of a shape, outside any capture) and the *_host
+ *     entry points (which return after the result is in host memory);
  *   - A is never modified; one handle may be applied to any number of matrices with any n
  *     (S is d x m, independent of n), e.g. A in FP16 and b in FP32 with the same map as in
  *     PAPER.md:356 / Table I.
  *   - a handle must not be used from two host threads at once.
+ *   - CUDA graphs (stream capture).  Every device-buffer apply can be captured, with two rules.  (1) Nothing is allocated
+ *     inside a capture: if the call would have to create or grow a library-owned scratch buffer (the partial sketches of
+ *     the FLAT / GENERIC variants with replicas > 1, those of a fused right-hand side, the packed hash array of the SMEM
+ *     variant / hash_mode 2) it fails with SKETCH_ERR_CAPTURE and enqueues nothing that uses it -- run the same apply once
+ *     outside the capture first (the *_noalloc entry point and the TMEM / SMALL variants without a right-hand side use
+ *     none).  (2) The graph holds the scratch pointers it was captured with.  The library keeps such a buffer alive until
+ *     sketch_destroy even when a later call needs a larger one (it then allocates a second buffer), so a replay never
+ *     touches freed memory; but the stream ordering the library provides between applies on different streams does not
+ *     extend to replays, which go through no library call: order every replay against other work on the same handle
+ *     yourself (one stream, or events), or give each graph a handle of its own.  Destroy the graph before the handle.
  */
 #ifndef SPARSE_SKETCH_H_
 #define SPARSE_SKETCH_H_
@@ -46,6 +56,8 @@ typedef struct sketch sketch_t; /* opaque, library-owned */
 #define SKETCH_ERR_UNSUPPORTED (-6) /* the forced variant cannot run this shape (AUTO never returns it) */
 #define SKETCH_ERR_CUDA (-7)        /* CUDA runtime error; text via sketch_last_error() */
 #define SKETCH_ERR_NOMEM (-8)       /* host or device allocation failed */
+#define SKETCH_ERR_CAPTURE (-10)    /* a library-owned scratch buffer would have to be created or grown inside a stream
+                                       capture (see "CUDA graphs" above); text in sketch_last_error() */
 #define SKETCH_ERR_SCRATCH_LIMIT (-9) /* sketch_apply_f16acc_noalloc only: two partial sketches of this d x n do not fit
                                          the built-in scratch (SKETCH_NOALLOC_SCRATCH_BYTES); sizes in sketch_last_error() */
 
@@ -119,7 +131,8 @@ int sketch_hashes_dump(const sketch_t* s, int32_t* bucket_dev, uint8_t* signbit_
 /* Build (once) the packed per-(row,block) hash array the hash_mode=2 kernels read; m*zeta entries, library-owned:
  * uint16 = bucket | reload<<14 | signbit<<15 in the sub-step order of the SMEM variant (entry (row, t) at row*zeta + t holds
  * block (row mod R + t) mod zeta, R = min(zeta, 4)) when zeta is 1, 2, 4 or 8 and d <= 2047, else uint32 = bucket | signbit<<31
- * at row*zeta + j.  Counted in "complete sketch" time by bench.py when that mode is used. */
+ * at row*zeta + j.  Counted in "complete sketch" time by bench.py when that mode is used.  Not inside a stream
+ * capture (SKETCH_ERR_CAPTURE): the handle would count the array as built while the graph has yet to run. */
 int sketch_precompute_hashes(sketch_t* s, void* stream);
 
 /* ---- scatter kernels ------------------------------------------------- */

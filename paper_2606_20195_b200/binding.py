@@ -32,7 +32,7 @@ class SketchOpts(C.Structure):
 class SketchError(RuntimeError):
     def __init__(self, code: int, where: str):
         self.code = code
-        detail = lib().sketch_last_error().decode() if code in (-7, -9) else ""
+        detail = lib().sketch_last_error().decode() if code in (-7, -9, -10) else ""
         super().__init__("%s failed: %s (%d) %s" % (where, lib().sketch_strerror(code).decode(), code, detail))
 
 

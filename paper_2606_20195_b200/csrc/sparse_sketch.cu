@@ -63,6 +63,13 @@ struct sketch {
   cudaStream_t scratch_stream;
   cudaEvent_t ev_scratch;
   int scratch_busy;   // 0 = never used, 1 = ev_scratch is valid
+  // stream capture: a captured apply bakes the scratch pointers into its graph, so a buffer a capture has used is pinned --
+  // when a later call needs a larger one, the old buffer is retired (kept until sketch_destroy), never freed under the graph
+  int rep_pinned, sbrep_pinned, packed_pinned;
+  struct Retired {
+    void* buf;
+    Retired* next;
+  }* retired;
   // tensor maps of the strided / column-sliced tensor-memory launches, keyed by what they encode (a handle is applied
   // to the same few matrices over and over: the hot call then does no encoding)
   struct TmapSlot {
@@ -102,10 +109,31 @@ int ensure_device(sketch* s) {
   return SKETCH_OK;
 }
 
-int ensure_scratch(void** buf, size_t* have, size_t want) {
-  if (*have >= want) return SKETCH_OK;
+// Grow a library-owned buffer to `want` bytes.  Inside a stream capture nothing may be allocated or freed: a buffer that
+// is large enough is marked pinned (the graph now refers to it), one that is not makes the call fail with
+// SKETCH_ERR_CAPTURE.  Outside a capture a pinned buffer that must grow is retired instead of freed.
+int ensure_scratch(sketch* s, void** buf, size_t* have, size_t want, bool capturing = false, int* pinned = nullptr) {
+  if (*have >= want) {
+    if (capturing && pinned) *pinned = 1;
+    return SKETCH_OK;
+  }
+  if (capturing) {
+    snprintf(g_last_error, sizeof(g_last_error),
+             "a library-owned scratch buffer would have to grow from %zu to %zu bytes inside a stream capture; run the same "
+             "apply once outside the capture first", *have, want);
+    return SKETCH_ERR_CAPTURE;
+  }
   if (*buf) {
-    CU_TRY(cudaFree(*buf));
+    if (pinned && *pinned) {
+      sketch::Retired* r = new (std::nothrow) sketch::Retired;
+      if (!r) return SKETCH_ERR_NOMEM;
+      r->buf = *buf;
+      r->next = s->retired;
+      s->retired = r;
+      *pinned = 0;
+    } else {
+      CU_TRY(cudaFree(*buf));
+    }
     *buf = nullptr;
     *have = 0;
   }
@@ -373,8 +401,8 @@ int launched(cudaError_t e, const char* what) {
 }
 
 // Order the library-owned scratch behind its previous use when the caller switches streams.  Inside a stream capture
-// nothing is recorded or waited for (events cannot cross a capture): captured applies that share scratch must be
-// ordered by the caller (include/sparse_sketch.h).
+// nothing is recorded or waited for (events cannot cross a capture): replays of a captured apply that uses scratch must
+// be ordered by the caller against every other apply on the handle (include/sparse_sketch.h, "CUDA graphs").
 int scratch_acquire(sketch* s, cudaStream_t st, bool* capturing) {
   cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
   CU_TRY(cudaStreamIsCapturing(st, &cs));
@@ -424,13 +452,23 @@ int tensor_map_for(sketch* s, const float* A, int n, int64_t lda, int64_t rows, 
 
 // a1 in its precomputed form.  16-bit entries in sub-step order (kernel_smem.cuh) when zeta is templated and the
 // sketch fits the 15-bit bucket field, else plain 32-bit entries (bucket | sign<<31).  force: re-run the kernel.
-int ensure_packed(sketch* s, cudaStream_t st, bool force) {
-  if (s->packed_width && !force) return SKETCH_OK;
+int ensure_packed(sketch* s, cudaStream_t st, bool force, bool capturing) {
+  if (s->packed_width && !force) {
+    if (capturing) s->packed_pinned = 1;
+    return SKETCH_OK;
+  }
+  if (capturing) {
+    // the array would be filled when the graph is replayed, not now, while the handle already counted it as built
+    snprintf(g_last_error, sizeof(g_last_error),
+             "the packed hash array cannot be built inside a stream capture; call sketch_precompute_hashes (or run the same "
+             "apply once) before capturing");
+    return SKETCH_ERR_CAPTURE;
+  }
   int rc = ensure_device(s);
   if (rc) return rc;
   const bool rot = rot_ok(s);
   const int64_t total = s->m * (int64_t)s->zeta;
-  rc = ensure_scratch(&s->packed, &s->packed_bytes, (size_t)total * (rot ? 2 : 4));
+  rc = ensure_scratch(s, &s->packed, &s->packed_bytes, (size_t)total * (rot ? 2 : 4), false, &s->packed_pinned);
   if (rc) return rc;
   int64_t blocks = rot ? (s->m / 28 + 1 + 7) / 8 : (total + 255) / 256;  // rot: one warp per 28 rows, 8 warps per block
   int64_t cap = (int64_t)s->sm_count * 16;
@@ -521,7 +559,7 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
         if (rc) return rc;
         g.sb_stride = padded_count(s->d);
         g.sb_replicas = kSbReplicas;
-        rc = ensure_scratch(&s->sbrep, &s->sbrep_bytes, (size_t)g.sb_stride * 4 * kSbReplicas);
+        rc = ensure_scratch(s, &s->sbrep, &s->sbrep_bytes, (size_t)g.sb_stride * 4 * kSbReplicas, capturing, &s->sbrep_pinned);
         if (rc) return rc;
         g.Sb = static_cast<float*>(s->sbrep);
         CU_TRY(cudaMemsetAsync(s->sbrep, 0, (size_t)g.sb_stride * 4 * kSbReplicas, st));
@@ -570,7 +608,7 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
       bool capturing = false;
       rc = scratch_acquire(s, st, &capturing);
       if (rc) return rc;
-      rc = ensure_packed(s, st, false);
+      rc = ensure_packed(s, st, false, capturing);
       if (rc) return rc;
       g.s.packed = s->packed;
       rc = launched(sk::launch_smem_f16(g, s->zeta, p.wpc, p.grid, p.smem_bytes, st), "k_smem");
@@ -594,7 +632,7 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
     if (rc) return rc;
   }
   if (P > 1) {
-    rc = ensure_scratch(&s->rep, &s->rep_bytes, (size_t)pstride * elem * P);
+    rc = ensure_scratch(s, &s->rep, &s->rep_bytes, (size_t)pstride * elem * P, capturing, &s->rep_pinned);
     if (rc) return rc;
     target = s->rep;
     CU_TRY(cudaMemsetAsync(target, 0, (size_t)pstride * elem * P, st));
@@ -603,7 +641,7 @@ int apply_device(const sketch_t* cs, const float* A, int32_t n, int64_t lda, voi
   }
   int pw = 0;
   if (packed_hashes) {
-    rc = ensure_packed(s, st, false);
+    rc = ensure_packed(s, st, false, capturing);
     if (rc) return rc;
     pw = s->packed_width;
   }
@@ -664,7 +702,7 @@ int apply_host_impl(sketch* s, const float* A, int32_t n, int64_t lda, void* B, 
   if (s->stage_bytes < chunk_bytes) {
     for (int k = 0; k < 2; ++k) {
       size_t have = s->stage[k] ? s->stage_bytes : 0;
-      rc = ensure_scratch(&s->stage[k], &have, chunk_bytes);
+      rc = ensure_scratch(s, &s->stage[k], &have, chunk_bytes);
       if (rc) return rc;
     }
     s->stage_bytes = chunk_bytes;
@@ -674,7 +712,7 @@ int apply_host_impl(sketch* s, const float* A, int32_t n, int64_t lda, void* B, 
   // on a single running sum (measured at c5: relF 2.5e-2 instead of 7e-3).
   const int64_t nchunks = rows > 0 ? (rows + chunk_rows - 1) / chunk_rows : 0;
   const int64_t kSlots = nchunks < 64 ? (nchunks > 0 ? nchunks : 1) : 64;
-  rc = ensure_scratch(&s->bdev, &s->bdev_bytes, slot_bytes * (size_t)(kSlots + 1));
+  rc = ensure_scratch(s, &s->bdev, &s->bdev_bytes, slot_bytes * (size_t)(kSlots + 1));
   if (rc) return rc;
   char* const slots = static_cast<char*>(s->bdev);            // [kSlots][padded d*n]
   char* const result = slots + slot_bytes * (size_t)kSlots;    // [d][n]
@@ -816,6 +854,12 @@ int sketch_destroy(sketch_t* s) {
   if (s->rep) cudaFree(s->rep);
   if (s->sbrep) cudaFree(s->sbrep);
   if (s->packed) cudaFree(s->packed);
+  while (s->retired) {
+    sketch::Retired* r = s->retired;
+    s->retired = r->next;
+    cudaFree(r->buf);
+    delete r;
+  }
   for (int k = 0; k < 2; ++k)
     if (s->stage[k]) cudaFree(s->stage[k]);
   if (s->bdev) cudaFree(s->bdev);
@@ -852,7 +896,7 @@ int sketch_precompute_hashes(sketch_t* s, void* stream) {
   bool capturing = false;
   int rc = scratch_acquire(s, st, &capturing);
   if (rc) return rc;
-  rc = ensure_packed(s, st, true);
+  rc = ensure_packed(s, st, true, capturing);
   if (rc) return rc;
   return scratch_release(s, st, capturing);
 }
@@ -1072,6 +1116,7 @@ const char* sketch_strerror(int code) {
     case SKETCH_ERR_UNSUPPORTED: return "the forced variant does not support this shape";
     case SKETCH_ERR_CUDA: return "CUDA runtime error (see sketch_last_error)";
     case SKETCH_ERR_NOMEM: return "out of memory";
+    case SKETCH_ERR_CAPTURE: return "library scratch would have to be allocated inside a stream capture (see sketch_last_error)";
     case SKETCH_ERR_SCRATCH_LIMIT: return "sketch too large for the built-in scratch of sketch_apply_f16acc_noalloc (see sketch_last_error)";
   }
   return "unknown error code";

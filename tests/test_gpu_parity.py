@@ -645,6 +645,79 @@ def test_applies_are_asynchronous_capturable_and_allocation_free(ss, m, n, d, ze
         assert ev.rel_fro(oracle.half_bits_to_f64(bits(out16)), B) <= 5e-3
 
 
+def test_capture_allocates_nothing_and_captured_scratch_survives_regrowth(ss):
+    # include/sparse_sketch.h "CUDA graphs": (1) a capture that would have to create library scratch fails with
+    # SKETCH_ERR_CAPTURE (-10) instead of running cudaMalloc inside the capture; (2) a scratch buffer a graph was captured
+    # with is kept until sketch_destroy even when a later eager apply on another stream needs a larger one, so the replay
+    # after that regrowth still reads and writes live memory.  Flat FP16 with 8 partial sketches = the scratch path.
+    m, n, n_big, d, zeta = 20000, 64, 512, 128, 4
+    seed = sketch_seed(91)
+    sk = ss.Sketch(m, d, zeta, seed)
+    A1, A2, A3 = wl.integer_valued(m, n, 51), wl.integer_valued(m, n, 52), wl.integer_valued(m, n_big, 53)
+    A = dev(A1)
+    out = torch.empty((d, n), dtype=torch.float16, device="cuda")
+    side, other = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    kw = dict(variant=VID["flat_vec"], replicas=8)
+    pl = sk.plan(n, **kw)
+    assert pl["variant"] == "flat_vec" and pl["replicas"] == 8
+    # (1) first use inside a capture: refused, nothing launched
+    g0 = torch.cuda.CUDAGraph()
+    launches0 = ss.sketch_launch_count()
+    code, text = None, ""
+    with torch.cuda.graph(g0, stream=side):
+        out.zero_()                                   # keeps the aborted capture non-empty
+        try:
+            sk.apply_f16acc(A, out=out, **kw)
+        except ss.SketchError as e:
+            code, text = e.code, str(e)
+    assert code == -10 and "capture" in text
+    assert ss.sketch_launch_count() == launches0
+    del g0
+    # the same for the packed hash array (hash_mode 2) and for building it explicitly
+    g0 = torch.cuda.CUDAGraph()
+    codes = []
+    with torch.cuda.graph(g0, stream=side):
+        out.zero_()
+        for call in (lambda: sk.apply_f16acc(A, out=out, variant=VID["flat_vec"], replicas=1, hash_mode=2), lambda: sk.precompute_hashes(stream=side)):
+            try:
+                call()
+                codes.append(0)
+            except ss.SketchError as e:
+                codes.append(e.code)
+    assert codes == [-10, -10]
+    del g0
+    # (2) warm-up outside, capture, replay
+    with torch.cuda.stream(side):
+        sk.apply_f16acc(A, out=out, **kw)
+    side.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        sk.apply_f16acc(A, out=out, **kw)
+    A.copy_(dev(A2))
+    out.fill_(3)
+    g.replay()
+    torch.cuda.synchronize()
+    want2 = oracle.f64_sketch(seed, d, zeta, A2)
+    assert np.array_equal(oracle.half_bits_to_f64(bits(out)), want2)
+    # an eager apply with eight times the columns on another stream: the handle's partial-sketch buffer has to grow
+    Ab = dev(A3)
+    with torch.cuda.stream(other):
+        big = sk.apply_f16acc(Ab, variant=VID["flat_vec"], replicas=8)
+    other.synchronize()
+    assert np.array_equal(oracle.half_bits_to_f64(bits(big)), oracle.f64_sketch(seed, d, zeta, A3))
+    # churn the allocator so that a freed buffer would have been handed out again and overwritten
+    junk = [torch.full((1 << 18,), 7.0, device="cuda") for _ in range(16)]
+    torch.cuda.synchronize()
+    for _ in range(3):
+        out.fill_(3)
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(oracle.half_bits_to_f64(bits(out)), want2)
+    del junk, g
+    sk.close()
+
+
 def test_one_handle_on_two_streams_keeps_its_scratch_ordered(ss):
     # the replicated partial sketches and the packed hash array belong to the handle; applies on different streams are
     # ordered behind each other's use of them
