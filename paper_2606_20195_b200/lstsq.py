@@ -35,19 +35,29 @@ def sketch_system(sk: Sketch, A, b, precision: str = "f16", SA=None, Sb=None, st
     raise ValueError("precision must be one of %s" % (PRECISIONS,))
 
 
-def solve_sketched(SA, Sb, W=None):
+def solve_sketched(SA, Sb, W=None, stream=None):
     """x = argmin ||SA x - Sb||_2 in FP32: exact promotion, Householder QR, Q^T Sb, back substitution.  W: optional
-    FP32 d x n workspace for the promoted copy."""
+    FP32 d x n workspace for the promoted copy.  stream: the torch stream SA and Sb were produced on (None = the current
+    one); the promotion and the library calls are issued on that same stream, so they are ordered behind the sketch, and the
+    returned vector is ready on it."""
     import torch
 
-    M = SA if SA.dtype == torch.float32 else sketch_widen(SA, out=W)
-    n = M.shape[1]
-    a, tau = torch.geqrf(M)
-    y = torch.ormqr(a, tau, Sb.reshape(-1, 1), left=True, transpose=True)[:n]
-    return torch.linalg.solve_triangular(a[:n].triu(), y, upper=True)[:, 0]
+    st = stream if stream is not None else torch.cuda.current_stream()
+    with torch.cuda.stream(st):
+        M = SA if SA.dtype == torch.float32 else sketch_widen(SA, out=W, stream=st)
+        n = M.shape[1]
+        a, tau = torch.geqrf(M)
+        y = torch.ormqr(a, tau, Sb.reshape(-1, 1), left=True, transpose=True)[:n]
+        return torch.linalg.solve_triangular(a[:n].triu(), y, upper=True)[:, 0]
 
 
 def sketch_and_solve(sk: Sketch, A, b, precision: str = "f16", SA=None, Sb=None, W=None, stream=None, **opts):
-    """The complete pipeline of PAPER.md:356 on device buffers; returns the FP32 solution vector (length n)."""
-    SA, Sb = sketch_system(sk, A, b, precision, SA=SA, Sb=Sb, stream=stream, **opts)
-    return solve_sketched(SA, Sb, W=W)
+    """The complete pipeline of PAPER.md:356 on device buffers; returns the FP32 solution vector (length n).  Every stage
+    runs on `stream` (None = torch's current stream); with a side stream the caller orders its own reads of the result
+    behind that stream, as for any torch op issued there."""
+    import torch
+
+    st = stream if stream is not None else torch.cuda.current_stream()
+    with torch.cuda.stream(st):       # the buffers sketch_system allocates belong to the stream that fills them
+        SA, Sb = sketch_system(sk, A, b, precision, SA=SA, Sb=Sb, stream=st, **opts)
+    return solve_sketched(SA, Sb, W=W, stream=st)

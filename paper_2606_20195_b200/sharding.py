@@ -21,10 +21,25 @@ def shard_rows(m_total: int, world_size: int, rank: int, align: int = 4):
 
 
 def all_reduce_sketch(partial, dist=None):
-    """Sum the ranks' partial sketches in place (NCCL on GPUs, gloo on CPU).  `partial` is a torch tensor
-    of the sketch dtype; for FP16 sketches this is one more level of the accumulation hierarchy."""
+    """Sum the ranks' partial sketches in place (NCCL on GPUs, gloo on CPU) -- the one collective of the sharded path,
+    called by bench.py after every apply.  `partial` is a torch tensor of the sketch dtype; for FP16 sketches this is one
+    more level of the accumulation hierarchy.  Runs whenever a process group exists, also with a single rank (the
+    communicator is then exercised on whatever box this is); without a process group it is the identity."""
     if dist is None:
         import torch.distributed as dist  # noqa: PLC0415
-    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+    if dist.is_available() and dist.is_initialized():
         dist.all_reduce(partial)
     return partial
+
+
+def max_over_ranks(value: float, dist=None, device=None) -> float:
+    """The slowest rank's value (bench.py's timing rule: a multi-GPU number is the max over ranks of the device time).
+    One FP64 all-reduce with MAX on `device` (the rank's GPU under NCCL, CPU under gloo); identity without a process group."""
+    import torch  # noqa: PLC0415
+
+    if dist is None:
+        import torch.distributed as dist  # noqa: PLC0415
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized():
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())

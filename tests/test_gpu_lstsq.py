@@ -94,3 +94,35 @@ def test_device_generators_have_the_families_structure(ss):
     A2, b2 = wl.ls_paper_low_coherence_device(m, n, 3, dv)
     s = torch.linalg.svdvals(A2.double())
     assert abs(float(s[0]) - 100.0) < 8.0 and abs(float(s[-1]) - 1.0) < 0.2
+
+
+def test_sketch_and_solve_on_a_side_stream_runs_every_stage_there(ss):
+    # lstsq.sketch_and_solve(stream=...) issues the sketch, the promotion and the library QR / solve on that one stream.  The
+    # side stream is kept busy first, so a factorisation issued on the (idle) current stream would read SA long before the
+    # sketch kernels have run and return something else.
+    from paper_2606_20195_b200 import lstsq
+
+    m, n, zeta, d = 1 << 18, 256, 4, 512
+    A, b = wl.ls_paper_low_coherence(m, n, 8)
+    sk = ss.Sketch(m, d, zeta, sketch_seed(93))
+    Ad, bd = dev(A), dev(b)
+    for prec in ("f32", "f16"):
+        x_ref = lstsq.sketch_and_solve(sk, Ad, bd, prec).double()
+        torch.cuda.synchronize()
+        side = torch.cuda.Stream()
+        SA = torch.full((d, n), float("nan"), dtype=torch.float32 if prec == "f32" else torch.float16, device="cuda")
+        Sb = torch.full((d,), float("nan"), dtype=torch.float32, device="cuda")
+        torch.cuda.synchronize()
+        with torch.cuda.stream(side):
+            busy = torch.randn(4096, 4096, device="cuda")
+            for _ in range(40):
+                busy = busy @ busy * 1e-2
+        x = lstsq.sketch_and_solve(sk, Ad, bd, prec, SA=SA, Sb=Sb, stream=side)
+        side.synchronize()
+        x = x.double()
+        assert bool(torch.isfinite(x).all())
+        # FP32 sketches differ only in the order of their atomic adds; FP16 ones in the order of the flush as well
+        tol = 1e-3 if prec == "f32" else 5e-2
+        assert float((x - x_ref).norm() / x_ref.norm()) <= tol
+        del busy
+    sk.close()

@@ -1,9 +1,11 @@
 """World-size-2 CPU (gloo) test of the N > 1 path's host logic (tier framing 5).
 
 The kernels cannot run here, so each rank forms its shard's partial sketch with the oracle (test
-infrastructure) using the row range `shard_rows` hands it, the partials are summed with the same
-`all_reduce_sketch` the bench uses, and the result must equal the oracle's sketch of the whole matrix:
-this pins the row bookkeeping (ranges tile [0, m) exactly, the global row index enters the hash).
+infrastructure) using the row range `shard_rows` hands it, the partials are summed with
+`sharding.all_reduce_sketch` -- the call bench.py makes after every apply -- and the result must equal the
+oracle's sketch of the whole matrix: this pins the row bookkeeping (ranges tile [0, m) exactly, the global
+row index enters the hash).  The bench's timing rule (`sharding.max_over_ranks`: the slowest rank's time, the
+same value on every rank) and its rank-0-only reporting are covered on the same two-rank group.
 """
 import os
 import socket
@@ -20,7 +22,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_2606_20195_b200.sharding import all_reduce_sketch, shard_rows  # noqa: E402
+from paper_2606_20195_b200.sharding import all_reduce_sketch, max_over_ranks, shard_rows  # noqa: E402
 
 
 def test_shard_rows_tile_the_matrix_exactly():
@@ -56,6 +58,11 @@ def _worker(rank: int, world: int, port: int, m: int, n: int, d: int, zeta: int,
         part = oracle.f64_sketch(seed, d, zeta, A[begin:begin + rows], row_begin=begin)
         t = torch.from_numpy(part)
         all_reduce_sketch(t, dist)
+        # the bench's collective leg around it: every rank learns the slowest rank's time; only rank 0 reports
+        slowest = max_over_ranks(10.0 + 5.0 * rank, dist)
+        h16 = torch.full((8,), 1.0 + rank, dtype=torch.float16)
+        all_reduce_sketch(h16, dist)                       # FP16 sketches are reduced in FP16
+        np.save(os.path.join(out_dir, "leg%d.npy" % rank), np.array([slowest, float(h16[0])]))
         if rank == 0:
             np.save(os.path.join(out_dir, "sum.npy"), t.numpy())
     finally:
@@ -72,7 +79,17 @@ def test_two_rank_row_sharded_sketch_equals_whole(tmp_path):
     port = _free_port()
     mp.spawn(_worker, args=(world, port, m, n, d, zeta, str(tmp_path)), nprocs=world, join=True)
     got = np.load(tmp_path / "sum.npy")
+    assert sorted(p.name for p in tmp_path.glob("sum*.npy")) == ["sum.npy"]          # one reporter
+    for r in range(world):
+        slowest, h = np.load(tmp_path / ("leg%d.npy" % r))
+        assert slowest == 10.0 + 5.0 * (world - 1) and h == sum(1.0 + k for k in range(world))
     want = oracle.f64_sketch(wl.sketch_seed(3), d, zeta, wl.gaussian(m, n, 11))
     # F64 partial sums: equal up to the rounding order of the final scaling (each rank scales its partial)
     assert np.allclose(got, want, rtol=0, atol=1e-12 * np.abs(want).max())
     assert np.linalg.norm(got - want) <= 1e-14 * np.linalg.norm(want)
+
+
+def test_collective_helpers_are_the_identity_without_a_process_group():
+    t = torch.arange(6, dtype=torch.float32)
+    assert all_reduce_sketch(t.clone()).equal(t)
+    assert max_over_ranks(3.25) == 3.25
