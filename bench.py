@@ -51,7 +51,7 @@ WORKLOADS = {
     "e1-d4096": (1 << 21, 1024, 4096, 4, 5),    # d/n = 4 of the paper's grid: 8 MiB sketch, beyond tensor memory
 }
 PAPER_GBPS = {"e1": (1 << 21) * 1024 * 4 / 7.11e-3 / 1e9}   # PAPER.md:322, H200 NVL (another machine: context)
-L2_RED_PAYLOAD_GBPS = 6000.0   # measured with sketch_red_probe on this pool's B200 (profiles/r01_red_probe.md)
+L2_RED_PAYLOAD_GBPS_R01 = 6000.0   # round-1 probe (profiles/r01_red_probe.md): context only; the bench measures its own
 VARIANTS = {"auto": 0, "flat_pair": 1, "flat_vec": 2, "smem": 3, "generic": 4, "tmem": 5, "small": 6}
 
 def ncu_traffic(workload, variant):
@@ -74,57 +74,120 @@ def measured_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons DURING the timed region (profiling recipe's clocks line)."""
+    """SM / memory clocks, board power and throttle reasons DURING the timed region (profiling recipe's clocks line), sampled
+    through NVML every ~5 ms in a thread of this process (an `nvidia-smi -lms 100` child process where NVML cannot be
+    loaded), so that every timed step gets the sample nearest to it and a change of regime inside a 50 ms region is visible."""
 
+    REASONS = ((0x8, "hw_slowdown"), (0x40, "hw_thermal_slowdown"), (0x20, "sw_thermal_slowdown"), (0x4, "sw_power_cap"),
+               (0x80, "hw_power_brake_slowdown"))
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,clocks.mem")
 
-    def __init__(self, index: int):
-        self.index, self.rows, self.proc = index, [], None
+    def __init__(self, index: int, uuid: str | None = None, period_s: float = 0.005):
+        self.index, self.uuid, self.period = index, uuid, period_s
+        self.rows = []            # (wall time, sm MHz, mem MHz, power W, [reasons])
+        self.sm_max, self.proc, self.th, self.stopflag, self.source = None, None, None, False, None
 
     def start(self):
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            try:
+                h = pynvml.nvmlDeviceGetHandleByUUID(self.uuid if isinstance(self.uuid, bytes) else str(self.uuid).encode()) if self.uuid else None
+            except Exception:
+                h = None
+            if h is None:
+                h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            reasons_fn = getattr(pynvml, "nvmlDeviceGetCurrentClocksEventReasons", None) or pynvml.nvmlDeviceGetCurrentClocksThrottleReasons
+
+            def pump():
+                while not self.stopflag:
+                    try:
+                        t = time.time()
+                        sm = float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM))
+                        mem = float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_MEM))
+                        pw = pynvml.nvmlDeviceGetPowerUsage(h) / 1e3
+                        bits = int(reasons_fn(h))
+                        self.rows.append((t, sm, mem, pw, [name for bit, name in self.REASONS if bits & bit]))
+                    except Exception:
+                        pass
+                    time.sleep(self.period)
+
+            self.source = "nvml, %.0f ms period" % (self.period * 1e3)
+            self.th = threading.Thread(target=pump, daemon=True)
+            self.th.start()
+            return
+        except Exception:
+            self.th = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
                                           "--format=csv,noheader,nounits", "-lms", "100"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
-            self.th = threading.Thread(target=self._pump, daemon=True)
+            self.source = "nvidia-smi -lms 100"
+            self.th = threading.Thread(target=self._pump_smi, daemon=True)
             self.th.start()
         except OSError:
             self.proc = None
 
-    def _pump(self):
+    def _pump_smi(self):
         for ln in self.proc.stdout:
-            self.rows.append((time.time(), ln.strip()))
-
-    def stop(self, t0: float, t1: float):
-        if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
-        sm, mx, reasons = [], None, set()
-        for ts, ln in self.rows:
             f = [x.strip() for x in ln.split(",")]
-            if len(f) < 9:
-                continue
             try:
-                clk, mxc = float(f[1]), float(f[2])
-            except ValueError:
+                sm, mx, pw, mem = float(f[1]), float(f[2]), float(f[3]), float(f[9])
+            except (ValueError, IndexError):
                 continue
-            mx = mxc
-            if t0 - 0.05 <= ts <= t1 + 0.15:
-                sm.append(clk)
-                for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
-                    if val.lower().startswith("active"):
-                        reasons.add(name)
-        if not sm:  # region shorter than the sampling period: use the closest samples
-            for ts, ln in self.rows[-3:]:
-                f = [x.strip() for x in ln.split(",")]
-                try:
-                    sm.append(float(f[1]))
-                except (ValueError, IndexError):
-                    pass
-        sm.sort()
-        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
+            self.sm_max = mx
+            names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+            self.rows.append((time.time(), sm, mem, pw, [nm for nm, val in zip(names, f[5:9]) if val.lower().startswith("active")]))
+
+    def halt(self):
+        time.sleep(0.02 if self.proc is None else 0.15)
+        self.stopflag = True
+        if self.proc:
+            self.proc.terminate()
+
+    def nearest(self, t: float):
+        if not self.rows:
+            return None
+        r = min(self.rows, key=lambda row: abs(row[0] - t))
+        return {"sm_mhz": r[1], "mem_mhz": r[2], "power_w": round(r[3], 1), "reasons": r[4], "dt_ms": round((r[0] - t) * 1e3, 1)}
+
+    def summary(self, t0: float, t1: float):
+        """Medians and the union of the reasons over the samples in [t0, t1] (the nearest ones when the window holds none)."""
+        if self.th is None and self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no NVML and no nvidia-smi"]}
+        rows = [r for r in self.rows if t0 <= r[0] <= t1]
+        if not rows:
+            rows = sorted(self.rows, key=lambda r: abs(r[0] - 0.5 * (t0 + t1)))[:3]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": ["no samples"], "samples": 0}
+
+        def med(k):
+            v = sorted(r[k] for r in rows)
+            return v[len(v) // 2]
+
+        return {"sm_mhz": med(1), "sm_max_mhz": self.sm_max, "reasons": sorted({x for r in rows for x in r[4]}), "samples": len(rows),
+                "sm_mhz_min": min(r[1] for r in rows), "mem_mhz": med(2), "mem_mhz_min": min(r[2] for r in rows),
+                "power_w": round(med(3), 1), "power_w_max": round(max(r[3] for r in rows), 1), "source": self.source}
+
+
+def step_stats(ms):
+    """mean / median / min / p90 of the per-step times and whether they fall into two regimes: the sorted series is cut at
+    its largest relative gap; a gap above 4 % with at least two steps (and 10 % of them) on either side is flagged."""
+    v = sorted(ms)
+    k = len(v)
+    out = {"mean": sum(v) / k, "median": v[k // 2] if k % 2 else 0.5 * (v[k // 2 - 1] + v[k // 2]), "min": v[0], "max": v[-1],
+           "p90": v[min(k - 1, int(0.9 * k))], "bimodal": False}
+    if k >= 4:
+        gap, cut = max(((v[i + 1] / v[i] - 1.0, i + 1) for i in range(k - 1)), key=lambda g: g[0])
+        need = max(2, k // 10)
+        if gap > 0.04 and cut >= need and k - cut >= need:
+            lo, hi = v[:cut], v[cut:]
+            out.update(bimodal=True, regimes={"fast_ms": sum(lo) / len(lo), "fast_steps": len(lo), "slow_ms": sum(hi) / len(hi),
+                                              "slow_steps": len(hi), "gap": gap})
+    return out
 
 
 def algorithmic_bytes(m, n, d, out_elem=2):
@@ -160,7 +223,8 @@ def run_reference(args):
         "impl": "reference", "metric": "sketch_A_read_GBps", "value": gbs, "unit": "GB/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "%s: SparseStack zeta=%d, m=%d, n=%d, d=%d, A FP32 N(0,1)" % (args.workload, zeta, m, n, d),
+        "config": {"workload": "%s (first %d of %d rows per step): SparseStack zeta=%d, m=%d, n=%d, d=%d, A FP32 N(0,1)"
+                               % (args.workload, sample_rows, m, zeta, m, n, d),
                    "sample": "first %d rows per step" % sample_rows},
         "cpu_baseline": {"value": gbs, "unit": "GB/s", "cores": threads, "kind": "oracle",
                          "sample": "oracle FP64 mode (row-chunk-private partials, %d threads) on %d of %d rows" % (threads, sample_rows, m)},
@@ -214,13 +278,92 @@ def cpu_baseline(workload, cpu_seconds=16.0):
 
 
 # ------------------------------------------------------------------------------------------- our arm
+def run_sustained(torch, step, ms_est, seconds, sampler, a_bytes):
+    """`seconds` (+15 %) of back-to-back steps with an event after every ~20 ms batch.  Returns the rate over the first half
+    second, the last second and the whole run, each with the clock / power samples of that window."""
+    per_batch = max(1, int(round(20.0 / max(ms_est, 1e-3))))
+    batches = max(4, int(seconds * 1e3 * 1.15 / (per_batch * ms_est)) + 1)
+    torch.cuda.synchronize()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(batches + 1)]
+    evs[0].record()
+    for b in range(batches):
+        for _ in range(per_batch):
+            step()
+        evs[b + 1].record()
+    torch.cuda.synchronize()
+    w1 = time.time()
+    t = [evs[0].elapsed_time(e) * 1e-3 for e in evs]            # seconds since the first event
+    total = t[-1]
+
+    def window(lo, hi):
+        idx = [i for i in range(1, len(t)) if t[i - 1] >= lo - 1e-9 and t[i] <= hi + 1e-9]
+        if not idx:
+            return None
+        dur = t[idx[-1]] - t[idx[0] - 1]
+        steps = len(idx) * per_batch
+        out = {"seconds": dur, "steps": steps, "ms_per_step": dur / steps * 1e3, "GBps": steps * a_bytes / dur / 1e9}
+        if sampler is not None:
+            out["clocks"] = sampler.summary(w1 - (total - t[idx[0] - 1]), w1 - (total - t[idx[-1]]))
+        return out
+
+    batch_ms = [(t[i] - t[i - 1]) / per_batch * 1e3 for i in range(1, len(t))]
+    return {"seconds": total, "steps": batches * per_batch, "steps_per_batch": per_batch,
+            "first_half_second": window(0.0, min(0.5, total / 2)), "last_second": window(max(0.0, total - 1.0), total), "whole": window(0.0, total),
+            "ms_per_step_by_batch": {"min": min(batch_ms), "median": sorted(batch_ms)[len(batch_ms) // 2], "max": max(batch_ms)},
+            "batch_stats": step_stats(batch_ms),
+            "note": "back-to-back complete sketches of the resident A, no L2 flush and no host work between them"}
+
+
+def measure_red_payload(torch, ss, dev, d, n, replicas, variant, f32=False):
+    """GB/s of RED payload the L2 atomic units take with the flat kernel's address pattern on a replicas x d x n sketch (FP16,
+    or FP32 with f32=True): the widest operand the row length allows (16 / 8 / 4 bytes per lane; one column or column pair
+    for flat_pair), 8 CTAs per SM, values from registers."""
+    eb = 4 if f32 else 2
+    if f32:
+        kind, vec = (5, 4) if n % 4 == 0 else (4, 2) if n % 2 == 0 else (3, 1)
+        if variant == "flat_pair":
+            kind, vec = 3, 1
+    else:
+        if n % 2:
+            return None
+        kind, vec = (2, 8) if n % 8 == 0 else (1, 4) if n % 4 == 0 else (0, 2)
+        if variant == "flat_pair":
+            kind, vec = 0, 2
+    grid = torch.cuda.get_device_properties(dev).multi_processor_count * 8
+    buf = torch.zeros(replicas * d * n * eb + 16, dtype=torch.uint8, device=dev)
+    ss.sketch_red_probe(buf, d, n, kind, replicas, grid, 200)
+    best = 0.0
+    for _ in range(3):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ops = ss.sketch_red_probe(buf, d, n, kind, replicas, grid, 2000)
+        e1.record()
+        torch.cuda.synchronize()
+        best = max(best, ops * vec * eb / (e0.elapsed_time(e1) * 1e-3) / 1e9)
+    return {"payload_GBps": best, "what": "%d-byte REDs into %d partial sketches of %d x %d %s, grid %d, best of 3 x 2000 rounds"
+                                          % (vec * eb, replicas, d, n, "FP32" if f32 else "FP16", grid)}
+
+
+def l2_red_from_capture(entry, ms_apply):
+    """L2-side reduction traffic of the dominant kernel from the committed ncu capture (profiles/ncu_traffic.json), turned
+    into rates with this run's time.  None where the capture holds no RED counters."""
+    if not entry or "lts_red_sectors" not in entry:
+        return None
+    sec = ms_apply * 1e-3
+    return {"lts__t_sectors_op_red_per_s": entry["lts_red_sectors"] / sec,
+            "smsp__inst_executed_op_global_red_per_s": entry.get("red_warp_inst", 0) / sec,
+            "l1tex_red_payload_GBps": entry.get("red_l1tex_bytes", 0) / sec / 1e9,
+            "per_launch": {k: entry[k] for k in ("lts_red_sectors", "red_warp_inst", "red_l1tex_bytes") if k in entry},
+            "source": "counters per launch from the committed capture %s, divided by this run's time" % entry["profile"]}
+
+
 def run_ours(args):
     import numpy as np
     import torch
 
     import paper_2606_20195_b200 as ss
     import workloads as wl
-    from paper_2606_20195_b200.sharding import shard_rows
+    from paper_2606_20195_b200.sharding import all_reduce_sketch, max_over_ranks, shard_rows
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -262,7 +405,7 @@ def run_ours(args):
         sk.apply_f16acc(A, out=out16, variant=vid, row_begin=row_begin, rows=m, replicas=args.replicas, hash_mode=args.hash_mode,
                         tmem_group_mode=args.tmem_group_mode)
         if dist is not None:
-            dist.all_reduce(out16)       # sum of the ranks' partial sketches: one more level of the FP16 hierarchy (sharding.py)
+            all_reduce_sketch(out16, dist)   # sum of the ranks' partial sketches: one more level of the FP16 hierarchy
 
     def step16():
         # complete sketch ("initialization, map generation, and application"): when the scatter
@@ -274,7 +417,7 @@ def run_ours(args):
     def step32():
         sk.apply_f32acc(A, out=out32, row_begin=row_begin, rows=m)
         if dist is not None:
-            dist.all_reduce(out32)
+            all_reduce_sketch(out32, dist)
 
     # like-for-like pairs (same privatisation on both sides): what FP16 PRECISION buys as opposed to what privatisation
     # buys (Eq. (5)): flat REDs on both sides, and tensor memory on both sides where the FP32 partial fits
@@ -323,17 +466,31 @@ def run_ours(args):
         barrier()
         w1 = time.time()
         ms = [a.elapsed_time(b) for a, b in evs]
-        total = torch.tensor([sum(ms)], dtype=torch.float64, device=dev)
-        if dist is not None:
-            dist.all_reduce(total, op=dist.ReduceOp.MAX)
-        return float(total.item()) / steps, ms, ss.sketch_launch_count() - l0, (w0, w1)
+        # wall-clock midpoint of every step: the device ran the steps back to back up to the synchronize that returned at w1
+        end = evs[0][0].elapsed_time(evs[-1][1])
+        mids = [w1 - (end - 0.5 * (evs[0][0].elapsed_time(a) + evs[0][0].elapsed_time(b))) * 1e-3 for a, b in evs]
+        total = max_over_ranks(sum(ms), dist, dev) if dist is not None else sum(ms)
+        return total / steps, ms, ss.sketch_launch_count() - l0, (w0, w1, mids)
 
-    sampler = ClockSampler(local)
+    try:
+        uuid = "GPU-" + str(torch.cuda.get_device_properties(local).uuid)
+    except Exception:
+        uuid = None
+    sampler = ClockSampler(local, uuid)
     if rank == 0:
         sampler.start()
-        time.sleep(0.3)
-    ms16, per16, launches16, (w0, w1) = timed(step16, args.steps, args.warmup)
-    clocks = sampler.stop(w0, w1) if rank == 0 else None
+        time.sleep(0.1)
+    ms16, per16, launches16, (w0, w1, mids16) = timed(step16, args.steps, args.warmup)
+    clocks = sampler.summary(w1 - sum(per16) * 1e-3 - 0.005, w1 + 0.005) if rank == 0 else None
+    per_step = [dict(ms=t, **(sampler.nearest(mid) or {})) for t, mid in zip(per16, mids16)] if rank == 0 else None
+
+    # sustained operation: >= args.sustained_seconds of back-to-back complete sketches (no flush, no host work in between),
+    # an event after every ~20 ms batch; the rate over the last second is what a caller streaming matrices for seconds gets
+    sustained = None
+    if args.sustained_seconds > 0 and not multi:
+        sustained = run_sustained(torch, step16, ms16, args.sustained_seconds, sampler if rank == 0 else None, m * n * 4)
+    if rank == 0:
+        sampler.halt()
     ms32, _, _, _ = timed(step32, max(2, args.steps // 2), 3)
     pairs = {}
     if not args.no_pairs and not multi:
@@ -345,6 +502,12 @@ def run_ours(args):
             a16, a32 = timed(tmem16, k2, 3)[0], timed(tmem32, k2, 3)[0]
             pairs["tmem"] = {"f16_ms": a16, "f32_ms": a32, "f16_over_f32": a32 / a16}
     ms16_apply, _, _, _ = timed(apply16, max(2, args.steps // 2), 3) if uses_packed else (ms16, None, None, None)
+
+    # second roofline term, measured in this run for the plans it bounds: result-discarding REDs with the flat kernel's
+    # address pattern on this workload's own d x n and replica count, values from registers, no A loads (sketch_red_probe)
+    red_probe = None
+    if plan16["variant"] in ("flat_vec", "flat_pair", "generic") and not multi:
+        red_probe = measure_red_payload(torch, ss, dev, d, n, max(1, int(plan16["replicas"])), plan16["variant"])
 
     # step a2 alone: how fast this GPU delivers A when it is only read (sketch_stream_probe; context for roofline.frac, whose
     # denominator is a COPY rate).  Plain 256-bit loads and k_tmem's TMA ring without consumers, median of 5 passes over A.
@@ -376,7 +539,7 @@ def run_ours(args):
                 sk.apply_f16acc_host(Ah, out_host=Bh, variant=vid, row_begin=row_begin, rows=m)
                 if dist is not None:
                     t = Bh.to(dev)
-                    dist.all_reduce(t)
+                    all_reduce_sketch(t, dist)
                     Bh.copy_(t)
 
             step_e2e()
@@ -386,16 +549,16 @@ def run_ours(args):
             for _ in range(ksteps):
                 step_e2e()
             barrier()
-            dt = torch.tensor([(time.perf_counter() - t0) / ksteps], dtype=torch.float64, device=dev)
+            dt = (time.perf_counter() - t0) / ksteps
             if dist is not None:
-                dist.all_reduce(dt, op=dist.ReduceOp.MAX)
-            e2e = {"value": world * m * n * 4 / float(dt.item()) / 1e9, "unit": "GB/s", "h2d_bytes_per_step": m * n * 4,
-                   "d2h_bytes_per_step": d * n * 2, "ms_per_step": float(dt.item()) * 1e3, "steps": ksteps,
+                dt = max_over_ranks(dt, dist, dev)
+            e2e = {"value": world * m * n * 4 / dt / 1e9, "unit": "GB/s", "h2d_bytes_per_step": m * n * 4,
+                   "d2h_bytes_per_step": d * n * 2, "ms_per_step": dt * 1e3, "steps": ksteps,
                    "api": "sketch_apply_f16acc_host (pinned host A, double-buffered 256 MiB H2D chunks)"}
             # the two entry points must agree on what they computed (same variant => same partial-sum tree up to RED order)
             chk = sk.apply_f16acc(A, variant=vid, row_begin=row_begin, rows=m)
             if dist is not None:
-                dist.all_reduce(chk)
+                all_reduce_sketch(chk, dist)
             diff = (chk.float().cpu() - Bh.float()).norm() / chk.float().norm().cpu()
             e2e["rel_diff_vs_device_path"] = float(diff)
             del Ah
@@ -431,10 +594,19 @@ def run_ours(args):
         "sketches_per_s": 1e3 / ms16,
         "contributions_per_s": zeta * m * n * world / (ms16 * 1e-3),
         "half2_updates_per_s": red_ops * world / (ms16 * 1e-3),
+        "half2_updates_note": "LOGICAL count: zeta*m*n/2 two-feature FP16 adds per sketch / time.  In the tensor-memory, shared-memory and "
+                              "small variants these adds happen on chip; what reaches the L2 atomic units is only the flush (l2_red below)",
+        "l2_red": l2_red_from_capture(traffic_src, ms16_apply),
+        "ms_per_step_stats": step_stats(per16),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm,
                      "traffic": traffic, "traffic_source": ("committed ncu capture %s (kernel %s)" % (traffic_src["profile"], traffic_src["kernel"])) if traffic_src else None,
                      "peak_source": peak_src,
                      "frac_of_nominal_8TBps": achieved / 8000.0,
+                     "frac_of_read_only_stream": (achieved / max(stream_probe.values())) if stream_probe else None,
+                     "frac_note": "`peak` is the driver's measured COPY rate (MEASURED_PEAKS.json), as the bench contract fixes; a kernel that only reads can "
+                                  "exceed it, so frac may read above 1.  frac_of_read_only_stream divides by the read-only streaming rate of the same A "
+                                  "measured in this run -- the actual ceiling of a complete sketch -- and stays at or below 1",
+                     "frac_sustained": (sustained["last_second"]["GBps"] * abytes / (m * n * 4) / hbm) if sustained else None,
                      "read_only_stream": dict(stream_probe, note="sketch_stream_probe over the same A in this run: what a kernel that only READS can reach; "
                                                                  "`peak` is a copy rate (read + write)") if stream_probe else None,
                      "algorithmic_bytes_per_launch": abytes,
@@ -447,13 +619,17 @@ def run_ours(args):
         "gpu_launches": int(launches16),
         "clocks": clocks,
         "per_step_ms": per16,
+        "per_step": per_step,
+        "sustained": sustained,
         "paper_context": "H200 NVL (PAPER.md:320-322): FP16 SS zeta=4 7.11 ms for 8 GiB (1.21 TB/s), up to 1.91x its FP32 scatter",
     }
     if plan16["variant"] in ("flat_vec", "flat_pair", "generic"):
         # a flat scatter is bound by the L2 atomic units, not by HBM: 2 bytes of RED payload per contribution
         payload = 2.0 * zeta * m * n / (ms16_apply * 1e-3) / 1e9
-        line["roofline"]["l2_atomic"] = {"achieved": payload, "peak": L2_RED_PAYLOAD_GBPS, "unit": "GB/s of RED payload",
-                                         "frac": payload / L2_RED_PAYLOAD_GBPS,
+        peak2 = red_probe["payload_GBps"] if red_probe else L2_RED_PAYLOAD_GBPS_R01
+        line["roofline"]["l2_atomic"] = {"achieved": payload, "peak": peak2, "unit": "GB/s of RED payload", "frac": payload / peak2,
+                                         "peak_source": ("sketch_red_probe in this run: %s" % red_probe["what"]) if red_probe
+                                                        else "round-1 probe (profiles/r01_red_probe.md)",
                                          "note": "second roofline term (SURVEY 8d): the slower of HBM and L2-atomic bounds this variant"}
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(args.workload)
@@ -633,6 +809,7 @@ def run_grid_study(args):
     peaks, peak_src = measured_peaks()
     hbm = float(peaks["hbm_gbs"])
     pts = []
+    red_rates = {}
     for m in ms_list:
         for kind in ("dense", "coordinate"):
             if kind == "dense":
@@ -654,17 +831,22 @@ def run_grid_study(args):
                           "fp16_variant": p16["variant"], "fp32_variant": p32["variant"], "fp16_GBps": m * n * 4 / t16 / 1e6,
                           "fp16_frac_hbm": (4 * m * n + 2 * d * n) / (t16 * 1e-3) / 1e9 / hbm,
                           "fp32_frac_hbm": (4 * m * n + 4 * d * n) / (t32 * 1e-3) / 1e9 / hbm}
-                    if p16["variant"] in ("flat_vec", "flat_pair"):
-                        pt["fp16_frac_l2_atomic"] = 2.0 * zeta * m * n / (t16 * 1e-3) / 1e9 / L2_RED_PAYLOAD_GBPS
-                    if p32["variant"] in ("flat_vec", "flat_pair"):
-                        pt["fp32_frac_l2_atomic"] = 4.0 * zeta * m * n / (t32 * 1e-3) / 1e9 / L2_RED_PAYLOAD_GBPS
+                    for key, pl, eb, tt in (("fp16", p16, 2.0, t16), ("fp32", p32, 4.0, t32)):
+                        if pl["variant"] in ("flat_vec", "flat_pair"):
+                            ck = (d, pl["replicas"], pl["variant"], key)
+                            if ck not in red_rates:       # the L2-atomic rate of this sketch shape, measured once per shape in this run
+                                pr = measure_red_payload(torch, ss, dev, d, n, max(1, pl["replicas"]), pl["variant"], f32=key == "fp32")
+                                red_rates[ck] = pr["payload_GBps"] if pr else None
+                            if red_rates[ck]:
+                                pt[key + "_frac_l2_atomic"] = eb * zeta * m * n / (tt * 1e-3) / 1e9 / red_rates[ck]
+                                pt[key + "_l2_atomic_peak_GBps"] = red_rates[ck]
                     pts.append(pt)
                     sk.close()
                 del o16, o32
             del A
             torch.cuda.empty_cache()
     print(json.dumps({"study": "paper timing grid (SURVEY 8f NEXT-2; PAPER.md:318-322)", "n": n, "hbm_peak_GBps": hbm, "peak_source": peak_src,
-                      "l2_atomic_payload_GBps": L2_RED_PAYLOAD_GBPS,
+                      "l2_atomic_payload_GBps": "sketch_red_probe on every (d, replicas, operand) of a flat point, in this run (fp*_l2_atomic_peak_GBps)",
                       "paper_context": "H200 NVL: FP16 SS 7.11 ms at m=2^21, d=2n, zeta=4 (PAPER.md:322); FP16 up to 1.91x its FP32 scatter (PAPER.md:320)",
                       "points": pts}))
     return 0
@@ -698,7 +880,7 @@ def run_coherence_study(args):
         for (r, z), sk in sks.items():
             e16, smin16 = eta(sk.apply_f16acc(U))
             e32, smin32 = eta(sk.apply_f32acc(U))
-            pts.append({"theta": theta, "coherence": mu, "d_over_n": r, "zeta": z, "eta_fp16": e16, "eta_fp32": e32,
+            pts.append({"theta": theta, "coherence": mu, "max_row_energy": mu * n / m, "d_over_n": r, "zeta": z, "eta_fp16": e16, "eta_fp32": e32,
                         "abs_diff": abs(e16 - e32), "sigma_min_fp16": smin16, "sigma_min_fp32": smin32,
                         "variant_fp16": sk.plan(n, f16=1)["variant"], "sqrt_n_over_d": (1.0 / r) ** 0.5})
         del U
@@ -795,6 +977,51 @@ def run_graph_study(args):
     return 0
 
 
+def run_sustained_study(args):
+    """Seconds-long operation (what a caller that streams one 16 GiB matrix after another sees): for c5, e1 and c2,
+    --sustained-seconds (default here: 4) of back-to-back complete FP16 sketches of the resident A, rate over the first half
+    second, the last second and the whole run, each with the SM / memory clocks, board power and throttle reasons NVML
+    reported in that window.  One JSON line; not the driver's bench line."""
+    import torch
+
+    import paper_2606_20195_b200 as ss
+    import workloads as wl
+
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    peaks, peak_src = measured_peaks()
+    hbm = float(peaks["hbm_gbs"])
+    seconds = args.sustained_seconds if args.sustained_seconds != 2.0 else 4.0
+    try:
+        uuid = "GPU-" + str(torch.cuda.get_device_properties(0).uuid)
+    except Exception:
+        uuid = None
+    sampler = ClockSampler(0, uuid)
+    sampler.start()
+    rows = []
+    for w in ([args.workload] if args.workload != "c5" else ["c5", "e1", "c2"]):
+        m, n, d, zeta, mseed = WORKLOADS[w]
+        sk = ss.Sketch(m, d, zeta, wl.sketch_seed(0))
+        A = wl.gaussian_device(m, n, mseed, dev)
+        out = torch.empty((d, n), dtype=torch.float16, device=dev)
+        step = lambda: sk.apply_f16acc(A, out=out)
+        ms = _time_ms(step, reps=5, warm=3)
+        time.sleep(1.0)                                  # start every workload from an idle board
+        r = run_sustained(torch, step, ms, seconds, sampler, m * n * 4)
+        scale = algorithmic_bytes(m, n, d, 2) / (m * n * 4)
+        for key in ("first_half_second", "last_second", "whole"):
+            if r[key]:
+                r[key]["frac_of_hbm_copy_peak"] = r[key]["GBps"] * scale / hbm
+        rows.append(dict(workload=w, variant=sk.plan(n)["variant"], cold_ms=ms, **r))
+        sk.close()
+        del A, out
+        torch.cuda.empty_cache()
+    sampler.halt()
+    print(json.dumps({"study": "sustained operation: back-to-back complete FP16 sketches for %.1f s per workload" % seconds,
+                      "hbm_peak_GBps": hbm, "peak_source": peak_src, "clock_source": sampler.source, "rows": rows}))
+    return 0
+
+
 def self_launch(args):
     """`python bench.py --gpus N` without a torchrun environment: re-run this very command under torch.distributed.run
     with N ranks on this node (one process per GPU, rendezvous on 127.0.0.1), so the line printed carries n_gpus = N only
@@ -827,7 +1054,7 @@ def main():
     ap.add_argument("--replicas", type=int, default=0)
     ap.add_argument("--hash-mode", type=int, default=0)
     ap.add_argument("--tmem-group-mode", type=int, default=0, help="sketch_opts_t.tmem_group_mode (tuning: 0 = auto)")
-    ap.add_argument("--study", default=None, choices=["range", "ls", "grid", "graph", "coherence", "replicas"],
+    ap.add_argument("--study", default=None, choices=["range", "ls", "grid", "graph", "coherence", "replicas", "sustained"],
                     help="extra reports: config-5 range / rounding study; GPU sketch-and-solve least squares; the paper's timing "
                          "grid (PAPER.md:318-322); launch-bound config 1 replayed from a CUDA graph; the U(theta) coherence sweep (PAPER.md:344-352); RN / SR / dither against the number of partial sketches")
     ap.add_argument("--grid", default="full", choices=["full", "quick"], help="--study grid / coherence: every point, or the corners / a small instance")
@@ -835,6 +1062,7 @@ def main():
     ap.add_argument("--no-pairs", action="store_true", help="skip the like-for-like flat/flat and tmem/tmem FP16-vs-FP32 timings")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-rows", type=int, default=1 << 21, help="rows per step of the reference arm's bounded sample")
+    ap.add_argument("--sustained-seconds", type=float, default=2.0, help="length of the back-to-back run behind `sustained` (0 = skip)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                           # timing rule: W >= 3
@@ -854,6 +1082,8 @@ def main():
         return run_coherence_study(args)
     if args.study == "replicas":
         return run_replica_study(args)
+    if args.study == "sustained":
+        return run_sustained_study(args)
     return run_ours(args)
 
 

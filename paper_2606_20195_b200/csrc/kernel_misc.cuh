@@ -102,7 +102,7 @@ __global__ void __launch_bounds__(kFlatThreads) k_red_probe(void* sketch, int32_
   }
 }
 
-// Candidates for sketches beyond tensor memory (VERDICT r01 item 6), same address pattern, no A loads:
+// Candidates for sketches beyond tensor memory (DESIGN.md section 5.4), same address pattern, no A loads:
 //   KIND 6  owner-exclusive plain read-modify-write in L2: ld.global.cg.v4 -> 4 x HADD2 -> st.global.cg.v4 (16 bytes per
 //           lane; hazards between lanes ignored -- an upper bound for any non-atomic L2-resident replica design)
 //   KIND 7/8  TMA bulk reduction: one elected lane per warp issues cp.reduce.async.bulk.global.shared::cta ... add of a

@@ -147,6 +147,20 @@ int ensure_scratch(sketch* s, void** buf, size_t* have, size_t want, bool captur
   return SKETCH_OK;
 }
 
+// Grid cap of the grid-stride helper kernels that take no handle (widen, conversion probe): 16 CTAs per SM of the
+// current device, the SM count asked once per device ordinal.
+int grid_cap_current_device() {
+  static std::atomic<int> sms[64];
+  int dev = 0, n = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 1024;
+  n = sms[dev].load(std::memory_order_relaxed);
+  if (n == 0) {
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return 1024;
+    sms[dev].store(n, std::memory_order_relaxed);
+  }
+  return n * 16;
+}
+
 inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 inline bool zeta_templated(int z) { return z == 1 || z == 2 || z == 4 || z == 8; }
 inline bool rot_ok(const sketch* s) { return zeta_templated(s->zeta) && s->d <= sk::smem_max_bucket(); }
@@ -1004,7 +1018,8 @@ int sketch_widen(const void* B16_dev, int64_t count, int is_bf16, float* out_dev
   if (count == 0) return SKETCH_OK;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
   int64_t blocks = (count + 255) / 256;
-  int grid = (int)(blocks < 148 * 16 ? blocks : 148 * 16);
+  const int cap = grid_cap_current_device();
+  int grid = (int)(blocks < cap ? blocks : cap);
   if (is_bf16) sk::k_widen<sk::OUT_BF16><<<grid, 256, 0, st>>>(static_cast<const uint16_t*>(B16_dev), count, out_dev);
   else sk::k_widen<sk::OUT_F16><<<grid, 256, 0, st>>>(static_cast<const uint16_t*>(B16_dev), count, out_dev);
   return launch_check("k_widen");
@@ -1077,7 +1092,8 @@ int sketch_convert_probe(const float* p_dev, const uint32_t* rbits_dev, int64_t 
   if ((kind == 1 || kind == 2 || kind >= 4) && !rbits_dev) return SKETCH_ERR_NULL;
   if (count == 0) return SKETCH_OK;
   int64_t blocks = (count + 255) / 256;
-  int grid = (int)(blocks < 148 * 16 ? blocks : 148 * 16);
+  const int cap = grid_cap_current_device();
+  int grid = (int)(blocks < cap ? blocks : cap);
   sk::k_convert_probe<<<grid, 256, 0, reinterpret_cast<cudaStream_t>(stream)>>>(p_dev, rbits_dev, count, kind, out_dev);
   return launch_check("k_convert_probe");
 }

@@ -5,8 +5,9 @@ computed ON THE HOST in FP64 (`evaluation.py`) from the GPU sketch and from the 
 Reading R19: GPU-FP32 must land within 1 % of the FP64-oracle value.  GPU-FP16 is order-dependent, so it
 is held to the one-sided rule "no further from the FP64 value than 1.01 x the oracle's own sequential-FP16 sketch, or
 within 1 % outright", plus Proposition 2's perturbation bound |eta(X) - eta(Y)| <= ||X - Y||_F.
-Sizes: config 2 in full; configs 3 and 4 with fewer rows (2^18) so that the single-threaded sequential-FP16 oracle
-finishes in seconds -- same n, d, zeta, generators and kernels (the tensor-memory variant, checked below).
+Sizes: config 2 in full; configs 3 and 4 both with fewer rows (2^18, the host generators) and at their full depth
+(m = 2^22 / 2^23, every d of config 4; device generators, the sequential-FP16 oracle column by column on all host threads)
+at the end of this file.
 """
 import numpy as np
 import pytest
@@ -203,4 +204,111 @@ def test_coherence_sweep_direct_sketch_of_U(ss, ratio):
         if theta == 1.0:   # the coordinate subspace: entries 0 / 1, every sum exact in FP16 -> the sketch itself is exact
             assert np.array_equal(D16, B64) and np.array_equal(D32, B64)
             assert np.linalg.matrix_rank(D16) == n                                  # zeta = 4 keeps full rank
-    assert mus[0] < 0.02 and abs(mus[-1] - 1.0) < 1e-6 and all(a <= b + 1e-9 for a, b in zip(mus, mus[1:]))   # coherence rises to 1
+    # Eq. (2): 1 <= mu <= m / n, the coordinate subspace attains the upper limit; it rises along theta
+    assert 1.0 <= mus[0] < 0.02 * m / n and abs(mus[-1] - m / n) < 1e-6 * m / n and all(a <= b + 1e-9 for a, b in zip(mus, mus[1:]))
+
+
+# ------------------------------------------------------------------------------------ configs 3 and 4 at their full depth
+# BASELINE.json configs[2] is m = 2^22 and configs[3] is m = 2^23 with d in {512, 1024, 2048}: the mean bucket depth
+# L = m zeta / d (2^14 .. 2^17 here) is what the FP16 accumulation error grows with, so the downstream
+# rule of the north star is asserted at these row counts too -- the same bytes on both sides (device generators, copied back
+# once), the FP64 oracle on all host threads, and the sequential-FP16 oracle column by column on all host threads (every
+# column keeps its ascending (i, j) order; columns are independent), so both halves of reading R19 are asserted.
+def _seq16_by_columns(seed, d, zeta, A):
+    from concurrent.futures import ThreadPoolExecutor
+
+    n = A.shape[1]
+    cols = [np.ascontiguousarray(A[:, c:c + 1]) for c in range(n)]
+    with ThreadPoolExecutor(max_workers=min(n, THREADS)) as ex:
+        outs = list(ex.map(lambda a: oracle.seq16_sketch(seed, d, zeta, a), cols))
+    return oracle.half_bits_to_f64(np.concatenate(outs, axis=1))
+
+
+_FULL = {}
+
+
+def _config3_full(alpha):
+    """(A on the device, the same bytes on the host, R of A = Q R) for one alpha; one alpha is kept at a time."""
+    if _FULL.get("c3_alpha") != alpha:
+        _FULL.clear()
+        Ad = wl.heavy_rows_device(1 << 22, 128, alpha, 3, torch.device("cuda"))
+        A = Ad.cpu().numpy()
+        _FULL.update(c3_alpha=alpha, c3=(Ad, A, ev.gram_R(np.array_split(A, 16), 128)))
+    return _FULL["c3"]
+
+
+@pytest.mark.parametrize("alpha", [0.0, 1.0])
+@pytest.mark.parametrize("zeta", [1, 4, 8])
+def test_config3_distortion_at_full_depth(ss, alpha, zeta):
+    m, n, d = 1 << 22, 128, 256
+    Ad, A, R = _config3_full(alpha)
+    seed = sketch_seed(30 + zeta)
+    sk = ss.Sketch(m, d, zeta, seed)
+    assert sk.plan(n)["variant"] == "tmem"
+    B64 = oracle.f64_sketch(seed, d, zeta, A, threads=THREADS)
+    Dseq = _seq16_by_columns(seed, d, zeta, A)
+    D16 = f16_to_f64(sk.apply_f16acc(Ad))
+    D32 = sk.apply_f32acc(Ad).cpu().numpy().astype(np.float64)
+    e64, eseq, e16, e32 = (ev.distortion(X, R) for X in (B64, Dseq, D16, D32))
+    print("config 3 full depth (L = %d) alpha=%.1f zeta=%d: eta f64 %.6f, gpu f32 %.6f, gpu f16 %.6f, oracle seq16 %.6f"
+          % (m * zeta // d, alpha, zeta, e64, e32, e16, eseq))
+    assert abs(e32 - e64) <= 0.01 * e64, (e32, e64)
+    assert abs(e16 - e64) <= max(1.01 * abs(eseq - e64), 0.01 * e64), (e16, eseq, e64)          # reading R19
+    for D, e in ((D16, e16), (D32, e32), (Dseq, eseq)):                                         # Prop. 2, Eq. (10)
+        pert = np.linalg.norm(ev.distortion_operator(D, R) - ev.distortion_operator(B64, R))
+        assert abs(e - e64) <= pert * (1 + 1e-9) + 1e-12, (e, e64, pert)
+    sk.close()
+
+
+def _config4_full():
+    """Config 4 at m = 2^23: (A, b on the device, A on the host, b column on the host, R_aug) with [A | b] = Q R_aug from a
+    streamed FP64 QR.  R_aug carries the FP64 QR solve (x_QR = R^-1 z with R_aug = [[R, z], [0, rho]], residual |rho|) and
+    the original-system residual of ANY x exactly: ||A x - b|| = ||R_aug [x; -1]||."""
+    if "c4" not in _FULL:
+        _FULL.clear()
+        m, n = 1 << 23, 256
+        Ad, bd, _ = wl.ls_system_device(m, n, 4, torch.device("cuda"))
+        A = Ad.cpu().numpy()
+        bcol = np.empty((m, 1), dtype=np.float32)
+        bcol[:, 0] = bd.cpu().numpy()
+        idx = np.array_split(np.arange(m), 64)
+        Raug = ev.gram_R((np.hstack([A[i[0]:i[-1] + 1], bcol[i[0]:i[-1] + 1]]) for i in idx), n + 1)
+        _FULL["c4"] = (Ad, bd, A, bcol, Raug)
+    return _FULL["c4"]
+
+
+@pytest.mark.parametrize("d", [512, 1024, 2048])
+def test_config4_residual_ratio_at_full_depth(ss, d):
+    m, n, zeta = 1 << 23, 256, 4
+    free, _ = torch.cuda.mem_get_info()
+    if free < m * n * 4 * 1.5 and "c4" not in _FULL:
+        pytest.skip("not enough device memory for config 4")
+    Ad, bd, A, bcol, Raug = _config4_full()
+    seed = sketch_seed(40 + d)
+    sk = ss.Sketch(m, d, zeta, seed)
+    assert sk.plan(n)["variant"] == "tmem"
+    r_ls = abs(float(Raug[n, n]))                                       # ||A x_QR - b||, the FP64 QR solve
+
+    def ratio(SA, Sb):
+        x = ev.sketch_and_solve(SA, Sb)
+        return float(np.linalg.norm(Raug @ np.concatenate([x, [-1.0]]))) / r_ls
+
+    Sb64 = oracle.f64_sketch(seed, d, zeta, bcol, threads=THREADS)[:, 0]
+    SA64 = oracle.f64_sketch(seed, d, zeta, A, threads=THREADS)
+    SAseq = _seq16_by_columns(seed, d, zeta, A)
+    # [A | b] in one pass, as the pipeline does (PAPER.md:356): A through the path under test, b in FP32 with the same map
+    SA16t, Sb32t = sk.apply_f16acc_with_rhs(Ad, bd)
+    SA32t, Sb32u = sk.apply_f32acc_with_rhs(Ad, bd)
+    SA16, SA32 = f16_to_f64(SA16t), SA32t.cpu().numpy().astype(np.float64)
+    Sb32, Sb32b = Sb32t.cpu().numpy().astype(np.float64), Sb32u.cpu().numpy().astype(np.float64)
+    assert ev.rel_fro(Sb32, Sb64) <= 1e-5 and ev.rel_fro(Sb32b, Sb64) <= 1e-5 and ev.rel_fro(SA32, SA64) <= 1e-5
+    q64, q32, q16, qseq = ratio(SA64, Sb64), ratio(SA32, Sb32b), ratio(SA16, Sb32), ratio(SAseq, Sb64)
+    print("config 4 full depth (L = %d) d=%d: residual ratio f64-sketch %.4f, gpu f32 %.4f, gpu f16 %.4f, oracle seq16 %.4f; relF f16 %.2e seq16 %.2e"
+          % (m * zeta // d, d, q64, q32, q16, qseq, ev.rel_fro(SA16, SA64), ev.rel_fro(SAseq, SA64)))
+    assert q64 >= 1.0 - 1e-9
+    assert abs(q32 - q64) <= 0.01 * q64, (q32, q64)
+    # reading R19: no further from the FP64 value than the sequential-FP16 oracle on the same bytes (or within 1 % outright)
+    assert q16 <= 1.01 * max(qseq, q64), (q16, qseq, q64)
+    sk.close()
+    if d == 2048:
+        _FULL.clear()

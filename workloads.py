@@ -223,7 +223,7 @@ def ls_paper_coherent_device(m: int, n: int, seed: int, device):
 def coherence_basis_device(m: int, n: int, thetas, seed: int, device):
     """The paper's coherence sweep (Sec. V-C): U(theta) = orth((1 - theta) Q_rand + theta [I_n 0]^T) with
     Q_rand an orthogonalised m x n Gaussian matrix.  Yields (theta, U FP32 [m, n] on `device`, coherence of Eq. (2) =
-    max_i ||U_i||^2).  The orthogonalisations run in FP64 (library QR), so U's columns are orthonormal to FP32 rounding;
+    (m / n) max_i ||U_i||^2, PAPER.md:67-72: between 1 and m / n, the coordinate subspace attains m / n).  The orthogonalisations run in FP64 (library QR), so U's columns are orthonormal to FP32 rounding;
     theta = 1 is the coordinate subspace [I_n 0]^T exactly."""
     import torch
 
@@ -239,6 +239,6 @@ def coherence_basis_device(m: int, n: int, thetas, seed: int, device):
             M[:n] += theta * torch.eye(n, dtype=torch.float64, device=device)
             U = torch.linalg.qr(M, mode="reduced")[0] if theta > 0.0 else Q
             del M
-        mu = float((U * U).sum(dim=1).max())
+        mu = float((U * U).sum(dim=1).max()) * m / n
         yield theta, U.to(torch.float32).contiguous(), mu    # library QR returns column-major factors
         del U
