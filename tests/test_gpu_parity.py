@@ -800,6 +800,15 @@ def test_full_size_sampled_columns(ss, name, m, n, d, zeta, variant):
     # FP16: never above 5e-2 (north star).  The flat kernel keeps one running sum per entry and replica, the
     # privatised kernels a two-level hierarchy; both stay far below at these depths (L = 2^14 .. 2^19)
     assert r16 <= 5e-2, r16
+    if name in ("c5", "e1"):
+        # the relative half of the north-star rule at the headline size: on two sampled columns (one column pair) the GPU's
+        # hierarchical FP16 sum is no further from FP64 than 1.5 x the oracle's own sequential-FP16 sum of the same bytes
+        two = [0, 1]
+        seq = oracle.half_bits_to_f64(_seq16_columns(seed, d, zeta, np.ascontiguousarray(Ac[:, two])))
+        ref = ev.rel_fro(seq, B[:, two])
+        r2 = ev.rel_fro(oracle.half_bits_to_f64(bits(got16[:, [cols[k] for k in two]])), B[:, two])
+        print("%s: relF on columns 0-1: gpu f16 %.3e, sequential-FP16 oracle %.3e" % (name, r2, ref))
+        assert cols[0] == 0 and cols[1] == 1 and r2 <= 1.5 * ref, (r2, ref)
 
 
 def _seq16_columns(seed, d, zeta, Ac, **kw):
