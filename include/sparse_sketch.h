@@ -264,8 +264,10 @@ int sketch_stream_probe(const void* src_dev, int64_t bytes, int32_t kind, int32_
  * cvt.rs.f16x2.f32 d, a, b, rbits with p in both sources: the half converted from b / from a;  6 / 7 = the library's SR pair
  * conversion with p and r24 in both halves (low / high half).  The two agree on the FP16 normal grid [2^-14, 65504) under a
  * fixed bit mapping and differ below 2^-14 (tests/test_gpu_modes.py, R22), so the library's SR kernels use the
- * hardware instruction exactly where both values of a pair lie on that grid and the integer rule 1 everywhere else: kinds
- * 6 / 7 equal kind 1 bit for bit on every input.  rbits_dev may be NULL for kinds 0 and 3.  Device pointers. */
+ * hardware instruction exactly where both values of a pair lie on that grid and the integer rule 1 everywhere else.  Shown
+ * by test, not proved: kinds 6 / 7 equal kind 1 on 2^30 random samples (tests/test_gpu_modes.py) and equal the oracle's
+ * SR16 on 2^26 random samples plus every FP32 value in windows around 2^-14, 65504, 65520, 2^-24 and 2^-25
+ * (tests/test_gpu_add_paths.py).  rbits_dev may be NULL for kinds 0 and 3.  Device pointers. */
 int sketch_convert_probe(const float* p_dev, const uint32_t* rbits_dev, int64_t count, int32_t kind, uint16_t* out_dev,
                          void* stream);
 
