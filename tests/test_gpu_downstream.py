@@ -218,8 +218,9 @@ def _seq16_by_columns(seed, d, zeta, A):
     from concurrent.futures import ThreadPoolExecutor
 
     n = A.shape[1]
-    cols = [np.ascontiguousarray(A[:, c:c + 1]) for c in range(n)]
-    with ThreadPoolExecutor(max_workers=min(n, THREADS)) as ex:
+    w = max(1, n // THREADS)          # a few columns per call: the call hashes every (row, block) once for all of them
+    cols = [np.ascontiguousarray(A[:, c:c + w]) for c in range(0, n, w)]
+    with ThreadPoolExecutor(max_workers=min(len(cols), THREADS)) as ex:
         outs = list(ex.map(lambda a: oracle.seq16_sketch(seed, d, zeta, a), cols))
     return oracle.half_bits_to_f64(np.concatenate(outs, axis=1))
 

@@ -70,7 +70,9 @@ def test_gpu_pipeline_against_host_fp64_solve_and_oracle_sketch(ss, family, rati
         # and the one-call form returns the same vector
         # (a second 16-bit sketch differs from the first in the order of its flush, and x moves with it: compare residuals)
         x_one = lstsq.sketch_and_solve(sk, Ad, bd, prec).cpu().numpy().astype(np.float64)
-        assert abs(res(x_one) - out[prec]) <= (1e-3 if prec == "f32" else 2e-2) * out[prec]
+        # FP16 (u = 2^-11): 2 %; bfloat16 (u = 2^-8: eight times coarser, +3 % residual over FP32 on its own) moves
+        # by a few % from one flush order to the next (the order of the atomic adds is free): 8 %
+        assert abs(res(x_one) - out[prec]) <= {"f32": 1e-3, "f16": 2e-2, "bf16": 8e-2}[prec] * out[prec], prec
     print("%s d/n=%d: residual/||b|| f64-sketch %.5f, gpu f32 %.5f, f16 %.5f (%+.3f %% over f32), bf16 %.5f (%+.2f %%)"
           % (family, ratio, r64, out["f32"], out["f16"], 100 * (out["f16"] / out["f32"] - 1), out["bf16"], 100 * (out["bf16"] / out["f32"] - 1)))
     # FP32 pipeline within 1 % of the FP64 oracle sketch solved on the host (BASELINE.json north_star's downstream rule)
