@@ -219,9 +219,10 @@ def _seq16_by_columns(seed, d, zeta, A):
 
     n = A.shape[1]
     w = max(1, n // THREADS)          # a few columns per call: the call hashes every (row, block) once for all of them
-    cols = [np.ascontiguousarray(A[:, c:c + w]) for c in range(0, n, w)]
-    with ThreadPoolExecutor(max_workers=min(len(cols), THREADS)) as ex:
-        outs = list(ex.map(lambda a: oracle.seq16_sketch(seed, d, zeta, a), cols))
+    starts = list(range(0, n, w))
+    # the strided gather of a column chunk out of a multi-GiB row-major A is itself seconds of work: it runs in the worker too
+    with ThreadPoolExecutor(max_workers=min(len(starts), THREADS)) as ex:
+        outs = list(ex.map(lambda c: oracle.seq16_sketch(seed, d, zeta, np.ascontiguousarray(A[:, c:c + w])), starts))
     return oracle.half_bits_to_f64(np.concatenate(outs, axis=1))
 
 
